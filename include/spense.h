@@ -1,0 +1,156 @@
+/*
+ * spense.h -- C ABI of the B200-native Spense hybrid sparse-dense FP8 GLU-MLP library.
+ *
+ * Method: arxiv/paper_2606_10445 (SpenseGPT).  Citations are lines of the paper text.
+ *   - 2:4 semi-structured sparsity along K, ||W[i,4j:4j+4]||_0 <= 2          Eq. 1
+ *   - compressed storage = non-zero values + a few position bits per group
+ *   - Spense format: one contiguous 2:4 region + one contiguous dense region   Sec. 3.2
+ *   - output-split (W_gate, W_up) and input-split (W_down, sparse then dense
+ *     accumulated into the same output)                                        Sec. 3.2
+ *   - intermediate-index permutation P, MLP(X) unchanged                       Eq. 4
+ *   - dense indices placed last
+ *
+ * Conventions
+ *   - Layout is PyTorch's: Y = X W^T, W in R^{N x K} row-major, X in R^{M x K}.
+ *     H = hidden size, I = intermediate size, I_dense = number of dense intermediate indices,
+ *     I_s = I - I_dense.  In PERMUTED intermediate order the sparse region is [0, I_s) and the dense
+ *     region is [I_s, I).  W_gate, W_up are [I, H]; W_down is [H, I].
+ *   - FP8 is E4M3 (FN: bias 7, no inf, NaN = 0x7F/0xFF, max 448), stored as uint8_t.
+ *     Weights carry one fp32 scale per matrix, activations one fp32 scale per token.
+ *   - Pointers prefixed d_ are DEVICE pointers, h_ are HOST pointers.  The library allocates no
+ *     device memory: the caller owns every buffer; size queries say how large they must be.
+ *     Device pointers must be 128-byte aligned.
+ *   - Every call returns a status (0 = SPENSE_OK, negative = error).  Nothing throws, aborts or
+ *     prints.  Argument errors are detected on the host before any launch.
+ *   - All GPU work is enqueued on the caller's stream.  GEMM calls never synchronise.
+ *     spense_pack synchronises the stream once to read back its validation word.
+ *   - There is NO CPU fallback: on a device that is not sm_100 the calls return SPENSE_ERR_ARCH.
+ */
+#ifndef SPENSE_H_
+#define SPENSE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct CUstream_st* spense_stream_t; /* == cudaStream_t */
+
+enum {
+  SPENSE_OK = 0,
+  SPENSE_ERR_ARG = -1,              /* null pointer, M < 1, bad enum */
+  SPENSE_ERR_ALIGN = -2,            /* pointer not aligned as required */
+  SPENSE_ERR_SHAPE = -3,            /* H, I, I_dense not multiples of 128, I_dense > I, too large */
+  SPENSE_ERR_BUFFER_TOO_SMALL = -4, /* blob_bytes / ws_bytes below the size query */
+  SPENSE_ERR_NOT_2_4 = -5,          /* a sparse-region group of 4 has > 2 non-zero bytes */
+  SPENSE_ERR_NAN_WEIGHT = -6,       /* a weight byte is 0x7F / 0xFF */
+  SPENSE_ERR_BAD_PERM = -7,         /* perm is not a bijection of [0, I) */
+  SPENSE_ERR_ARCH = -8,             /* current device is not sm_100 */
+  SPENSE_ERR_CUDA = -9,             /* a CUDA call failed; cudaGetLastError is preserved */
+  SPENSE_ERR_BAD_BLOB = -10         /* blob header does not match the shape / version */
+};
+
+enum { SPENSE_F32 = 0, SPENSE_BF16 = 1 };          /* y_dtype */
+enum { SPENSE_PER_TENSOR = 0, SPENSE_PER_ROW = 1 }; /* quantise mode */
+
+typedef struct {
+  int32_t H;       /* hidden size,        multiple of 128 */
+  int32_t I;       /* intermediate size,  multiple of 128 */
+  int32_t I_dense; /* dense intermediate indices (last block after permutation), multiple of 128, 0..I */
+} spense_shape_t;
+
+/* Canonical (layout-independent) result of the pack, DEVICE arrays owned by the caller; any member
+ * may be NULL (not written).  Encoding (readings Q6/Q7):
+ *   vals[r, 2g], vals[r, 2g+1] = the bytes at positions i0 < i1 of group g of row r;
+ *   nibble(g) = i0 | i1 << 2;  meta byte b of a row = nibble(2b) | nibble(2b+1) << 4.            */
+typedef struct {
+  int32_t* perm;         /* [I]         new -> old (as used)                                  */
+  uint8_t* gate_sp_val;  /* [I_s, H/2]                                                         */
+  uint8_t* up_sp_val;    /* [I_s, H/2]                                                         */
+  uint8_t* gate_sp_meta; /* [I_s, H/8]                                                         */
+  uint8_t* up_sp_meta;   /* [I_s, H/8]                                                         */
+  uint8_t* gate_dn;      /* [I_dense, H]                                                       */
+  uint8_t* up_dn;        /* [I_dense, H]                                                       */
+  uint8_t* down_sp_val;  /* [H, I_s/2]                                                         */
+  uint8_t* down_sp_meta; /* [H, I_s/8]                                                         */
+  uint8_t* down_dn;      /* [H, I_dense]                                                       */
+} spense_canon_t;
+
+int spense_version(void);
+const char* spense_strerror(int status);
+
+/* Host helper (Sec. 3.3.1; reading Q9): the permutation that moves the chosen dense
+ * indices to the back, keeping ascending original order inside both regions.  h_perm[new] = old. */
+int spense_perm_from_dense_idx(int32_t I, const int32_t* h_dense_idx, int32_t n_dense, int32_t* h_perm);
+
+/* Bytes of the packed blob and of the pack workspace for a shape. */
+int spense_pack_sizes(const spense_shape_t* shape, size_t* blob_bytes, size_t* workspace_bytes);
+
+/* spense_pack -- "When deploying, we rearrange the indices for kernel efficiency" (Fig. 4,
+ * PAPER.md:137): P1 permute the intermediate indices (rows of W_gate / W_up, columns of W_down),
+ * P2 validate Eq. 1 on the sparse region and compress it to values + 2-bit position metadata
+ * (PAPER.md:74), P3 re-tile everything into the opaque device blob the GEMM kernels stream.
+ *   d_wgate, d_wup [I, H], d_wdown [H, I]: E4M3 bytes in ORIGINAL index order (read only).
+ *   h_w_scale[3]: per-tensor fp32 scales of gate, up, down (host), stored in the blob header.
+ *   d_perm [I] (device) new -> old, or NULL for the identity.
+ *   d_blob / blob_bytes: output; canon: optional canonical outputs (NULL or members NULL).
+ *   d_ws / ws_bytes: scratch.  h_err_where[4] (nullable, host): on NOT_2_4 / NAN_WEIGHT receives
+ *   {matrix (0 gate, 1 up, 2 down), row, group, number of offending groups}; first offender in
+ *   (matrix, row, group) order.  On error the blob contents are undefined.                       */
+int spense_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8_t* d_wup,
+                const uint8_t* d_wdown, const float* h_w_scale, const int32_t* d_perm, void* d_blob,
+                size_t blob_bytes, const spense_canon_t* canon, void* d_ws, size_t ws_bytes,
+                int64_t* h_err_where, spense_stream_t stream);
+
+/* Workspace for the GEMM calls at up to M tokens (split-K partial tiles + flags).  The workspace
+ * must be initialised ONCE with spense_workspace_init before its first use (it is left clean by
+ * every successful call).  One workspace must not be used by two streams concurrently.          */
+int spense_workspace_size(const spense_shape_t* shape, int32_t M, size_t* bytes);
+int spense_workspace_init(void* d_ws, size_t ws_bytes, spense_stream_t stream);
+
+/* spense_gate_up -- output-split Spense GEMM for W_gate and W_up fused with the GLU
+ * (Eq. 4, sigma = SiLU) and FP8 re-quantisation for the down projection:
+ *   g = (X Wg^T) * s_x[m] * s_gate,  u = (X Wu^T) * s_x[m] * s_up,  h = g / (1 + exp(-g)) * u,
+ *   hq[m, j] = E4M3_rne_sat(h[m, j] / s_h[m])          (j in PERMUTED intermediate order)
+ * Row tiles j < I_s run on 2:4 sparse tensor-core MMAs, the others on dense MMAs.
+ *   d_x [M, H] E4M3, d_sx [M] fp32; d_sh: requant scale, sh_stride 0 = one scalar, 1 = per token.
+ *   d_hq [M, I] E4M3 out; d_h_f32 nullable [M, I] fp32 out (h before re-quantisation, for parity). */
+int spense_gate_up(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_x,
+                   const float* d_sx, int32_t M, const float* d_sh, int32_t sh_stride, uint8_t* d_hq,
+                   float* d_h_f32, void* d_ws, size_t ws_bytes, spense_stream_t stream);
+
+/* spense_down -- input-split Spense GEMM: the K loop runs the sparse K range
+ * [0, I_s) on sparse MMAs and continues with the dense range [I_s, I) into the SAME accumulator:
+ *   y[m, n] = (sum_k hq[m, k] * Wd[n, k]) * s_h[m] * s_down.
+ *   d_hq [M, I] E4M3 (permuted order); d_y [M, H] fp32 (SPENSE_F32) or bf16 (SPENSE_BF16).        */
+int spense_down(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_hq, const float* d_sh,
+                int32_t sh_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, size_t ws_bytes,
+                spense_stream_t stream);
+
+/* spense_mlp -- the whole layer: gate_up then down on one stream (programmatic dependent launch).
+ *   d_hq_scratch [M, I] E4M3 scratch; d_h_f32 nullable as in spense_gate_up.                     */
+int spense_mlp(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx,
+               int32_t M, const float* d_sh, int32_t sh_stride, uint8_t* d_hq_scratch, float* d_h_f32,
+               void* d_y, int32_t y_dtype, void* d_ws, size_t ws_bytes, spense_stream_t stream);
+
+/* spense_mlp_host -- same, with HOST activations and results: copies h_x [M, H], h_sx [M], h_sh
+ * (1 or M floats) to the device staging buffers, runs spense_mlp, copies y back to h_y and
+ * synchronises the stream.  Staging (device): d_x [M, H], d_scales [2*M] fp32, d_hq_scratch [M, I],
+ * d_y [M, H] of y_dtype.  Host buffers should be pinned for full copy bandwidth.                 */
+int spense_mlp_host(const spense_shape_t* shape, const void* d_blob, const uint8_t* h_x, const float* h_sx,
+                    int32_t M, const float* h_sh, int32_t sh_stride, void* h_y, int32_t y_dtype,
+                    uint8_t* d_x, float* d_scales, uint8_t* d_hq_scratch, void* d_y, void* d_ws,
+                    size_t ws_bytes, spense_stream_t stream);
+
+/* spense_quantize_e4m3 -- helper (reading Q5): scale = amax / 448 (1 if amax == 0), per tensor or
+ * per row; out = E4M3_rne_sat(in / scale) with an IEEE fp32 division.  d_scales: 1 or rows floats.
+ * d_ws needs 4 bytes * (rows + 1). Bit-exact against the oracle.                                  */
+int spense_quantize_e4m3(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out,
+                         float* d_scales, void* d_ws, size_t ws_bytes, spense_stream_t stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPENSE_H_ */

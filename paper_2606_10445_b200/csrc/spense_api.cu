@@ -1,0 +1,404 @@
+// C-ABI entry points of libspense (include/spense.h): argument checking, stream-K schedule,
+// tensor-map creation and launches.  No device allocation, no synchronisation in the GEMM calls.
+#include <cudaTypedefs.h>
+
+#include <cstring>
+#include <mutex>
+#include <vector>
+
+#include "spense_internal.cuh"
+
+namespace spense {
+namespace {
+
+int g_num_sms = 0;
+int g_arch_ok = -1;
+PFN_cuTensorMapEncodeTiled_v12000 g_encode = nullptr;
+
+int check_device() {
+  if (g_arch_ok >= 0) return g_arch_ok ? SPENSE_OK : SPENSE_ERR_ARCH;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return SPENSE_ERR_CUDA;
+  int major = 0, minor = 0;
+  cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+  cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev);
+  cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
+  g_arch_ok = (major == 10 && minor == 0) ? 1 : 0;
+  if (g_arch_ok) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) {
+      g_arch_ok = -1;
+      return SPENSE_ERR_CUDA;
+    }
+    g_encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(fn);
+  }
+  return g_arch_ok ? SPENSE_OK : SPENSE_ERR_ARCH;
+}
+
+int check_shape(const spense_shape_t* s) {
+  if (!s) return SPENSE_ERR_ARG;
+  if (s->H < 128 || s->I < 128 || s->I_dense < 0 || s->I_dense > s->I) return SPENSE_ERR_SHAPE;
+  if (s->H % 128 || s->I % 128 || s->I_dense % 128) return SPENSE_ERR_SHAPE;
+  if (s->H > (1 << 20) || s->I > (1 << 20)) return SPENSE_ERR_SHAPE;
+  return SPENSE_OK;
+}
+
+bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+int n_pad_of(int M) { int n = (M + 15) / 16 * 16; return n > 128 ? 128 : n; }
+
+size_t ws_bytes_for(int n_pad, int spans) { return kFlagBytes + (size_t)spans * 2 * n_pad * 128 * sizeof(float); }
+
+// ---- stream-K schedule: cut the stage sequence into n_spans spans of (nearly) equal bytes.
+struct Schedule {
+  int mode, H, I, I_d, n_pad, sms;
+  int n_spans;
+  int span_begin[kMaxSpans + 1];
+};
+std::mutex g_sched_mu;
+std::vector<Schedule> g_sched;
+
+const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms) {
+  std::lock_guard<std::mutex> lk(g_sched_mu);
+  for (const Schedule& s : g_sched)
+    if (s.mode == mode && s.H == g.H && s.I == g.I && s.I_d == g.I_d && s.n_pad == n_pad && s.sms == sms) return s;
+  Schedule sc = {};
+  sc.mode = mode; sc.H = g.H; sc.I = g.I; sc.I_d = g.I_d; sc.n_pad = n_pad; sc.sms = sms;
+  // cost of a stage = bytes it moves into shared memory
+  const double cs = kSparseStageBytes + 2.0 * n_pad * 128, cd = kDenseStageBytes + 1.0 * n_pad * 128;
+  std::vector<double> cost;
+  if (mode == 0) {
+    cost.insert(cost.end(), (size_t)g.gu_tiles_sparse * g.gu_ns, cs);
+    cost.insert(cost.end(), (size_t)(g.gu_tiles - g.gu_tiles_sparse) * g.gu_nd, cd);
+  } else {
+    for (int t = 0; t < g.dn_tiles; ++t) {
+      cost.insert(cost.end(), (size_t)g.dn_ns, cs);
+      cost.insert(cost.end(), (size_t)g.dn_nd, cd);
+    }
+  }
+  const int total = (int)cost.size();
+  int spans = sms < kMaxSpans ? sms : kMaxSpans;
+  if (spans > total) spans = total;
+  double sum = 0;
+  for (double c : cost) sum += c;
+  sc.n_spans = spans;
+  double acc = 0;
+  int s = 0;
+  sc.span_begin[0] = 0;
+  for (int i = 1; i < spans; ++i) {
+    const double target = sum * i / spans;
+    while (s < total && acc + 0.5 * cost[s] < target) acc += cost[s++];
+    int b = s;
+    if (b <= sc.span_begin[i - 1]) b = sc.span_begin[i - 1] + 1;     // every span owns >= 1 stage
+    if (b > total - (spans - i)) b = total - (spans - i);
+    while (s < b) acc += cost[s++];
+    sc.span_begin[i] = b;
+  }
+  sc.span_begin[spans] = total;
+  g_sched.push_back(sc);
+  return g_sched.back();
+}
+
+int make_tmap(CUtensorMap* map, const uint8_t* base, int K, int rows, int box_rows) {
+  cuuint64_t dims[2] = {(cuuint64_t)K, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)K};
+  cuuint32_t box[2] = {128u, (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1u, 1u};
+  CUresult r = g_encode(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint8_t*>(base), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? SPENSE_OK : SPENSE_ERR_CUDA;
+}
+
+// header cache: one D2H copy per (blob pointer), so the GEMM calls stay asynchronous afterwards
+struct HeaderEntry { const void* p; BlobHeader h; };
+std::mutex g_hdr_mu;
+std::vector<HeaderEntry> g_hdr_cache;
+
+void forget_header(const void* d_blob) {
+  std::lock_guard<std::mutex> lk(g_hdr_mu);
+  for (size_t i = 0; i < g_hdr_cache.size(); ++i)
+    if (g_hdr_cache[i].p == d_blob) { g_hdr_cache.erase(g_hdr_cache.begin() + i); break; }
+}
+
+int read_header(const void* d_blob, const spense_shape_t* shape, BlobHeader* out) {
+  std::mutex& mu = g_hdr_mu;
+  std::vector<HeaderEntry>& cache = g_hdr_cache;
+  using Entry = HeaderEntry;
+  {
+    std::lock_guard<std::mutex> lk(mu);
+    for (const Entry& e : cache)
+      if (e.p == d_blob && e.h.H == shape->H && e.h.I == shape->I && e.h.I_dense == shape->I_dense) { *out = e.h; return SPENSE_OK; }
+  }
+  BlobHeader h;
+  if (cudaMemcpy(&h, d_blob, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess) return SPENSE_ERR_CUDA;
+  if (h.magic != kBlobMagic || h.version != kBlobVersion || h.H != shape->H || h.I != shape->I || h.I_dense != shape->I_dense)
+    return SPENSE_ERR_BAD_BLOB;
+  std::lock_guard<std::mutex> lk(mu);
+  for (Entry& e : cache)
+    if (e.p == d_blob) { e.h = h; *out = h; return SPENSE_OK; }
+  cache.push_back({d_blob, h});
+  *out = h;
+  return SPENSE_OK;
+}
+
+void fill_common(GemmParams& p, const Schedule& sc, int M, int n_pad, void* d_ws) {
+  p.n_spans = sc.n_spans;
+  std::memcpy(p.span_begin, sc.span_begin, sizeof(int) * (sc.n_spans + 1));
+  p.M = M;
+  p.n_pad = n_pad;
+  p.slot_bytes = kSparseStageBytes + 2 * n_pad * 128;
+  int stages = (232448 - 1024 - 256) / p.slot_bytes;
+  p.num_stages = stages > 8 ? 8 : stages;
+  p.acc_stride = n_pad <= 32 ? 32 : (n_pad <= 64 ? 64 : 128);
+  p.num_acc_bufs = n_pad <= 64 ? 2 : 1;
+  p.flags = reinterpret_cast<int*>(d_ws);
+  p.partials = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes);
+}
+
+int gate_up_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_x,
+                 const float* d_sx, int32_t M, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32,
+                 void* d_ws, bool pdl, cudaStream_t stream) {
+  const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
+  for (int m0 = 0; m0 < M; m0 += 128) {
+    const int Mb = (M - m0) < 128 ? (M - m0) : 128;
+    const int n_pad = n_pad_of(Mb);
+    const Schedule& sc = get_schedule(0, g, n_pad, g_num_sms);
+    GemmParams p = {};
+    fill_common(p, sc, Mb, n_pad, d_ws);
+    p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.gate_up_off;
+    p.mode = 0;
+    p.num_tiles = g.gu_tiles; p.tiles_sparse = g.gu_tiles_sparse;
+    p.ns = g.gu_ns; p.nd = g.gu_nd; p.dense_k0 = 0;
+    p.s_act = d_sx + m0;
+    p.s_h = d_sh + (size_t)m0 * sh_stride; p.sh_stride = sh_stride;
+    p.w_scale0 = hdr.w_scale[0]; p.w_scale1 = hdr.w_scale[1];
+    p.hq = d_hq + (size_t)m0 * g.I;
+    p.h_f32 = d_h_f32 ? d_h_f32 + (size_t)m0 * g.I : nullptr;
+    p.ld_out = g.I; p.out_rows = g.I;
+    CUtensorMap tm;
+    int st = make_tmap(&tm, d_x + (size_t)m0 * g.H, g.H, Mb, n_pad);
+    if (st) return st;
+    st = launch_gemm(p, tm, pdl, stream);
+    if (st) return st;
+  }
+  return SPENSE_OK;
+}
+
+int down_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_hq,
+              const float* d_sh, int32_t sh_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, bool pdl,
+              cudaStream_t stream) {
+  const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
+  const size_t esz = y_dtype == SPENSE_F32 ? 4 : 2;
+  for (int m0 = 0; m0 < M; m0 += 128) {
+    const int Mb = (M - m0) < 128 ? (M - m0) : 128;
+    const int n_pad = n_pad_of(Mb);
+    const Schedule& sc = get_schedule(1, g, n_pad, g_num_sms);
+    GemmParams p = {};
+    fill_common(p, sc, Mb, n_pad, d_ws);
+    p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off;
+    p.mode = 1;
+    p.num_tiles = g.dn_tiles; p.tiles_sparse = 0;
+    p.ns = g.dn_ns; p.nd = g.dn_nd; p.dense_k0 = g.I_s;
+    p.s_act = d_sh + (size_t)m0 * sh_stride; p.sh_stride = sh_stride;
+    p.w_scale0 = hdr.w_scale[2]; p.w_scale1 = hdr.w_scale[2];
+    p.y = reinterpret_cast<uint8_t*>(d_y) + (size_t)m0 * g.H * esz;
+    p.y_dtype = y_dtype;
+    p.ld_out = g.H; p.out_rows = g.H;
+    CUtensorMap tm;
+    int st = make_tmap(&tm, d_hq + (size_t)m0 * g.I, g.I, Mb, n_pad);
+    if (st) return st;
+    st = launch_gemm(p, tm, pdl, stream);
+    if (st) return st;
+  }
+  return SPENSE_OK;
+}
+
+int check_ws(const spense_shape_t* shape, int M, const void* d_ws, size_t ws_bytes) {
+  if (!d_ws) return SPENSE_ERR_ARG;
+  if (!aligned(d_ws, 128)) return SPENSE_ERR_ALIGN;
+  size_t need = 0;
+  int st = spense_workspace_size(shape, M, &need);
+  if (st) return st;
+  return ws_bytes < need ? SPENSE_ERR_BUFFER_TOO_SMALL : SPENSE_OK;
+}
+
+}  // namespace
+}  // namespace spense
+
+using namespace spense;
+
+extern "C" {
+
+int spense_version(void) { return 100 * 0 + 1; }
+
+const char* spense_strerror(int status) {
+  switch (status) {
+    case SPENSE_OK: return "ok";
+    case SPENSE_ERR_ARG: return "invalid argument";
+    case SPENSE_ERR_ALIGN: return "pointer not sufficiently aligned";
+    case SPENSE_ERR_SHAPE: return "unsupported shape (H, I, I_dense must be multiples of 128, I_dense <= I)";
+    case SPENSE_ERR_BUFFER_TOO_SMALL: return "buffer smaller than the size query";
+    case SPENSE_ERR_NOT_2_4: return "a group of 4 in the sparse region has more than 2 non-zeros";
+    case SPENSE_ERR_NAN_WEIGHT: return "NaN weight byte (0x7F / 0xFF)";
+    case SPENSE_ERR_BAD_PERM: return "perm is not a bijection";
+    case SPENSE_ERR_ARCH: return "device is not sm_100 (no fallback path exists)";
+    case SPENSE_ERR_CUDA: return "CUDA error";
+    case SPENSE_ERR_BAD_BLOB: return "blob header does not match";
+    default: return "unknown status";
+  }
+}
+
+int spense_perm_from_dense_idx(int32_t I, const int32_t* h_dense_idx, int32_t n_dense, int32_t* h_perm) {
+  if (I < 0 || n_dense < 0 || n_dense > I || !h_perm || (n_dense && !h_dense_idx)) return SPENSE_ERR_ARG;
+  std::vector<uint8_t> is_dense((size_t)I, 0);
+  for (int i = 0; i < n_dense; ++i) {
+    const int d = h_dense_idx[i];
+    if (d < 0 || d >= I || is_dense[d]) return SPENSE_ERR_ARG;
+    is_dense[d] = 1;
+  }
+  int w = 0;
+  for (int i = 0; i < I; ++i) if (!is_dense[i]) h_perm[w++] = i;
+  for (int i = 0; i < I; ++i) if (is_dense[i]) h_perm[w++] = i;
+  return SPENSE_OK;
+}
+
+int spense_pack_sizes(const spense_shape_t* shape, size_t* blob_bytes, size_t* workspace_bytes) {
+  int st = check_shape(shape);
+  if (st) return st;
+  const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
+  if (blob_bytes) *blob_bytes = g.total_bytes;
+  if (workspace_bytes) *workspace_bytes = 128 + (size_t)shape->I * sizeof(int);
+  return SPENSE_OK;
+}
+
+int spense_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8_t* d_wup, const uint8_t* d_wdown,
+                const float* h_w_scale, const int32_t* d_perm, void* d_blob, size_t blob_bytes,
+                const spense_canon_t* canon, void* d_ws, size_t ws_bytes, int64_t* h_err_where, spense_stream_t stream) {
+  int st = check_shape(shape);
+  if (st) return st;
+  if (!d_wgate || !d_wup || !d_wdown || !h_w_scale || !d_blob || !d_ws) return SPENSE_ERR_ARG;
+  if (!aligned(d_wgate, 128) || !aligned(d_wup, 128) || !aligned(d_wdown, 128) || !aligned(d_blob, 128) ||
+      !aligned(d_ws, 128) || (d_perm && !aligned(d_perm, 4)))
+    return SPENSE_ERR_ALIGN;
+  size_t need_blob = 0, need_ws = 0;
+  spense_pack_sizes(shape, &need_blob, &need_ws);
+  if (blob_bytes < need_blob || ws_bytes < need_ws) return SPENSE_ERR_BUFFER_TOO_SMALL;
+  st = check_device();
+  if (st) return st;
+  forget_header(d_blob);
+  return launch_pack(shape, d_wgate, d_wup, d_wdown, h_w_scale, d_perm, d_blob, canon, d_ws, h_err_where,
+                     reinterpret_cast<cudaStream_t>(stream));
+}
+
+int spense_workspace_size(const spense_shape_t* shape, int32_t M, size_t* bytes) {
+  int st = check_shape(shape);
+  if (st) return st;
+  if (M < 1 || !bytes) return SPENSE_ERR_ARG;
+  *bytes = ws_bytes_for(n_pad_of(M), kMaxSpans);
+  return SPENSE_OK;
+}
+
+int spense_workspace_init(void* d_ws, size_t ws_bytes, spense_stream_t stream) {
+  if (!d_ws) return SPENSE_ERR_ARG;
+  if (ws_bytes < (size_t)kFlagBytes) return SPENSE_ERR_BUFFER_TOO_SMALL;
+  return cudaMemsetAsync(d_ws, 0, kFlagBytes, reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;
+}
+
+int spense_gate_up(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx, int32_t M,
+                   const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32, void* d_ws, size_t ws_bytes,
+                   spense_stream_t stream) {
+  int st = check_shape(shape);
+  if (st) return st;
+  if (!d_blob || !d_x || !d_sx || !d_sh || !d_hq || M < 1 || (sh_stride != 0 && sh_stride != 1)) return SPENSE_ERR_ARG;
+  if (!aligned(d_blob, 128) || !aligned(d_x, 128) || !aligned(d_hq, 16) || !aligned(d_sx, 4) || !aligned(d_sh, 4) ||
+      (d_h_f32 && !aligned(d_h_f32, 16)))
+    return SPENSE_ERR_ALIGN;
+  st = check_ws(shape, M, d_ws, ws_bytes);
+  if (st) return st;
+  st = check_device();
+  if (st) return st;
+  BlobHeader hdr;
+  st = read_header(d_blob, shape, &hdr);
+  if (st) return st;
+  return gate_up_impl(shape, hdr, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq, d_h_f32, d_ws, false,
+                      reinterpret_cast<cudaStream_t>(stream));
+}
+
+int spense_down(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_hq, const float* d_sh, int32_t sh_stride,
+                int32_t M, void* d_y, int32_t y_dtype, void* d_ws, size_t ws_bytes, spense_stream_t stream) {
+  int st = check_shape(shape);
+  if (st) return st;
+  if (!d_blob || !d_hq || !d_sh || !d_y || M < 1 || (sh_stride != 0 && sh_stride != 1) ||
+      (y_dtype != SPENSE_F32 && y_dtype != SPENSE_BF16))
+    return SPENSE_ERR_ARG;
+  if (!aligned(d_blob, 128) || !aligned(d_hq, 128) || !aligned(d_y, 16) || !aligned(d_sh, 4)) return SPENSE_ERR_ALIGN;
+  st = check_ws(shape, M, d_ws, ws_bytes);
+  if (st) return st;
+  st = check_device();
+  if (st) return st;
+  BlobHeader hdr;
+  st = read_header(d_blob, shape, &hdr);
+  if (st) return st;
+  return down_impl(shape, hdr, d_blob, d_hq, d_sh, sh_stride, M, d_y, y_dtype, d_ws, false,
+                   reinterpret_cast<cudaStream_t>(stream));
+}
+
+int spense_mlp(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx, int32_t M,
+               const float* d_sh, int32_t sh_stride, uint8_t* d_hq_scratch, float* d_h_f32, void* d_y, int32_t y_dtype,
+               void* d_ws, size_t ws_bytes, spense_stream_t stream) {
+  int st = check_shape(shape);
+  if (st) return st;
+  if (!d_blob || !d_x || !d_sx || !d_sh || !d_hq_scratch || !d_y || M < 1 || (sh_stride != 0 && sh_stride != 1) ||
+      (y_dtype != SPENSE_F32 && y_dtype != SPENSE_BF16))
+    return SPENSE_ERR_ARG;
+  if (!aligned(d_blob, 128) || !aligned(d_x, 128) || !aligned(d_hq_scratch, 128) || !aligned(d_y, 16) ||
+      !aligned(d_sx, 4) || !aligned(d_sh, 4) || (d_h_f32 && !aligned(d_h_f32, 16)))
+    return SPENSE_ERR_ALIGN;
+  st = check_ws(shape, M, d_ws, ws_bytes);
+  if (st) return st;
+  st = check_device();
+  if (st) return st;
+  BlobHeader hdr;
+  st = read_header(d_blob, shape, &hdr);
+  if (st) return st;
+  cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
+  st = gate_up_impl(shape, hdr, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq_scratch, d_h_f32, d_ws, true, s);
+  if (st) return st;
+  return down_impl(shape, hdr, d_blob, d_hq_scratch, d_sh, sh_stride, M, d_y, y_dtype, d_ws, true, s);
+}
+
+int spense_mlp_host(const spense_shape_t* shape, const void* d_blob, const uint8_t* h_x, const float* h_sx, int32_t M,
+                    const float* h_sh, int32_t sh_stride, void* h_y, int32_t y_dtype, uint8_t* d_x, float* d_scales,
+                    uint8_t* d_hq_scratch, void* d_y, void* d_ws, size_t ws_bytes, spense_stream_t stream) {
+  int st = check_shape(shape);
+  if (st) return st;
+  if (!h_x || !h_sx || !h_sh || !h_y || !d_x || !d_scales || M < 1 || (sh_stride != 0 && sh_stride != 1) ||
+      (y_dtype != SPENSE_F32 && y_dtype != SPENSE_BF16))
+    return SPENSE_ERR_ARG;
+  cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
+  const size_t n_sh = sh_stride ? (size_t)M : 1;
+  if (cudaMemcpyAsync(d_x, h_x, (size_t)M * shape->H, cudaMemcpyHostToDevice, s) != cudaSuccess) return SPENSE_ERR_CUDA;
+  if (cudaMemcpyAsync(d_scales, h_sx, (size_t)M * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) return SPENSE_ERR_CUDA;
+  if (cudaMemcpyAsync(d_scales + M, h_sh, n_sh * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) return SPENSE_ERR_CUDA;
+  st = spense_mlp(shape, d_blob, d_x, d_scales, M, d_scales + M, sh_stride, d_hq_scratch, nullptr, d_y, y_dtype, d_ws,
+                  ws_bytes, stream);
+  if (st) return st;
+  const size_t esz = y_dtype == SPENSE_F32 ? 4 : 2;
+  if (cudaMemcpyAsync(h_y, d_y, (size_t)M * shape->H * esz, cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPENSE_ERR_CUDA;
+  return cudaStreamSynchronize(s) == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;
+}
+
+int spense_quantize_e4m3(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out, float* d_scales,
+                         void* d_ws, size_t ws_bytes, spense_stream_t stream) {
+  if (!d_in || !d_out || !d_scales || !d_ws || rows < 1 || cols < 1 || (mode != SPENSE_PER_TENSOR && mode != SPENSE_PER_ROW))
+    return SPENSE_ERR_ARG;
+  if (rows > 0x7FFFFFFF) return SPENSE_ERR_SHAPE;
+  if (ws_bytes < (size_t)(rows + 1) * 4) return SPENSE_ERR_BUFFER_TOO_SMALL;
+  int st = check_device();
+  if (st) return st;
+  return launch_quantize(d_in, rows, cols, mode, d_out, d_scales, d_ws, reinterpret_cast<cudaStream_t>(stream));
+}
+
+}  // extern "C"

@@ -1,0 +1,235 @@
+// Internal definitions shared by the CUDA translation units of libspense (never installed).
+// Blob geometry, kernel parameter blocks and the sm_100a PTX wrappers (mbarrier, TMA / bulk copy,
+// tcgen05 MMA / TMEM).  Nothing here is shared with oracle/.
+#pragma once
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "spense.h"
+
+namespace spense {
+
+// ------------------------------------------------------------------------------------------
+// Blob geometry.  The blob is a sequence of pipeline-stage images: each stage is EXACTLY the bytes
+// one cp.async.bulk drops into shared memory (128B-swizzle pre-applied), so the producer streams
+// perfectly sequential DRAM pages with one bulk copy per stage and needs no tensor map for weights.
+//
+//   "pair tile" = two 128-row A operands (MMA-M = 128 each) that share one B (activation) tile:
+//       gate_up : rows [128t, 128t+128) of W_gate and of W_up       (tile t < I_s/128 sparse, else dense)
+//       down    : rows [256t, 256t+128) and [256t+128, 256t+256) of W_down (sparse K range, then dense)
+//   sparse stage (K = 256 logical): A0 vals 16 KB | A1 vals 16 KB | A0 meta 4 KB | A1 meta 4 KB
+//   dense  stage (K = 128)        : A0 16 KB | A1 16 KB
+//   vals / dense images: 128 rows x 128 B, canonical K-major SWIZZLE_128B (8-row x 128 B atoms,
+//       16-byte chunk index XOR (row & 7)).  meta image: 2 atoms of 128 rows x 16 B, row-major
+//       (one atom = K 128 logical = what one tcgen05.cp.128x128b moves to TMEM).
+// ------------------------------------------------------------------------------------------
+constexpr int kTileRows = 128;
+constexpr int kSparseStageK = 256;           // logical K per sparse stage
+constexpr int kDenseStageK = 128;            // K per dense stage
+constexpr int kOperandBytes = 128 * 128;     // one 128 x 128 B operand image
+constexpr int kMetaBytes = 128 * 32;         // one operand's metadata per sparse stage
+constexpr int kSparseStageBytes = 2 * kOperandBytes + 2 * kMetaBytes;  // 40960
+constexpr int kDenseStageBytes = 2 * kOperandBytes;                    // 32768
+constexpr int kBlobHeaderBytes = 1024;
+constexpr uint32_t kBlobMagic = 0x53504E53u;  // "SNPS"
+constexpr int kBlobVersion = 1;
+constexpr int kMaxSpans = 160;
+constexpr int kFlagBytes = 4096;
+
+struct BlobHeader {
+  uint32_t magic;
+  int32_t version;
+  int32_t H, I, I_dense;
+  float w_scale[3];
+  uint64_t gate_up_off, down_off, total_bytes;
+};
+
+struct Geometry {
+  int H, I, I_d, I_s;
+  // gate_up
+  int gu_tiles, gu_tiles_sparse;   // I/128, I_s/128
+  int gu_ns, gu_nd;                // stages per sparse tile: ceil(H/256); per dense tile: H/128
+  // down
+  int dn_tiles;                    // ceil(H/256)
+  int dn_ns, dn_nd;                // ceil(I_s/256), I_d/128
+  size_t gate_up_off, down_off, total_bytes;
+};
+
+__host__ __device__ inline Geometry make_geometry(int H, int I, int I_d) {
+  Geometry g;
+  g.H = H; g.I = I; g.I_d = I_d; g.I_s = I - I_d;
+  g.gu_tiles = I / 128;
+  g.gu_tiles_sparse = g.I_s / 128;
+  g.gu_ns = (H + 255) / 256;
+  g.gu_nd = H / 128;
+  g.dn_tiles = (H + 255) / 256;
+  g.dn_ns = (g.I_s + 255) / 256;
+  g.dn_nd = I_d / 128;
+  g.gate_up_off = kBlobHeaderBytes;
+  size_t gu = (size_t)g.gu_tiles_sparse * g.gu_ns * kSparseStageBytes +
+              (size_t)(g.gu_tiles - g.gu_tiles_sparse) * g.gu_nd * kDenseStageBytes;
+  g.down_off = g.gate_up_off + gu;
+  size_t dn = (size_t)g.dn_tiles * ((size_t)g.dn_ns * kSparseStageBytes + (size_t)g.dn_nd * kDenseStageBytes);
+  g.total_bytes = g.down_off + dn;
+  return g;
+}
+
+// byte offset of element (row r, byte column b) inside one 128 x 128 B SWIZZLE_128B operand image
+__host__ __device__ inline int sw128_offset(int r, int b) {
+  return (r >> 3) * 1024 + (r & 7) * 128 + ((((b >> 4) ^ (r & 7)) & 7) << 4) + (b & 15);
+}
+
+// ------------------------------------------------------------------------------------------
+// GEMM kernel parameters.  One kernel serves gate_up (mode 0) and down (mode 1): a byte-balanced
+// stream-K walk over the linear sequence of stages; span i = stages [span_begin[i], span_begin[i+1]).
+// ------------------------------------------------------------------------------------------
+struct GemmParams {
+  const uint8_t* section;   // first stage image of this matrix family
+  int mode;                 // 0 gate_up, 1 down
+  int num_tiles, tiles_sparse;
+  int ns, nd;               // mode 0: stages of a sparse tile / of a dense tile; mode 1: per tile both
+  int dense_k0;             // K byte offset of the first dense stage in the B operand (mode 1: I_s)
+  int n_spans;
+  int M, n_pad;             // tokens in this launch, padded to 16
+  int num_stages, slot_bytes, acc_stride, num_acc_bufs;
+  // epilogue
+  const float* s_act;       // mode 0: s_x [M]; mode 1: s_h (stride sh_stride)
+  const float* s_h;         // mode 0: requant scale
+  int sh_stride;
+  float w_scale0, w_scale1; // mode 0: gate, up; mode 1: down, down
+  uint8_t* hq;              // mode 0 out [M, ld_out]
+  float* h_f32;             // mode 0 optional out
+  void* y;                  // mode 1 out [M, ld_out]
+  int y_dtype;
+  int ld_out;               // I (mode 0) or H (mode 1)
+  int out_rows;             // valid output columns (I or H) for masking padded tiles
+  float* partials;          // workspace: n_spans slots of 2 * n_pad * 128 floats
+  int* flags;               // workspace: n_spans ints, zero between launches
+  int span_begin[kMaxSpans + 1];
+};
+
+// ------------------------------------------------------------------------------------------
+// PTX wrappers
+// ------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "WAIT_LOOP:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra WAIT_DONE;\n\t"
+      "bra WAIT_LOOP;\n\t"
+      "WAIT_DONE:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void fence_barrier_init() {
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+__device__ __forceinline__ uint64_t policy_evict_first() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ uint64_t policy_evict_last() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+// 1-D bulk copy global -> shared, completion on an mbarrier (SASS: UBLKCP)
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t pol) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+      ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+}
+// 2-D tiled TMA load (SASS: UTMALDG)
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar, uint64_t pol) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint "
+      "[%0], [%1, {%2, %3}], [%4], %5;"
+      ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map) {
+  asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
+}
+
+// TMEM
+__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+// tcgen05.commit: arrive on an mbarrier when all prior tcgen05 ops of this thread are done
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// dense FP8 MMA: D[tmem] (+)= A[smem] * B[smem]^T   (SASS: UTCQMMA)
+__device__ __forceinline__ void mma_f8_dense(uint32_t d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+}
+// 2:4 sparse FP8 MMA: A is compressed (K = 64 logical per instruction), metadata in TMEM at `e`
+__device__ __forceinline__ void mma_f8_sparse(uint32_t d, uint64_t adesc, uint64_t bdesc, uint32_t e, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %5, 0;\n\t"
+      "tcgen05.mma.sp.cta_group::1.kind::f8f6f4 [%0], %1, %2, [%3], %4, p;\n\t}"
+      ::"r"(d), "l"(adesc), "l"(bdesc), "r"(e), "r"(idesc), "r"(acc) : "memory");
+}
+// shared -> TMEM copy of one metadata atom: 128 lanes x 128 bit (SASS: UTCCP)
+__device__ __forceinline__ void tc_cp_128x128b(uint32_t taddr, uint64_t sdesc) {
+  asm volatile("tcgen05.cp.cta_group::1.128x128b [%0], %1;" ::"r"(taddr), "l"(sdesc) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+      : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// shared-memory matrix descriptor (sm_100 "version 1")
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes, uint32_t layout) {
+  return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16) |
+         ((uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32) | (1ull << 46) | ((uint64_t)layout << 61);
+}
+constexpr uint32_t kLayoutSW128 = 2, kLayoutNone = 0;
+
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
+#endif  // __CUDACC__
+
+// host-side entry points implemented in the .cu files
+int launch_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8_t* d_wup, const uint8_t* d_wdown,
+                const float* h_w_scale, const int32_t* d_perm, void* d_blob, const spense_canon_t* canon, void* d_ws,
+                int64_t* h_err_where, cudaStream_t stream);
+int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, bool pdl, cudaStream_t stream);
+int launch_quantize(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out, float* d_scales,
+                    void* d_ws, cudaStream_t stream);
+
+}  // namespace spense

@@ -1,0 +1,228 @@
+"""Thin ctypes binding of libspense.so (include/spense.h).  Argument marshalling only: every step
+of the path runs in the CUDA kernels.  PyTorch supplies device memory and streams, nothing else.
+
+There is no fallback: if the shared library is missing or a call fails, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, c_char_p, c_float, c_int, c_int32, c_int64, c_size_t, c_void_p
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libspense.so")
+
+SPENSE_F32, SPENSE_BF16 = 0, 1
+SPENSE_PER_TENSOR, SPENSE_PER_ROW = 0, 1
+
+STATUS = {0: "SPENSE_OK", -1: "SPENSE_ERR_ARG", -2: "SPENSE_ERR_ALIGN", -3: "SPENSE_ERR_SHAPE",
+          -4: "SPENSE_ERR_BUFFER_TOO_SMALL", -5: "SPENSE_ERR_NOT_2_4", -6: "SPENSE_ERR_NAN_WEIGHT",
+          -7: "SPENSE_ERR_BAD_PERM", -8: "SPENSE_ERR_ARCH", -9: "SPENSE_ERR_CUDA", -10: "SPENSE_ERR_BAD_BLOB"}
+
+EXPORTS = ["spense_version", "spense_strerror", "spense_perm_from_dense_idx", "spense_pack_sizes", "spense_pack",
+           "spense_workspace_size", "spense_workspace_init", "spense_gate_up", "spense_down", "spense_mlp",
+           "spense_mlp_host", "spense_quantize_e4m3"]
+
+
+class SpenseError(RuntimeError):
+    def __init__(self, status: int, where=None):
+        self.status = status
+        self.code = STATUS.get(status, str(status))
+        self.where = where
+        super().__init__(f"{self.code} ({lib().spense_strerror(status).decode()})" + (f" at {where}" if where else ""))
+
+
+class Shape(ctypes.Structure):
+    _fields_ = [("H", c_int32), ("I", c_int32), ("I_dense", c_int32)]
+
+
+class Canon(ctypes.Structure):
+    _fields_ = [(n, c_void_p) for n in ("perm", "gate_sp_val", "up_sp_val", "gate_sp_meta", "up_sp_meta",
+                                        "gate_dn", "up_dn", "down_sp_val", "down_sp_meta", "down_dn")]
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libspense.so (built in-tree by paper_2606_10445_b200.build).  Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} not found: build it with `python -m paper_2606_10445_b200.build` "
+                               "(there is no CPU / PyTorch fallback for the Spense path)")
+        L = ctypes.CDLL(LIB_PATH)
+        L.spense_version.restype = c_int
+        L.spense_strerror.restype = c_char_p
+        L.spense_strerror.argtypes = [c_int]
+        L.spense_perm_from_dense_idx.argtypes = [c_int32, POINTER(c_int32), c_int32, POINTER(c_int32)]
+        L.spense_pack_sizes.argtypes = [POINTER(Shape), POINTER(c_size_t), POINTER(c_size_t)]
+        L.spense_pack.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, POINTER(c_float), c_void_p, c_void_p,
+                                  c_size_t, POINTER(Canon), c_void_p, c_size_t, POINTER(c_int64), c_void_p]
+        L.spense_workspace_size.argtypes = [POINTER(Shape), c_int32, POINTER(c_size_t)]
+        L.spense_workspace_init.argtypes = [c_void_p, c_size_t, c_void_p]
+        L.spense_gate_up.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_int32, c_void_p, c_int32,
+                                     c_void_p, c_void_p, c_void_p, c_size_t, c_void_p]
+        L.spense_down.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_void_p, c_int32,
+                                  c_void_p, c_size_t, c_void_p]
+        L.spense_mlp.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_int32, c_void_p, c_int32, c_void_p,
+                                 c_void_p, c_void_p, c_int32, c_void_p, c_size_t, c_void_p]
+        L.spense_mlp_host.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_int32, c_void_p, c_int32,
+                                      c_void_p, c_int32, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_size_t,
+                                      c_void_p]
+        L.spense_quantize_e4m3.argtypes = [c_void_p, c_int64, c_int64, c_int32, c_void_p, c_void_p, c_void_p,
+                                           c_size_t, c_void_p]
+        for name in EXPORTS:
+            if name not in ("spense_strerror",):
+                getattr(L, name).restype = c_int
+        _lib = L
+    return _lib
+
+
+def _check(st: int, where=None):
+    if st != 0:
+        raise SpenseError(st, where)
+
+
+def _ptr(t):
+    return None if t is None else c_void_p(t.data_ptr())
+
+
+def _stream():
+    return c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dev(t: torch.Tensor, dtype=None):
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError(f"expected dtype {dtype}, got {t.dtype}")
+    return t
+
+
+def spense_version() -> int:
+    return lib().spense_version()
+
+
+def spense_perm_from_dense_idx(I: int, dense_idx) -> torch.Tensor:
+    idx = (c_int32 * len(dense_idx))(*[int(v) for v in dense_idx])
+    out = (c_int32 * I)()
+    _check(lib().spense_perm_from_dense_idx(I, idx, len(dense_idx), out))
+    return torch.tensor(list(out), dtype=torch.int32)
+
+
+def spense_pack_sizes(H: int, I: int, I_dense: int):
+    b, w = c_size_t(), c_size_t()
+    _check(lib().spense_pack_sizes(ctypes.byref(Shape(H, I, I_dense)), ctypes.byref(b), ctypes.byref(w)))
+    return b.value, w.value
+
+
+class PackedLayer:
+    """A packed Spense layer: the opaque device blob plus (optionally) the canonical arrays."""
+
+    def __init__(self, H, I, I_dense, blob, canon=None):
+        self.H, self.I, self.I_dense, self.blob, self.canon = H, I, I_dense, blob, canon
+        self.shape = Shape(H, I, I_dense)
+
+
+def spense_pack(wgate, wup, wdown, w_scale, perm, I_dense: int, want_canon: bool = False) -> PackedLayer:
+    """wgate, wup uint8 [I, H]; wdown uint8 [H, I] (CUDA, original index order); perm int32 [I] or None."""
+    _dev(wgate, torch.uint8), _dev(wup, torch.uint8), _dev(wdown, torch.uint8)
+    I, H = wgate.shape
+    dev = wgate.device
+    blob_bytes, ws_bytes = spense_pack_sizes(H, I, I_dense)
+    blob = torch.empty(blob_bytes, dtype=torch.uint8, device=dev)
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
+    I_s = I - I_dense
+    canon, cstruct = None, None
+    if want_canon:
+        e = lambda *s: torch.empty(*s, dtype=torch.uint8, device=dev)
+        canon = dict(perm=torch.empty(I, dtype=torch.int32, device=dev),
+                     gate_sp_val=e(I_s, H // 2), up_sp_val=e(I_s, H // 2), gate_sp_meta=e(I_s, H // 8),
+                     up_sp_meta=e(I_s, H // 8), gate_dn=e(I_dense, H), up_dn=e(I_dense, H),
+                     down_sp_val=e(H, I_s // 2), down_sp_meta=e(H, I_s // 8), down_dn=e(H, I_dense))
+        cstruct = Canon(**{k: v.data_ptr() for k, v in canon.items()})
+    if perm is not None:
+        _dev(perm, torch.int32)
+    scales = (c_float * 3)(*[float(s) for s in w_scale])
+    where = (c_int64 * 4)(-1, -1, -1, -1)
+    st = lib().spense_pack(ctypes.byref(Shape(H, I, I_dense)), _ptr(wgate), _ptr(wup), _ptr(wdown), scales, _ptr(perm),
+                           _ptr(blob), blob_bytes, ctypes.byref(cstruct) if cstruct else None, _ptr(ws), ws_bytes,
+                           where, _stream())
+    _check(st, tuple(where))
+    return PackedLayer(H, I, I_dense, blob, canon)
+
+
+def spense_workspace_size(H: int, I: int, I_dense: int, M: int) -> int:
+    b = c_size_t()
+    _check(lib().spense_workspace_size(ctypes.byref(Shape(H, I, I_dense)), M, ctypes.byref(b)))
+    return b.value
+
+
+def spense_workspace(layer: PackedLayer, M: int) -> torch.Tensor:
+    """Allocate and initialise a GEMM workspace for up to M tokens."""
+    n = spense_workspace_size(layer.H, layer.I, layer.I_dense, M)
+    ws = torch.empty(n, dtype=torch.uint8, device=layer.blob.device)
+    _check(lib().spense_workspace_init(_ptr(ws), n, _stream()))
+    return ws
+
+
+def spense_gate_up(layer: PackedLayer, x, s_x, s_h, ws, hq=None, h_f32=None):
+    """x uint8 [M, H], s_x f32 [M], s_h f32 [1] or [M].  Returns hq uint8 [M, I] (permuted order)."""
+    _dev(x, torch.uint8), _dev(s_x, torch.float32), _dev(s_h, torch.float32)
+    M = x.shape[0]
+    if hq is None:
+        hq = torch.empty(M, layer.I, dtype=torch.uint8, device=x.device)
+    stride = 0 if s_h.numel() == 1 else 1
+    _check(lib().spense_gate_up(ctypes.byref(layer.shape), _ptr(layer.blob), _ptr(x), _ptr(s_x), M, _ptr(s_h), stride,
+                                _ptr(hq), _ptr(h_f32), _ptr(ws), ws.numel(), _stream()))
+    return hq
+
+
+def spense_down(layer: PackedLayer, hq, s_h, ws, y=None, dtype=torch.float32):
+    _dev(hq, torch.uint8), _dev(s_h, torch.float32)
+    M = hq.shape[0]
+    if y is None:
+        y = torch.empty(M, layer.H, dtype=dtype, device=hq.device)
+    stride = 0 if s_h.numel() == 1 else 1
+    _check(lib().spense_down(ctypes.byref(layer.shape), _ptr(layer.blob), _ptr(hq), _ptr(s_h), stride, M, _ptr(y),
+                             SPENSE_F32 if y.dtype == torch.float32 else SPENSE_BF16, _ptr(ws), ws.numel(), _stream()))
+    return y
+
+
+def spense_mlp(layer: PackedLayer, x, s_x, s_h, ws, hq_scratch=None, y=None, h_f32=None, dtype=torch.float32):
+    _dev(x, torch.uint8), _dev(s_x, torch.float32), _dev(s_h, torch.float32)
+    M = x.shape[0]
+    if hq_scratch is None:
+        hq_scratch = torch.empty(M, layer.I, dtype=torch.uint8, device=x.device)
+    if y is None:
+        y = torch.empty(M, layer.H, dtype=dtype, device=x.device)
+    stride = 0 if s_h.numel() == 1 else 1
+    _check(lib().spense_mlp(ctypes.byref(layer.shape), _ptr(layer.blob), _ptr(x), _ptr(s_x), M, _ptr(s_h), stride,
+                            _ptr(hq_scratch), _ptr(h_f32), _ptr(y),
+                            SPENSE_F32 if y.dtype == torch.float32 else SPENSE_BF16, _ptr(ws), ws.numel(), _stream()))
+    return y
+
+
+def spense_mlp_host(layer: PackedLayer, h_x, h_sx, h_sh, h_y, staging, ws):
+    """HOST (pinned) x uint8 [M, H], s_x [M], s_h [1|M] -> HOST y [M, H].  staging = dict of device
+    buffers d_x, d_scales, d_hq, d_y.  Synchronises the stream."""
+    M = h_x.shape[0]
+    stride = 0 if h_sh.numel() == 1 else 1
+    _check(lib().spense_mlp_host(ctypes.byref(layer.shape), _ptr(layer.blob), _ptr(h_x), _ptr(h_sx), M, _ptr(h_sh),
+                                 stride, _ptr(h_y), SPENSE_F32 if h_y.dtype == torch.float32 else SPENSE_BF16,
+                                 _ptr(staging["d_x"]), _ptr(staging["d_scales"]), _ptr(staging["d_hq"]),
+                                 _ptr(staging["d_y"]), _ptr(ws), ws.numel(), _stream()))
+    return h_y
+
+
+def spense_quantize_e4m3(x: torch.Tensor, mode: int):
+    _dev(x, torch.float32)
+    rows, cols = x.shape
+    out = torch.empty(rows, cols, dtype=torch.uint8, device=x.device)
+    scales = torch.empty(rows if mode == SPENSE_PER_ROW else 1, dtype=torch.float32, device=x.device)
+    ws = torch.empty((rows + 1) * 4, dtype=torch.uint8, device=x.device)
+    _check(lib().spense_quantize_e4m3(_ptr(x), rows, cols, mode, _ptr(out), _ptr(scales), _ptr(ws), ws.numel(), _stream()))
+    return out, scales

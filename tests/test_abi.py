@@ -1,0 +1,67 @@
+"""CPU-side checks of the C-ABI boundary: libspense.so builds, loads and exports every symbol that
+include/spense.h declares; host-only entry points behave; argument errors are caught on the host."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle import spense_oracle as o
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def sp():
+    from paper_2606_10445_b200 import build, spense
+    build.build()
+    return spense
+
+
+def test_every_declared_symbol_is_exported(sp):
+    hdr = open(os.path.join(ROOT, "include", "spense.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = set(re.findall(r"\b(spense_[a-z0-9_]+)\s*\(", hdr))
+    assert names == set(sp.EXPORTS), names ^ set(sp.EXPORTS)
+    L = ctypes.CDLL(sp.LIB_PATH)
+    for n in names:
+        assert hasattr(L, n), n
+    assert sp.spense_version() >= 1
+    assert sp.lib().spense_strerror(-5).decode().startswith("a group of 4")
+
+
+def test_perm_from_dense_idx_matches_oracle(sp):
+    rng = np.random.default_rng(0)
+    for I, nd in ((10, 3), (1024, 256), (128, 0), (128, 128)):
+        d = rng.choice(I, nd, replace=False)
+        got = sp.spense_perm_from_dense_idx(I, d.tolist()).numpy()
+        assert np.array_equal(got, o.perm_from_dense_idx(I, d))
+    with pytest.raises(sp.SpenseError) as e:
+        sp.spense_perm_from_dense_idx(8, [1, 1])
+    assert e.value.code == "SPENSE_ERR_ARG"
+
+
+def test_size_queries_and_host_side_argument_errors(sp):
+    blob, ws = sp.spense_pack_sizes(5120, 25600, 6400)
+    assert blob == 1024 + 282_624_000          # Qwen3-32B-shaped, p = 25 %
+    blob, _ = sp.spense_pack_sizes(5120, 27648, 0)
+    assert blob == 1024 + 265_420_800
+    blob, _ = sp.spense_pack_sizes(256, 1024, 256)
+    assert blob == 1024 + 565_248
+    for bad in ((100, 1024, 0), (256, 1000, 0), (256, 1024, 100), (256, 1024, 2048)):
+        with pytest.raises(sp.SpenseError) as e:
+            sp.spense_pack_sizes(*bad)
+        assert e.value.code == "SPENSE_ERR_SHAPE"
+    assert sp.spense_workspace_size(256, 1024, 256, 8) > 4096
+    with pytest.raises(sp.SpenseError) as e:
+        sp.spense_workspace_size(256, 1024, 256, 0)
+    assert e.value.code == "SPENSE_ERR_ARG"
+    # null pointers are rejected before anything touches CUDA (works on a box without a GPU)
+    L = sp.lib()
+    shp = sp.Shape(256, 1024, 256)
+    st = L.spense_gate_up(ctypes.byref(shp), None, None, None, 8, None, 0, None, None, None, 0, None)
+    assert sp.STATUS[st] == "SPENSE_ERR_ARG"
+    st = L.spense_down(ctypes.byref(shp), ctypes.c_void_p(1024), ctypes.c_void_p(3), ctypes.c_void_p(4), 0, 8,
+                       ctypes.c_void_p(16), 0, ctypes.c_void_p(128), 1 << 30, None)
+    assert sp.STATUS[st] == "SPENSE_ERR_ALIGN"

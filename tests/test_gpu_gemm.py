@@ -1,0 +1,164 @@
+"""-m gpu: spense_gate_up / spense_down / spense_mlp through the C ABI against the CPU oracle.
+
+Bar (BASELINE.json north_star): |gpu - oracle| <= 2e-3 * sum|a*w| + 1e-5 per element, measured
+before FP8 re-quantisation (on the fp32 dump of h and on the fp32 y)."""
+import numpy as np
+import pytest
+import torch
+
+import spense_inputs as si
+from oracle import spense_oracle as o
+from tests.gpu_common import Case, assert_down_parity, assert_gate_up_parity, cuda
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def sp():
+    from paper_2606_10445_b200 import build, spense
+    build.build()
+    assert torch.cuda.is_available()
+    return spense
+
+
+def run_gate_up(sp, c, pk, s_h, ws=None):
+    ws = ws if ws is not None else sp.spense_workspace(pk, c.M)
+    h = torch.full((c.M, c.I), float("nan"), dtype=torch.float32, device="cuda")
+    hq = sp.spense_gate_up(pk, cuda(c.x), cuda(c.s_x), cuda(torch.as_tensor(s_h, dtype=torch.float32).reshape(-1)), ws, h_f32=h)
+    torch.cuda.synchronize()
+    return h.cpu().numpy(), hq.cpu().numpy()
+
+
+# H, I, p, I_dense, M  -- Tiny is BASELINE.json configs[0]; the rest span several tiles, ragged tails,
+# every padding case and both degenerate splits
+GEMM_CASES = [
+    (256, 1024, 0.25, None, 8),
+    (256, 1024, 1.0, None, 8),      # all dense  == the baseline kernel
+    (256, 1024, 0.0, None, 8),      # all sparse
+    (256, 1024, 0.25, None, 1),
+    (256, 1024, 0.25, None, 33),
+    (256, 1024, 0.25, None, 64),
+    (256, 1024, 0.25, None, 100),
+    (256, 1024, 0.25, None, 128),
+    (256, 1024, 0.25, None, 200),   # two token blocks
+    (384, 640, None, 128, 16),      # H % 256 == 128
+    (128, 384, None, 0, 5),         # I_s % 256 == 128, single half down tile
+    (640, 896, None, 384, 48),
+    (1024, 4096, 0.25, None, 64),   # enough stages for many spans / split-K partials
+]
+
+
+@pytest.mark.parametrize("H,I,p,I_d,M", GEMM_CASES)
+def test_gate_up_down_mlp_parity(sp, H, I, p, I_d, M):
+    c = Case(H, I, p if p is not None else 0.0, M, seed=1000 + H + I + M, I_dense=I_d)
+    pk = c.pack_gpu(sp)
+    s_h = c.default_s_h()
+    r = c.oracle_gate_up(s_h)
+    ws = sp.spense_workspace(pk, M)
+    h_gpu, hq_gpu = run_gate_up(sp, c, pk, s_h, ws)
+    assert not np.isnan(h_gpu).any()
+    frac = assert_gate_up_parity(r, h_gpu, hq_gpu, s_h, "gate_up")
+    assert frac < 5e-3, f"too many Hq bytes differ from the oracle: {frac}"
+    # down, fed the GPU's own Hq bytes (strict tolerance)
+    sh_dev = cuda(torch.from_numpy(s_h))
+    y = sp.spense_down(pk, cuda(torch.from_numpy(hq_gpu)), sh_dev, ws)
+    torch.cuda.synchronize()
+    assert_down_parity(y.cpu().numpy(), hq_gpu, s_h, c.wd, c.L.w_scale[2], "down")
+    # chained spense_mlp == gate_up followed by down, bit for bit; and repeated runs are bitwise identical
+    y2 = sp.spense_mlp(pk, cuda(c.x), cuda(c.s_x), sh_dev, ws)
+    y3 = sp.spense_mlp(pk, cuda(c.x), cuda(c.s_x), sh_dev, ws)
+    torch.cuda.synchronize()
+    assert torch.equal(y, y2) and torch.equal(y2, y3)
+    # bf16 output = RNE rounding of the fp32 output
+    yb = sp.spense_mlp(pk, cuda(c.x), cuda(c.s_x), sh_dev, ws, dtype=torch.bfloat16)
+    torch.cuda.synchronize()
+    assert torch.equal(yb, y.to(torch.bfloat16))
+    # workspace is left clean (flags zero) so it can be reused
+    assert int(ws[:4096].view(torch.int32).abs().sum()) == 0
+
+
+def test_scalar_requant_scale(sp):
+    c = Case(256, 1024, 0.25, 8, seed=77)
+    pk = c.pack_gpu(sp)
+    s_h = np.float32(np.abs(c.oracle_gate_up(1.0)["h"]).max() / 448)
+    r = c.oracle_gate_up(s_h)
+    h_gpu, hq_gpu = run_gate_up(sp, c, pk, np.array([s_h], np.float32))
+    assert_gate_up_parity(r, h_gpu, hq_gpu, s_h, "scalar s_h")
+
+
+def test_one_hot_tokens_return_weight_columns_exactly(sp):
+    """A one-hot activation row makes g = one column of W~gate: exact in fp32 whatever the MMA order.
+    A wrong nibble order / lane mapping / swizzle shows up here as a permuted or zeroed column."""
+    H, I = 512, 1024
+    L = si.make_layer(H, I, 0.5, seed=21)
+    ks = [0, 1, 2, 3, 5, 31, 32, 63, 64, 127, 128, 255, 256, 300, 511, 17]
+    x = torch.zeros(len(ks), H, dtype=torch.uint8)
+    for r_, k in enumerate(ks):
+        x[r_, k] = 0x38
+    c = Case(H, I, 0.5, len(ks), seed=21, layer=L, x=x, s_x=torch.ones(len(ks)))
+    pk = c.pack_gpu(sp)
+    # u = g for identical weights is not available; instead read h = silu(g) * u against the oracle with
+    # tolerance ZERO on the accumulators: g and u are single products, so h is deterministic up to expf
+    r = c.oracle_gate_up(1.0)
+    h_gpu, _ = run_gate_up(sp, c, pk, np.array([1.0], np.float32))
+    assert np.allclose(h_gpu, r["h"], rtol=2e-6, atol=1e-30)
+    nz_ref = r["h"] != 0
+    assert np.array_equal(h_gpu != 0, nz_ref)           # exactly the same support: no column is dropped or moved
+    # down: one-hot Hq rows select columns of W~down exactly
+    hq = torch.zeros(len(ks), I, dtype=torch.uint8)
+    cols = [0, 1, 2, 3, 4, 7, 64, 127, 128, 255, 256, 511, 512, 700, 1000, 1023]
+    for r_, k in enumerate(cols):
+        hq[r_, k] = 0x38
+    ws = sp.spense_workspace(pk, len(ks))
+    y = sp.spense_down(pk, cuda(hq), cuda(torch.ones(1)), ws).cpu().numpy()
+    want = (o.e4m3_decode(c.wd[:, cols]).T * np.float32(L.w_scale[2])).astype(np.float32)
+    assert np.array_equal(y, want)
+
+
+def test_small_integer_inputs_are_exact(sp):
+    """Small-integer weights and activations: every partial sum is an integer < 2^24, so the fp32
+    result must equal the oracle EXACTLY in any accumulation order (split-K partials included)."""
+    H, I, I_d, M = 1024, 2048, 512, 32
+    wg, wu, wd, x = si.make_small_int_case(H, I, I_d, M, seed=4)
+    pk = sp.spense_pack(cuda(wg), cuda(wu), cuda(wd), (1.0, 1.0, 1.0), None, I_d)
+    ws = sp.spense_workspace(pk, M)
+    hq = x.new_zeros(M, I)
+    hq[:, ::3] = 0x38
+    hq[:, 1::5] = 0xC0
+    y = sp.spense_down(pk, cuda(hq), cuda(torch.ones(1)), ws).cpu().numpy()
+    ref = o.down(hq.numpy(), 1.0, np.where((wd.numpy() & 0x7F) == 0, 0, wd.numpy()), 1.0)
+    assert np.array_equal(y.astype(np.float64), ref["y"])
+    # gate_up accumulators are exact too; h goes through expf, so compare with a tight relative bound
+    r = o.gate_up(x.numpy(), np.ones(M), wg.numpy(), wu.numpy(), 1.0, 1.0, 1.0)
+    h = torch.empty(M, I, dtype=torch.float32, device="cuda")
+    sp.spense_gate_up(pk, cuda(x), cuda(torch.ones(M)), cuda(torch.ones(1)), ws, h_f32=h)
+    assert np.allclose(h.cpu().numpy(), r["h"], rtol=3e-6, atol=1e-6)
+
+
+def test_dense_fraction_invariance_on_gpu(sp):
+    L0 = si.make_layer(512, 1024, 0.0, seed=31, all_2_4=True)
+    x, sx = si.make_activations(24, 512, seed=31)
+    ys = []
+    for I_d in (0, 128, 512, 1024):
+        pk = sp.spense_pack(cuda(L0.wgate), cuda(L0.wup), cuda(L0.wdown), L0.w_scale, None, I_d)
+        ws = sp.spense_workspace(pk, 24)
+        h = torch.empty(24, 1024, dtype=torch.float32, device="cuda")
+        sp.spense_gate_up(pk, cuda(x), cuda(sx), cuda(torch.full((1,), 0.01)), ws, h_f32=h)
+        ys.append(h.cpu().numpy())
+    ref = o.gate_up(x.numpy(), sx.numpy(), *[np.where((w.numpy() & 0x7F) == 0, 0, w.numpy()) for w in (L0.wgate, L0.wup)],
+                    L0.w_scale[0], L0.w_scale[1], 0.01)
+    for y in ys:
+        assert (np.abs(y - ref["h"]) <= o.tol_glu(ref)).all()
+
+
+def test_gemm_argument_errors(sp):
+    c = Case(256, 1024, 0.25, 8, seed=3)
+    pk = c.pack_gpu(sp)
+    ws = sp.spense_workspace(pk, 8)
+    with pytest.raises(sp.SpenseError) as e:
+        sp.spense_gate_up(pk, cuda(c.x), cuda(c.s_x), cuda(torch.ones(1)), ws[:1024])
+    assert e.value.code == "SPENSE_ERR_BUFFER_TOO_SMALL"
+    bad = sp.PackedLayer(256, 1024, 128, pk.blob)       # header says I_dense = 256
+    with pytest.raises(sp.SpenseError) as e:
+        sp.spense_gate_up(bad, cuda(c.x), cuda(c.s_x), cuda(torch.ones(1)), ws)
+    assert e.value.code == "SPENSE_ERR_BAD_BLOB"

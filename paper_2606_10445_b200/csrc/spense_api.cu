@@ -143,13 +143,16 @@ int read_header(const void* d_blob, const spense_shape_t* shape, BlobHeader* out
   return SPENSE_OK;
 }
 
+long long* g_trace = nullptr;   // debug: set by spense_debug_set_trace (not part of the public ABI)
+
 void fill_common(GemmParams& p, const Schedule& sc, int M, int n_pad, void* d_ws) {
+  p.trace = g_trace;
   p.n_spans = sc.n_spans;
   std::memcpy(p.span_begin, sc.span_begin, sizeof(int) * (sc.n_spans + 1));
   p.M = M;
   p.n_pad = n_pad;
   p.slot_bytes = kSparseStageBytes + 2 * n_pad * 128;
-  int stages = (232448 - 1024 - 256) / p.slot_bytes;
+  int stages = (232448 - 1024 - 256 - 16 * n_pad) / p.slot_bytes;
   p.num_stages = stages > 8 ? 8 : stages;
   p.acc_stride = n_pad <= 32 ? 32 : (n_pad <= 64 ? 64 : 128);
   p.num_acc_bufs = n_pad <= 64 ? 2 : 1;
@@ -232,6 +235,9 @@ using namespace spense;
 extern "C" {
 
 int spense_version(void) { return 100 * 0 + 1; }
+
+// debug hook (undeclared in spense.h): per-CTA clock64 timeline, 16 int64 per span, of the next launches
+void spense_debug_set_trace(void* d_buf) { g_trace = reinterpret_cast<long long*>(d_buf); }
 
 const char* spense_strerror(int status) {
   switch (status) {

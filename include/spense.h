@@ -104,9 +104,11 @@ int spense_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8
                 size_t blob_bytes, const spense_canon_t* canon, void* d_ws, size_t ws_bytes,
                 int64_t* h_err_where, spense_stream_t stream);
 
-/* Workspace for the GEMM calls at up to M tokens (split-K partial tiles + flags).  The workspace
- * must be initialised ONCE with spense_workspace_init before its first use (it is left clean by
- * every successful call).  One workspace must not be used by two streams concurrently.          */
+/* Workspace for the GEMM calls at up to M tokens (split-K partial tiles, flags, a launch-epoch word).
+ * The workspace must be initialised ONCE with spense_workspace_init before its first use; every
+ * launch advances the epoch word, so nothing needs resetting between calls or CUDA-graph replays.
+ * One workspace must not be used by two streams concurrently.  The CTAs of one GEMM launch wait
+ * for each other (split-K fix-up): the device must not be shared with other work that pins SMs.  */
 int spense_workspace_size(const spense_shape_t* shape, int32_t M, size_t* bytes);
 int spense_workspace_init(void* d_ws, size_t ws_bytes, spense_stream_t stream);
 
@@ -124,16 +126,21 @@ int spense_gate_up(const spense_shape_t* shape, const void* d_blob, const uint8_
 /* spense_down -- input-split Spense GEMM: the K loop runs the sparse K range
  * [0, I_s) on sparse MMAs and continues with the dense range [I_s, I) into the SAME accumulator:
  *   y[m, n] = (sum_k hq[m, k] * Wd[n, k]) * s_h[m] * s_down.
- *   d_hq [M, I] E4M3 (permuted order); d_y [M, H] fp32 (SPENSE_F32) or bf16 (SPENSE_BF16).        */
+ *   d_hq [M, I] E4M3 (permuted order); d_y [M, H] fp32 (SPENSE_F32) or bf16 (SPENSE_BF16).
+ *   d_next_blob (nullable): packed blob of the layer that runs NEXT on this stream, same shape; while
+ *   this launch drains, the first stages that layer's gate_up will stream are prefetched into L2
+ *   (a performance hint only: results never depend on it).                                         */
 int spense_down(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_hq, const float* d_sh,
                 int32_t sh_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, size_t ws_bytes,
-                spense_stream_t stream);
+                const void* d_next_blob, spense_stream_t stream);
 
 /* spense_mlp -- the whole layer: gate_up then down on one stream (programmatic dependent launch).
- *   d_hq_scratch [M, I] E4M3 scratch; d_h_f32 nullable as in spense_gate_up.                     */
+ *   d_hq_scratch [M, I] E4M3 scratch; d_h_f32 nullable as in spense_gate_up; d_next_blob nullable as
+ *   in spense_down.                                                                               */
 int spense_mlp(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx,
                int32_t M, const float* d_sh, int32_t sh_stride, uint8_t* d_hq_scratch, float* d_h_f32,
-               void* d_y, int32_t y_dtype, void* d_ws, size_t ws_bytes, spense_stream_t stream);
+               void* d_y, int32_t y_dtype, void* d_ws, size_t ws_bytes, const void* d_next_blob,
+               spense_stream_t stream);
 
 /* spense_mlp_host -- same, with HOST activations and results: copies h_x [M, H], h_sx [M], h_sh
  * (1 or M floats) to the device staging buffers, runs spense_mlp, copies y back to h_y and
@@ -142,7 +149,7 @@ int spense_mlp(const spense_shape_t* shape, const void* d_blob, const uint8_t* d
 int spense_mlp_host(const spense_shape_t* shape, const void* d_blob, const uint8_t* h_x, const float* h_sx,
                     int32_t M, const float* h_sh, int32_t sh_stride, void* h_y, int32_t y_dtype,
                     uint8_t* d_x, float* d_scales, uint8_t* d_hq_scratch, void* d_y, void* d_ws,
-                    size_t ws_bytes, spense_stream_t stream);
+                    size_t ws_bytes, const void* d_next_blob, spense_stream_t stream);
 
 /* spense_quantize_e4m3 -- helper (reading Q5): scale = amax / 448 (1 if amax == 0), per tensor or
  * per row; out = E4M3_rne_sat(in / scale) with an IEEE fp32 division.  d_scales: 1 or rows floats.

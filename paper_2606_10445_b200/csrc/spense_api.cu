@@ -2,6 +2,7 @@
 // tensor-map creation and launches.  No device allocation, no synchronisation in the GEMM calls.
 #include <cudaTypedefs.h>
 
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <vector>
@@ -48,14 +49,27 @@ bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) %
 
 int n_pad_of(int M) { int n = (M + 15) / 16 * 16; return n > 128 ? 128 : n; }
 
-size_t ws_bytes_for(int n_pad, int spans) { return kFlagBytes + (size_t)spans * 2 * n_pad * 128 * sizeof(float); }
+size_t ws_bytes_for(int n_pad, int spans) { return kFlagBytes + (size_t)spans * 2 * 2 * n_pad * 128 * sizeof(float); }
+
+double env_double(const char* name, double dflt) {
+  const char* v = std::getenv(name);
+  return v ? std::atof(v) : dflt;
+}
 
 // ---- stream-K schedule: cut the stage sequence into n_spans spans of (nearly) equal bytes.
 struct Schedule {
   int mode, H, I, I_d, n_pad, sms;
   int n_spans;
   int span_begin[kMaxSpans + 1];
+  uint32_t span_off[kMaxSpans];   // byte offset of the span's first stage image inside its section
+  uint32_t span_pre[kMaxSpans];   // bytes of the stages the producer issues before anything else (one ring)
 };
+
+int slot_bytes_of(int n_pad) { return kSparseStageBytes + 2 * n_pad * 128; }
+int ring_stages_of(int n_pad) {
+  const int stages = (232448 - 1024 - 256 - 16 * n_pad) / slot_bytes_of(n_pad);
+  return stages > 8 ? 8 : stages;
+}
 std::mutex g_sched_mu;
 std::vector<Schedule> g_sched;
 
@@ -65,8 +79,11 @@ const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms) {
     if (s.mode == mode && s.H == g.H && s.I == g.I && s.I_d == g.I_d && s.n_pad == n_pad && s.sms == sms) return s;
   Schedule sc = {};
   sc.mode = mode; sc.H = g.H; sc.I = g.I; sc.I_d = g.I_d; sc.n_pad = n_pad; sc.sms = sms;
-  // cost of a stage = bytes it moves into shared memory
-  const double cs = kSparseStageBytes + 2.0 * n_pad * 128, cd = kDenseStageBytes + 1.0 * n_pad * 128;
+  // cost of a stage.  Every CTA keeps the same number of ring slots in flight, so under HBM contention a
+  // stage costs one slot latency plus its bytes: measured on B200 (profiles/) a 40 KB sparse stage takes
+  // ~1.12x a 32 KB dense one => fixed part ~36 KB-equivalents; activation bytes come from L2 and weigh less.
+  static const double fixed = env_double("SPENSE_SCHED_FIXED", 36864.0), gamma = env_double("SPENSE_SCHED_GAMMA", 0.25);
+  const double cs = fixed + kSparseStageBytes + gamma * 2.0 * n_pad * 128, cd = fixed + kDenseStageBytes + gamma * 1.0 * n_pad * 128;
   std::vector<double> cost;
   if (mode == 0) {
     cost.insert(cost.end(), (size_t)g.gu_tiles_sparse * g.gu_ns, cs);
@@ -96,6 +113,24 @@ const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms) {
     sc.span_begin[i] = b;
   }
   sc.span_begin[spans] = total;
+  // byte offsets: the blob stores the stage images in exactly this linear order
+  std::vector<uint32_t> bytes(total);
+  if (mode == 0) {
+    for (int i = 0; i < total; ++i) bytes[i] = i < g.gu_tiles_sparse * g.gu_ns ? kSparseStageBytes : kDenseStageBytes;
+  } else {
+    const int per = g.dn_ns + g.dn_nd;
+    for (int i = 0; i < total; ++i) bytes[i] = (i % per) < g.dn_ns ? kSparseStageBytes : kDenseStageBytes;
+  }
+  const int ring = ring_stages_of(n_pad);
+  uint64_t off = 0;
+  int st = 0;
+  for (int i = 0; i < spans; ++i) {
+    while (st < sc.span_begin[i]) off += bytes[st++];
+    sc.span_off[i] = (uint32_t)off;
+    uint32_t pre = 0;
+    for (int k = sc.span_begin[i]; k < sc.span_begin[i + 1] && k < sc.span_begin[i] + ring; ++k) pre += bytes[k];
+    sc.span_pre[i] = pre;
+  }
   g_sched.push_back(sc);
   return g_sched.back();
 }
@@ -151,18 +186,30 @@ void fill_common(GemmParams& p, const Schedule& sc, int M, int n_pad, void* d_ws
   std::memcpy(p.span_begin, sc.span_begin, sizeof(int) * (sc.n_spans + 1));
   p.M = M;
   p.n_pad = n_pad;
-  p.slot_bytes = kSparseStageBytes + 2 * n_pad * 128;
-  int stages = (232448 - 1024 - 256 - 16 * n_pad) / p.slot_bytes;
-  p.num_stages = stages > 8 ? 8 : stages;
+  p.slot_bytes = slot_bytes_of(n_pad);
+  p.num_stages = ring_stages_of(n_pad);
   p.acc_stride = n_pad <= 32 ? 32 : (n_pad <= 64 ? 64 : 128);
   p.num_acc_bufs = n_pad <= 64 ? 2 : 1;
-  p.flags = reinterpret_cast<int*>(d_ws);
+  p.ws_ctrl = reinterpret_cast<int*>(d_ws);
+  p.flags = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(d_ws) + 128);
   p.partials = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes);
+}
+
+// L2 prefetch hint: while this launch runs its fix-up tail, pull what the next launch streams first.
+void fill_next(GemmParams& p, const uint8_t* next_section, const Schedule& next) {
+  static const bool enabled = env_double("SPENSE_L2_PREFETCH", 1.0) != 0.0;
+  if (!enabled || !next_section) return;
+  p.next_base = next_section;
+  for (int i = 0; i < p.n_spans; ++i) {
+    const int k = i < next.n_spans ? i : next.n_spans - 1;
+    p.next_off[i] = next.span_off[k];
+    p.next_len[i] = i < next.n_spans ? next.span_pre[k] : 0;
+  }
 }
 
 int gate_up_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_x,
                  const float* d_sx, int32_t M, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32,
-                 void* d_ws, bool pdl, cudaStream_t stream) {
+                 void* d_ws, bool pdl, bool down_follows, cudaStream_t stream) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
   for (int m0 = 0; m0 < M; m0 += 128) {
     const int Mb = (M - m0) < 128 ? (M - m0) : 128;
@@ -180,6 +227,8 @@ int gate_up_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void*
     p.hq = d_hq + (size_t)m0 * g.I;
     p.h_f32 = d_h_f32 ? d_h_f32 + (size_t)m0 * g.I : nullptr;
     p.ld_out = g.I; p.out_rows = g.I;
+    if (down_follows && m0 + 128 >= M)                       // the same layer's down projection streams next
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off, get_schedule(1, g, n_pad_of(M < 128 ? M : 128), g_num_sms));
     CUtensorMap tm;
     int st = make_tmap(&tm, d_x + (size_t)m0 * g.H, g.H, Mb, n_pad);
     if (st) return st;
@@ -191,7 +240,7 @@ int gate_up_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void*
 
 int down_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_hq,
               const float* d_sh, int32_t sh_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, bool pdl,
-              cudaStream_t stream) {
+              const void* d_next_blob, cudaStream_t stream) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
   const size_t esz = y_dtype == SPENSE_F32 ? 4 : 2;
   for (int m0 = 0; m0 < M; m0 += 128) {
@@ -209,6 +258,8 @@ int down_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_
     p.y = reinterpret_cast<uint8_t*>(d_y) + (size_t)m0 * g.H * esz;
     p.y_dtype = y_dtype;
     p.ld_out = g.H; p.out_rows = g.H;
+    if (d_next_blob && m0 + 128 >= M)                        // the next layer's gate/up weights stream next
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + hdr.gate_up_off, get_schedule(0, g, n_pad_of(M < 128 ? M : 128), g_num_sms));
     CUtensorMap tm;
     int st = make_tmap(&tm, d_hq + (size_t)m0 * g.I, g.I, Mb, n_pad);
     if (st) return st;
@@ -328,18 +379,20 @@ int spense_gate_up(const spense_shape_t* shape, const void* d_blob, const uint8_
   BlobHeader hdr;
   st = read_header(d_blob, shape, &hdr);
   if (st) return st;
-  return gate_up_impl(shape, hdr, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq, d_h_f32, d_ws, false,
+  return gate_up_impl(shape, hdr, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq, d_h_f32, d_ws, false, false,
                       reinterpret_cast<cudaStream_t>(stream));
 }
 
 int spense_down(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_hq, const float* d_sh, int32_t sh_stride,
-                int32_t M, void* d_y, int32_t y_dtype, void* d_ws, size_t ws_bytes, spense_stream_t stream) {
+                int32_t M, void* d_y, int32_t y_dtype, void* d_ws, size_t ws_bytes, const void* d_next_blob,
+                spense_stream_t stream) {
   int st = check_shape(shape);
   if (st) return st;
   if (!d_blob || !d_hq || !d_sh || !d_y || M < 1 || (sh_stride != 0 && sh_stride != 1) ||
       (y_dtype != SPENSE_F32 && y_dtype != SPENSE_BF16))
     return SPENSE_ERR_ARG;
-  if (!aligned(d_blob, 128) || !aligned(d_hq, 128) || !aligned(d_y, 16) || !aligned(d_sh, 4)) return SPENSE_ERR_ALIGN;
+  if (!aligned(d_blob, 128) || !aligned(d_hq, 128) || !aligned(d_y, 16) || !aligned(d_sh, 4) || !aligned(d_next_blob, 128))
+    return SPENSE_ERR_ALIGN;
   st = check_ws(shape, M, d_ws, ws_bytes);
   if (st) return st;
   st = check_device();
@@ -347,20 +400,20 @@ int spense_down(const spense_shape_t* shape, const void* d_blob, const uint8_t* 
   BlobHeader hdr;
   st = read_header(d_blob, shape, &hdr);
   if (st) return st;
-  return down_impl(shape, hdr, d_blob, d_hq, d_sh, sh_stride, M, d_y, y_dtype, d_ws, false,
+  return down_impl(shape, hdr, d_blob, d_hq, d_sh, sh_stride, M, d_y, y_dtype, d_ws, false, d_next_blob,
                    reinterpret_cast<cudaStream_t>(stream));
 }
 
 int spense_mlp(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx, int32_t M,
                const float* d_sh, int32_t sh_stride, uint8_t* d_hq_scratch, float* d_h_f32, void* d_y, int32_t y_dtype,
-               void* d_ws, size_t ws_bytes, spense_stream_t stream) {
+               void* d_ws, size_t ws_bytes, const void* d_next_blob, spense_stream_t stream) {
   int st = check_shape(shape);
   if (st) return st;
   if (!d_blob || !d_x || !d_sx || !d_sh || !d_hq_scratch || !d_y || M < 1 || (sh_stride != 0 && sh_stride != 1) ||
       (y_dtype != SPENSE_F32 && y_dtype != SPENSE_BF16))
     return SPENSE_ERR_ARG;
   if (!aligned(d_blob, 128) || !aligned(d_x, 128) || !aligned(d_hq_scratch, 128) || !aligned(d_y, 16) ||
-      !aligned(d_sx, 4) || !aligned(d_sh, 4) || (d_h_f32 && !aligned(d_h_f32, 16)))
+      !aligned(d_sx, 4) || !aligned(d_sh, 4) || (d_h_f32 && !aligned(d_h_f32, 16)) || !aligned(d_next_blob, 128))
     return SPENSE_ERR_ALIGN;
   st = check_ws(shape, M, d_ws, ws_bytes);
   if (st) return st;
@@ -370,14 +423,15 @@ int spense_mlp(const spense_shape_t* shape, const void* d_blob, const uint8_t* d
   st = read_header(d_blob, shape, &hdr);
   if (st) return st;
   cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
-  st = gate_up_impl(shape, hdr, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq_scratch, d_h_f32, d_ws, true, s);
+  st = gate_up_impl(shape, hdr, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq_scratch, d_h_f32, d_ws, true, true, s);
   if (st) return st;
-  return down_impl(shape, hdr, d_blob, d_hq_scratch, d_sh, sh_stride, M, d_y, y_dtype, d_ws, true, s);
+  return down_impl(shape, hdr, d_blob, d_hq_scratch, d_sh, sh_stride, M, d_y, y_dtype, d_ws, true, d_next_blob, s);
 }
 
 int spense_mlp_host(const spense_shape_t* shape, const void* d_blob, const uint8_t* h_x, const float* h_sx, int32_t M,
                     const float* h_sh, int32_t sh_stride, void* h_y, int32_t y_dtype, uint8_t* d_x, float* d_scales,
-                    uint8_t* d_hq_scratch, void* d_y, void* d_ws, size_t ws_bytes, spense_stream_t stream) {
+                    uint8_t* d_hq_scratch, void* d_y, void* d_ws, size_t ws_bytes, const void* d_next_blob,
+                    spense_stream_t stream) {
   int st = check_shape(shape);
   if (st) return st;
   if (!h_x || !h_sx || !h_sh || !h_y || !d_x || !d_scales || M < 1 || (sh_stride != 0 && sh_stride != 1) ||
@@ -389,7 +443,7 @@ int spense_mlp_host(const spense_shape_t* shape, const void* d_blob, const uint8
   if (cudaMemcpyAsync(d_scales, h_sx, (size_t)M * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) return SPENSE_ERR_CUDA;
   if (cudaMemcpyAsync(d_scales + M, h_sh, n_sh * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) return SPENSE_ERR_CUDA;
   st = spense_mlp(shape, d_blob, d_x, d_scales, M, d_scales + M, sh_stride, d_hq_scratch, nullptr, d_y, y_dtype, d_ws,
-                  ws_bytes, stream);
+                  ws_bytes, d_next_blob, stream);
   if (st) return st;
   const size_t esz = y_dtype == SPENSE_F32 ? 4 : 2;
   if (cudaMemcpyAsync(h_y, d_y, (size_t)M * shape->H * esz, cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPENSE_ERR_CUDA;

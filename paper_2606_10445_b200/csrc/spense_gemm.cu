@@ -1,25 +1,33 @@
 // Spense hybrid sparse-dense FP8 GEMM for sm_100a (tcgen05 + TMEM + TMA / bulk copy).
 //
-// One kernel, two modes:
-//   mode 0  gate_up : output-split.  Pair tile = 128 rows of W_gate + the same 128 rows
+// One kernel template, two instances:
+//   MODE 0  gate_up : output-split.  Pair tile = 128 rows of W_gate + the same 128 rows
 //                     of W_up; tiles below I_s are 2:4 compressed (tcgen05.mma.sp), the rest dense
 //                     (tcgen05.mma).  Epilogue: scales -> SiLU(g)*u (Eq. 4) -> E4M3.
-//   mode 1  down    : input-split.  Pair tile = 2 x 128 rows of W_down; the K loop runs
+//   MODE 1  down    : input-split.  Pair tile = 2 x 128 rows of W_down; the K loop runs
 //                     the sparse stages and then the dense stages INTO THE SAME TMEM ACCUMULATOR.
 //
 // Swap-AB: only the A operand of tcgen05.mma.sp can be sparse, so weights are A (MMA-M = 128 weight
 // rows) and tokens are B (MMA-N = padded token count); the accumulator holds Y^T [128 rows x tokens].
 //
-// Decode is weight-streaming bound, so the grid is a byte-balanced stream-K: the linear sequence of
-// stage images is cut into n_spans equal-byte spans, one persistent CTA per span.  A CTA whose span
-// starts inside a tile contributes an fp32 partial through an L2-resident workspace; the CTA that
-// holds the tile's first stage owns the epilogue and adds the partials in fixed span order, so
-// results are bitwise reproducible.  Span i runs on CTA n_spans-1-i: an owner only ever waits for
-// higher-numbered spans = lower-numbered CTAs, which the hardware schedules first.
+// Decode is weight-streaming bound, so the grid is a cost-balanced stream-K: the linear sequence of
+// stage images (= the byte order of the blob) is cut into n_spans spans, one persistent CTA per span.
+// A tile whose stages fall into several spans is fixed up through an L2-resident fp32 workspace, always
+// adding the partials in span order, so results are bitwise reproducible:
+//   * 2 spans  : the second span finishes its part early (it is its first segment), dumps it and
+//                publishes a flag; the first span (owner) adds it to its TMEM accumulator and runs the
+//                epilogue -- nothing but the flag check sits on the owner's critical path;
+//   * > 2 spans: every span finishes late, so all dump, and the n spans reduce M/n token columns each
+//                (reduce-scatter) instead of one owner reducing n partials serially.
+// Flags hold the epoch of the launch (a device-side counter in the workspace), so nothing has to be
+// reset between launches and CUDA-graph replays see fresh values.
+// Span i runs on CTA n_spans-1-i.  CTAs of one launch wait for each other, so all n_spans <= #SM CTAs
+// must be co-resident: 1 CTA/SM by construction (shared memory), the device must not be shared.
 //
 // Warp roles (384 threads): warp 0 producer (bulk copy of the weight stage + TMA of the activation
 // tile), warp 1 MMA issuer, warp 2 TMEM allocator, warps 4-11 epilogue (TMEM lane quadrant = warp & 3,
-// half of the token columns = (warp - 4) >> 2).
+// half of the token columns = (warp - 4) >> 2).  Rarely executed code is kept rolled: the kernel is
+// latency-sensitive at its tail and instruction-cache misses on cold paths showed up in the timeline.
 #include <cuda_bf16.h>
 
 #include "spense_internal.cuh"
@@ -28,37 +36,53 @@ namespace spense {
 
 namespace {
 
-struct TileInfo {
-  int tile;        // pair-tile index
-  int first;       // linear stage index of the tile's first stage
-  int ns, nd;      // sparse / dense stages of this tile
-  size_t offset;   // byte offset of the tile's first stage image in the section
+// Position in the linear stage sequence: pair tile, stage inside the tile, stages of the tile.
+struct Cursor {
+  int tile, j, ns, nd, first;   // first = linear index of the tile's first stage
 };
 
-__device__ __forceinline__ TileInfo tile_of_stage(const GemmParams& p, int s) {
-  TileInfo t;
-  if (p.mode == 0) {
+// The only place with integer divisions (one copy, called once per role).
+template <int MODE>
+__device__ __noinline__ Cursor cursor_at(const GemmParams& p, int s, unsigned long long* byte_off) {
+  Cursor c;
+  size_t off;
+  if (MODE == 0) {
     const int sparse_total = p.tiles_sparse * p.ns;
     if (s < sparse_total) {
-      t.tile = s / p.ns;
-      t.first = t.tile * p.ns;
-      t.ns = p.ns; t.nd = 0;
-      t.offset = (size_t)t.first * kSparseStageBytes;
+      c.tile = s / p.ns;
+      c.first = c.tile * p.ns;
+      c.ns = p.ns; c.nd = 0;
+      off = (size_t)s * kSparseStageBytes;
     } else {
       const int td = (s - sparse_total) / p.nd;
-      t.tile = p.tiles_sparse + td;
-      t.first = sparse_total + td * p.nd;
-      t.ns = 0; t.nd = p.nd;
-      t.offset = (size_t)sparse_total * kSparseStageBytes + (size_t)td * p.nd * kDenseStageBytes;
+      c.tile = p.tiles_sparse + td;
+      c.first = sparse_total + td * p.nd;
+      c.ns = 0; c.nd = p.nd;
+      off = (size_t)sparse_total * kSparseStageBytes + (size_t)(s - sparse_total) * kDenseStageBytes;
     }
+    c.j = s - c.first;
   } else {
     const int per = p.ns + p.nd;
-    t.tile = s / per;
-    t.first = t.tile * per;
-    t.ns = p.ns; t.nd = p.nd;
-    t.offset = (size_t)t.tile * ((size_t)p.ns * kSparseStageBytes + (size_t)p.nd * kDenseStageBytes);
+    c.tile = s / per;
+    c.first = c.tile * per;
+    c.ns = p.ns; c.nd = p.nd;
+    c.j = s - c.first;
+    off = (size_t)c.tile * ((size_t)p.ns * kSparseStageBytes + (size_t)p.nd * kDenseStageBytes);
+    off += c.j < c.ns ? (size_t)c.j * kSparseStageBytes
+                      : (size_t)c.ns * kSparseStageBytes + (size_t)(c.j - c.ns) * kDenseStageBytes;
   }
-  return t;
+  *byte_off = off;
+  return c;
+}
+
+template <int MODE>
+__device__ __forceinline__ void next_tile(const GemmParams& p, Cursor& c) {
+  c.first += c.ns + c.nd;
+  ++c.tile;
+  c.j = 0;
+  if (MODE == 0) {
+    if (c.tile < p.tiles_sparse) { c.ns = p.ns; c.nd = 0; } else { c.ns = 0; c.nd = p.nd; }
+  }
 }
 
 // SiLU(g) * u on the hardware exp2 / reciprocal units: branch-free, relative error ~1e-6 (far inside
@@ -86,7 +110,7 @@ __device__ __forceinline__ uint32_t to_e4m3x2(float lo, float hi) {
   return r;
 }
 
-// optional per-CTA timeline (debug builds of the harness set GemmParams::trace; nullptr in production)
+// optional per-CTA timeline (the harness sets GemmParams::trace through a debug hook; nullptr in production)
 __device__ __forceinline__ void trace(const GemmParams& p, int span, int slot) {
   if (p.trace) p.trace[(size_t)span * 16 + slot] = clock64();
 }
@@ -95,13 +119,55 @@ __device__ __forceinline__ long long globaltimer() {
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
   return t;
 }
+__device__ __forceinline__ int ld_acquire(const int* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release(int* p, int v) {
+  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ void epi_sync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }   // the 8 epilogue warps
 
 constexpr int kThreads = 384;
 constexpr int kTmemCols = 512;
 constexpr int kMetaCol = 480;   // 2 buffers x 16 columns of 2:4 metadata
 
+// One output element (token m, weight row r of pair tile `tile`): scales, GLU + requant, or the Y store.
+template <int MODE>
+__device__ __forceinline__ void finish(const GemmParams& p, const float* sc, int tile, int r, int m, float f0, float f1) {
+  if (MODE == 0) {
+    const float g = f0 * sc[m];
+    const float u = f1 * sc[p.n_pad + m];
+    const float h = silu_mul(g, u);
+    const float qv = div_by(h, sc[2 * p.n_pad + m], sc[3 * p.n_pad + m]);
+    const size_t o = (size_t)m * p.ld_out + tile * 128 + r;
+    if (p.h_f32) p.h_f32[o] = h;
+    p.hq[o] = (uint8_t)(to_e4m3x2(qv, 0.0f) & 0xFFu);
+  } else {
+    const int out_row = tile * 256 + r;
+    const float scl = sc[m];
+    const float y0 = f0 * scl, y1 = f1 * scl;
+    const size_t o = (size_t)m * p.ld_out + out_row;
+    const bool second = out_row + 128 < p.out_rows;
+    if (p.y_dtype == SPENSE_F32) {
+      float* y = reinterpret_cast<float*>(p.y);
+      y[o] = y0;
+      if (second) y[o + 128] = y1;
+    } else {
+      __nv_bfloat16* y = reinterpret_cast<__nv_bfloat16*>(p.y);
+      y[o] = __float2bfloat16_rn(y0);
+      if (second) y[o + 128] = __float2bfloat16_rn(y1);
+    }
+  }
+}
+
+// A tile shared by more than two spans [a, b]: reduced at the end of the span (reduce-scatter).
+struct Group { int a, b, tile, first; };
+
 }  // namespace
 
+template <int MODE>
 __global__ void __launch_bounds__(kThreads, 1)
 spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__ CUtensorMap tmap_b) {
   extern __shared__ uint8_t smem_raw[];
@@ -111,21 +177,23 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
 
   const int S = p.num_stages;
   // barriers live after the stage ring
-  const uint32_t bar_base = smem_base + (uint32_t)S * p.slot_bytes;
+  const uint32_t ring_bytes = (uint32_t)S * p.slot_bytes;
+  const uint32_t bar_base = smem_base + ring_bytes;
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
   auto empty_bar = [&](int s) { return bar_base + 8u * (8 + s); };
   auto accf_bar = [&](int b) { return bar_base + 8u * (16 + b); };
   auto acce_bar = [&](int b) { return bar_base + 8u * (18 + b); };
-  auto part_bar = [&](int r) { return bar_base + 8u * (22 + r); };
+  const uint32_t red_bar = bar_base + 8u * 22;
   const uint32_t tmem_slot = bar_base + 8u * 20;
   uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
-  volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(smem_gen + (size_t)S * p.slot_bytes + 8 * 20);
+  volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(smem_gen + ring_bytes + 8 * 20);
+  volatile int* epoch_ptr = reinterpret_cast<volatile int*>(smem_gen + ring_bytes + 8 * 21);
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmap_b);
     for (int s = 0; s < S; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(accf_bar(b), 1); mbar_init(acce_bar(b), 256); }
-    for (int r = 0; r < 8; ++r) mbar_init(part_bar(r), 1);
+    mbar_init(red_bar, 1);
     fence_barrier_init();
   }
   if (warp == 2) tmem_alloc(tmem_slot, kTmemCols);
@@ -141,53 +209,84 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
   const int sb = p.span_begin[span];
   const int se = p.span_begin[span + 1];
   const uint32_t b_tile_bytes = (uint32_t)p.n_pad * 128u;
-  if (p.trace && threadIdx.x == 0) { p.trace[(size_t)span * 16 + 0] = clock64(); p.trace[(size_t)span * 16 + 12] = globaltimer(); }
+  if (p.trace && threadIdx.x == 0) {
+    uint32_t smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    p.trace[(size_t)span * 16 + 0] = clock64(); p.trace[(size_t)span * 16 + 12] = globaltimer(); p.trace[(size_t)span * 16 + 14] = smid;
+  }
 
   if (warp == 0) {
     // ===================== producer =====================
     if (lane == 0) {
       const uint64_t pol_w = policy_evict_first();
       const uint64_t pol_a = policy_evict_last();
-      bool waited = false;
-      int it = 0;
-      for (int s = sb; s < se;) {
-        const TileInfo t = tile_of_stage(p, s);
-        const int seg_end = min(se, t.first + t.ns + t.nd);
-        for (; s < seg_end; ++s, ++it) {
-          const int j = s - t.first;
-          const int slot = it % S;
-          const uint32_t ph = (uint32_t)(it / S) & 1u;
-          mbar_wait(empty_bar(slot), ph ^ 1u);
-          if (it == 0) trace(p, span, 1);
-          const uint32_t a_dst = smem_base + (uint32_t)slot * p.slot_bytes;
-          const uint32_t b_dst = a_dst + kSparseStageBytes;
-          if (j < t.ns) {
-            mbar_expect_tx(full_bar(slot), kSparseStageBytes + 2 * b_tile_bytes);
-            bulk_g2s(a_dst, p.section + t.offset + (size_t)j * kSparseStageBytes, kSparseStageBytes, full_bar(slot), pol_w);
-            if (!waited) { pdl_wait(); waited = true; }   // weights never depend on the previous kernel; activations do
-            tma_load_2d(b_dst, &tmap_b, j * kSparseStageK, 0, full_bar(slot), pol_a);
-            tma_load_2d(b_dst + b_tile_bytes, &tmap_b, j * kSparseStageK + 128, 0, full_bar(slot), pol_a);
-          } else {
-            const int jd = j - t.ns;
-            mbar_expect_tx(full_bar(slot), kDenseStageBytes + b_tile_bytes);
-            bulk_g2s(a_dst, p.section + t.offset + (size_t)t.ns * kSparseStageBytes + (size_t)jd * kDenseStageBytes,
-                     kDenseStageBytes, full_bar(slot), pol_w);
-            if (!waited) { pdl_wait(); waited = true; }
-            tma_load_2d(b_dst, &tmap_b, p.dense_k0 + jd * kDenseStageK, 0, full_bar(slot), pol_a);
-          }
+      unsigned long long off;
+      Cursor c = cursor_at<MODE>(p, sb, &off);
+      const uint8_t* src = p.section + off;
+      const int n = se - sb;
+      const int pre = n < S ? n : S;
+      uint32_t info[8];                                    // stages issued before pdl_wait: K coordinate | sparse << 31
+      auto load_b = [&](int it, uint32_t inf) {
+        const uint32_t b_dst = smem_base + (uint32_t)(it % S) * p.slot_bytes + kSparseStageBytes;
+        const int k0 = (int)(inf & 0x7FFFFFFFu);
+        tma_load_2d(b_dst, &tmap_b, k0, 0, full_bar(it % S), pol_a);
+        if (inf >> 31) tma_load_2d(b_dst + b_tile_bytes, &tmap_b, k0 + 128, 0, full_bar(it % S), pol_a);
+      };
+      // Weights never depend on the previous kernel of the stream, activations do: fill the whole ring with
+      // weight stages, then wait for the previous kernel and add the activation tiles.
+      auto flush = [&]() {
+        trace(p, span, 1);
+        pdl_wait();
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+          if (k < pre) load_b(k, info[k]);
+      };
+#pragma unroll 1
+      for (int it = 0; it < n; ++it) {
+        if (it == pre) flush();
+        const bool sp = c.j < c.ns;
+        const uint32_t wb = sp ? (uint32_t)kSparseStageBytes : (uint32_t)kDenseStageBytes;
+        const uint32_t inf = (uint32_t)(sp ? c.j * kSparseStageK : p.dense_k0 + (c.j - c.ns) * kDenseStageK) | (sp ? 0x80000000u : 0u);
+        const int slot = it % S;
+        if (it >= pre) mbar_wait(empty_bar(slot), ((uint32_t)(it / S) & 1u) ^ 1u);
+        mbar_expect_tx(full_bar(slot), wb + (sp ? 2u : 1u) * b_tile_bytes);
+        bulk_g2s(smem_base + (uint32_t)slot * p.slot_bytes, src, wb, full_bar(slot), pol_w);
+        if (it >= pre) {
+          load_b(it, inf);
+        } else {
+#pragma unroll
+          for (int k = 0; k < 8; ++k)
+            if (k == it) info[k] = inf;
+        }
+        src += wb;
+        if (++c.j == c.ns + c.nd) next_tile<MODE>(p, c);
+      }
+      if (n <= pre) flush();
+      trace(p, span, 2);
+      // HBM goes idle while the CTAs run their fix-up tails: use that time to pull the first stages of
+      // the NEXT kernel's span into L2 (the next GEMM of this layer / the next layer's gate_up).
+      if (p.next_base) {
+        const uint8_t* nb = p.next_base + (size_t)p.next_off[span];
+        const uint32_t bytes = p.next_len[span];
+#pragma unroll 1
+        for (uint32_t o = 0; o < bytes; o += 32768u) {
+          const uint32_t chunk = bytes - o < 32768u ? bytes - o : 32768u;
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(nb + o), "r"(chunk) : "memory");
         }
       }
-      trace(p, span, 2);
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     if (lane == 0) {
       const uint32_t idesc_d = (1u << 4) | ((uint32_t)(p.n_pad >> 3) << 17) | ((128u >> 4) << 24);
       const uint32_t idesc_s = idesc_d | (1u << 2);
+      unsigned long long off;
+      Cursor c = cursor_at<MODE>(p, sb, &off);
       int it = 0, seg = 0;
+#pragma unroll 1
       for (int s = sb; s < se; ++seg) {
-        const TileInfo t = tile_of_stage(p, s);
-        const int seg_end = min(se, t.first + t.ns + t.nd);
+        const int tile_end = c.first + c.ns + c.nd;
+        const int seg_end = min(se, tile_end);
         const int buf = seg % p.num_acc_bufs;
         const uint32_t use = (uint32_t)(seg / p.num_acc_bufs);
         mbar_wait(acce_bar(buf), (use & 1u) ^ 1u);         // epilogue has drained this accumulator
@@ -195,8 +294,8 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
         const uint32_t d0 = tmem_base + (uint32_t)(buf * 2 * p.acc_stride);
         const uint32_t d1 = d0 + (uint32_t)p.acc_stride;
         uint32_t acc = 0;
-        for (; s < seg_end; ++s, ++it) {
-          const int j = s - t.first;
+#pragma unroll 1
+        for (; s < seg_end; ++s, ++it, ++c.j) {
           const int slot = it % S;
           const uint32_t ph = (uint32_t)(it / S) & 1u;
           mbar_wait(full_bar(slot), ph);
@@ -205,7 +304,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
           const uint32_t a0 = smem_base + (uint32_t)slot * p.slot_bytes;
           const uint32_t a1 = a0 + kOperandBytes;
           const uint32_t b0 = a0 + kSparseStageBytes;
-          if (j < t.ns) {
+          if (c.j < c.ns) {
             const uint32_t e_base = tmem_base + kMetaCol + (uint32_t)(it & 1) * 16u;
             const uint32_t m0 = a0 + 2 * kOperandBytes;   // A0 meta: 2 atoms of 2 KB, then A1 meta
 #pragma unroll
@@ -230,6 +329,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
           tc_commit(empty_bar(slot));                     // smem slot free once these MMAs have read it
         }
         tc_commit(accf_bar(buf));                         // accumulator complete for this segment
+        if (s == tile_end) next_tile<MODE>(p, c);
       }
       trace(p, span, 4);
     }
@@ -240,48 +340,109 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
     const int half = (warp - 4) >> 2;
     const int row = q * 32 + lane;                         // accumulator lane = weight row inside the tile
     const int et = threadIdx.x - 128;                      // 0..255
-    const int cols_half = p.n_pad >> 1;                    // multiple of 8
-    const int c_begin = half * cols_half;
-    float* sc = reinterpret_cast<float*>(smem_gen + (size_t)S * p.slot_bytes + 256);   // [4][n_pad] per-token scales
+    const int cols_used = min(p.n_pad, (p.M + 7) & ~7);    // token columns holding real tokens, rounded to the TMEM load width
+    const int c_begin = half * (p.n_pad >> 1);
+    const int c_end = min(c_begin + (p.n_pad >> 1), cols_used);
+    float* sc = reinterpret_cast<float*>(smem_gen + ring_bytes + 256);   // [4][n_pad] per-token scales
+    const float* stg = reinterpret_cast<const float*>(smem_gen);         // the stage ring doubles as partial staging
+    const size_t part_floats = (size_t)2 * p.n_pad * 128;  // one partial: [mat][col][row]
+
+    // scales, the workspace and the epoch word may be produced / still in use by the previous kernel
+    pdl_wait();
+    if (et < p.n_pad) {
+      const int m = et < p.M ? et : p.M - 1;
+      if (MODE == 0) {
+        const float sx = __ldg(p.s_act + m);
+        sc[et] = sx * p.w_scale0;
+        sc[p.n_pad + et] = sx * p.w_scale1;
+        const float sh = __ldg(p.s_h + (size_t)m * p.sh_stride);
+        sc[2 * p.n_pad + et] = sh;
+        sc[3 * p.n_pad + et] = __frcp_rn(sh);
+      } else {
+        sc[et] = __ldg(p.s_act + (size_t)m * p.sh_stride) * p.w_scale0;
+      }
+    }
+    if (et == 255) {
+      // Epoch of this launch = epoch word + 1.  Every CTA reads the word BEFORE it counts itself; the CTA
+      // that counts last therefore knows all have read it and advances it for the next launch.
+      const int e = ld_acquire(p.ws_ctrl);
+      *epoch_ptr = e + 1;
+      if (atomicAdd(p.ws_ctrl + 1, 1) == p.n_spans - 1) {
+        p.ws_ctrl[1] = 0;
+        st_release(p.ws_ctrl, e + 1);
+      }
+    }
+    epi_sync();
+    const int epoch = *epoch_ptr;                          // flag value of THIS launch (never equals a stale flag)
+
+    Group groups[2];
+    int n_groups = 0;
+    uint32_t red_round = 0;                                // uses of the staging barrier so far
+    unsigned long long off;
+    Cursor cur = cursor_at<MODE>(p, sb, &off);
     int seg = 0;
-    bool waited = false;
-    uint32_t stage_round = 0;                              // parity of the partial-staging barriers
+#pragma unroll 1
     for (int s = sb; s < se; ++seg) {
-      const TileInfo t = tile_of_stage(p, s);
-      const int tile_end = t.first + t.ns + t.nd;
+      const int tile_end = cur.first + cur.ns + cur.nd;
       const int seg_end = min(se, tile_end);
-      const bool owner = (s == t.first);
       const int buf = seg % p.num_acc_bufs;
       const uint32_t use = (uint32_t)(seg / p.num_acc_bufs);
-      if (!waited) {
-        // scales and the workspace may be produced / still in use by the previous kernel of the stream
-        pdl_wait();
-        waited = true;
-        if (et < p.n_pad) {
-          const int m = et < p.M ? et : p.M - 1;
-          if (p.mode == 0) {
-            const float sx = __ldg(p.s_act + m);
-            sc[et] = sx * p.w_scale0;
-            sc[p.n_pad + et] = sx * p.w_scale1;
-            const float sh = __ldg(p.s_h + (size_t)m * p.sh_stride);
-            sc[2 * p.n_pad + et] = sh;
-            sc[3 * p.n_pad + et] = __frcp_rn(sh);
-          } else {
-            sc[et] = __ldg(p.s_act + (size_t)m * p.sh_stride) * p.w_scale0;
-          }
-        }
-        asm volatile("bar.sync 1, 256;" ::: "memory");
-      }
+      // spans [a, b] that hold stages of this tile
+      int a = span, b = span;
+      while (p.span_begin[a] > cur.first) --a;
+      while (b + 1 < p.n_spans && p.span_begin[b + 1] < tile_end) ++b;
+
       mbar_wait(accf_bar(buf), use & 1u);
       tc_fence_after();
       if (et == 0) trace(p, span, seg == 0 ? 5 : 7);
       const uint32_t t0 = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 2 * p.acc_stride);
       const uint32_t t1 = t0 + (uint32_t)p.acc_stride;
 
-      if (!owner) {
-        // contributor: dump the raw fp32 partial [mat][col][row], then publish
-        float* slot = p.partials + (size_t)span * (2 * p.n_pad * 128);
-        for (int c = c_begin; c < c_begin + cols_half; c += 8) {
+      if (a == b || (b == a + 1 && span == a)) {
+        // the whole tile is ours, or we own a tile whose tail the next span has (usually long ago) dumped
+        const bool add = a != b;
+        if (add) {
+          // Owner of a split tile = last segment of the span: every MMA of this CTA is complete, the ring is free.
+          if (et == 0) {
+            const int* f = p.flags + b * 2;                // span b starts inside the tile: its first segment
+            while (ld_acquire(f) != epoch) {}
+            const float* part = p.partials + (size_t)b * 2 * part_floats;
+            mbar_expect_tx(red_bar, 2u * (uint32_t)cols_used * 512u);
+            bulk_g2s(smem_base, part, (uint32_t)cols_used * 512u, red_bar, policy_evict_first());
+            bulk_g2s(smem_base + (uint32_t)cols_used * 512u, part + (size_t)p.n_pad * 128, (uint32_t)cols_used * 512u, red_bar, policy_evict_first());
+          }
+          mbar_wait(red_bar, red_round & 1u);
+          ++red_round;
+          if (et == 0) trace(p, span, 8);
+        }
+#pragma unroll 1
+        for (int c = c_begin; c < c_end; c += 8) {
+          uint32_t v0[8], v1[8];
+          tmem_ld8(t0 + c, v0);
+          tmem_ld8(t1 + c, v1);
+          tmem_ld_wait();
+          float f0[8], f1[8];
+#pragma unroll
+          for (int i = 0; i < 8; ++i) { f0[i] = __uint_as_float(v0[i]); f1[i] = __uint_as_float(v1[i]); }
+          if (add) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              f0[i] += stg[(size_t)(c + i) * 128 + row];
+              f1[i] += stg[(size_t)(cols_used + c + i) * 128 + row];
+            }
+          }
+#pragma unroll
+          for (int i = 0; i < 8; ++i)
+            if (c + i < p.M) finish<MODE>(p, sc, cur.tile, row, c + i, f0[i], f1[i]);
+        }
+        tc_fence_before();
+        mbar_arrive(acce_bar(buf));
+      } else {
+        // split tile, not (solely) ours to finish: dump the raw fp32 partial [mat][col][row] and publish it
+        const int which = (sb >= cur.first) ? 0 : 1;       // our first segment, or our last one
+        float* slot = p.partials + ((size_t)span * 2 + which) * part_floats;
+#pragma unroll 1
+        for (int c = c_begin; c < c_end; c += 8) {
           uint32_t v0[8], v1[8];
           tmem_ld8(t0 + c, v0);
           tmem_ld8(t1 + c, v1);
@@ -294,120 +455,70 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
         }
         tc_fence_before();
         mbar_arrive(acce_bar(buf));
-        asm volatile("bar.sync 1, 256;" ::: "memory");     // all partial stores issued (CTA scope) ...
-        if (et == 0) {                                     // ... one gpu-scope release publishes them (cumulativity)
-          __threadfence();
-          asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p.flags + span), "r"(1) : "memory");
+        epi_sync();                                        // all partial stores issued (CTA scope) ...
+        if (et == 0) st_release(p.flags + span * 2 + which, epoch);   // ... one gpu-scope release publishes them (cumulativity)
+        if (b > a + 1) {
+          groups[n_groups].a = a; groups[n_groups].b = b; groups[n_groups].tile = cur.tile; groups[n_groups].first = cur.first;
+          ++n_groups;
         }
-      } else {
-        // owner.  Contributors are the following spans that start inside this tile; that can only
-        // happen on the CTA's last segment, when the whole stage ring is free: stage their partials
-        // into shared memory with bulk copies (one L2 round trip for all of them), then add in span order.
-        int n_contrib = 0;
-        while (span + 1 + n_contrib < p.n_spans && p.span_begin[span + 1 + n_contrib] < tile_end) ++n_contrib;
-        const uint32_t region_bytes = (uint32_t)p.n_pad * 1024u;
-        int n_regions = (int)(((uint32_t)S * p.slot_bytes) / region_bytes);
-        n_regions = n_regions > 8 ? 8 : n_regions;
-        const int out_row = (p.mode == 0) ? (t.tile * 128 + row) : (t.tile * 256 + row);
-        int base = 0;
-        do {
-          const int cnt = min(n_regions, n_contrib - base);
-          if (cnt > 0) {
-            if (base > 0) {                                // regions are being reused: order our reads before the new async writes
-              fence_proxy_async();
-              asm volatile("bar.sync 1, 256;" ::: "memory");
-            }
-            if (et < cnt) {
-              const int* f = p.flags + span + 1 + base + et;
-              int v;
-              do {
-                asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(f) : "memory");
-              } while (v == 0);
-              asm volatile("st.relaxed.gpu.global.s32 [%0], %1;" ::"l"(f), "r"(0) : "memory");   // leave the workspace clean
-              mbar_expect_tx(part_bar(et), region_bytes);
-              bulk_g2s(smem_base + (uint32_t)et * region_bytes, p.partials + (size_t)(span + 1 + base + et) * (2 * p.n_pad * 128),
-                       region_bytes, part_bar(et), policy_evict_first());
-            }
-            for (int r = 0; r < cnt; ++r) mbar_wait(part_bar(r), stage_round & 1u);
-            ++stage_round;
-            if (et == 0 && base == 0) trace(p, span, 8);
-          }
-          const bool last_round = base + cnt >= n_contrib;
-          for (int c = c_begin; c < c_begin + cols_half; c += 8) {
-            uint32_t v0[8], v1[8];
-            tmem_ld8(t0 + c, v0);
-            tmem_ld8(t1 + c, v1);
-            tmem_ld_wait();
-            float f0[8], f1[8];
-#pragma unroll
-            for (int i = 0; i < 8; ++i) { f0[i] = __uint_as_float(v0[i]); f1[i] = __uint_as_float(v1[i]); }
-            for (int r = 0; r < cnt; ++r) {                // fixed span order: deterministic
-              const float* reg = reinterpret_cast<const float*>(smem_gen + (size_t)r * region_bytes);
-#pragma unroll
-              for (int i = 0; i < 8; ++i) {
-                f0[i] += reg[(size_t)(c + i) * 128 + row];
-                f1[i] += reg[(size_t)(p.n_pad + c + i) * 128 + row];
-              }
-            }
-            if (!last_round) {                             // more contributors than staging regions: park the sum in TMEM
-#pragma unroll
-              for (int i = 0; i < 8; ++i) { v0[i] = __float_as_uint(f0[i]); v1[i] = __float_as_uint(f1[i]); }
-              tmem_st8(t0 + c, v0);
-              tmem_st8(t1 + c, v1);
-              continue;
-            }
-            if (p.mode == 0) {
-#pragma unroll
-              for (int i = 0; i < 8; i += 2) {
-                float h[2], qv[2];
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                  const int m = c + i + e;
-                  const float g = f0[i + e] * sc[m];
-                  const float u = f1[i + e] * sc[p.n_pad + m];
-                  h[e] = silu_mul(g, u);
-                  qv[e] = div_by(h[e], sc[2 * p.n_pad + m], sc[3 * p.n_pad + m]);
-                }
-                const uint32_t qb = to_e4m3x2(qv[0], qv[1]);
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                  const int m = c + i + e;
-                  if (m < p.M) {
-                    const size_t o = (size_t)m * p.ld_out + out_row;
-                    if (p.h_f32) p.h_f32[o] = h[e];
-                    p.hq[o] = (uint8_t)(qb >> (8 * e));
-                  }
-                }
-              }
-            } else {
-#pragma unroll
-              for (int i = 0; i < 8; ++i) {
-                const int m = c + i;
-                if (m < p.M) {
-                  const float scl = sc[m];
-                  const float y0 = f0[i] * scl, y1 = f1[i] * scl;
-                  const size_t o = (size_t)m * p.ld_out + out_row;
-                  if (p.y_dtype == SPENSE_F32) {
-                    float* y = reinterpret_cast<float*>(p.y);
-                    y[o] = y0;
-                    if (out_row + 128 < p.out_rows) y[o + 128] = y1;
-                  } else {
-                    __nv_bfloat16* y = reinterpret_cast<__nv_bfloat16*>(p.y);
-                    y[o] = __float2bfloat16_rn(y0);
-                    if (out_row + 128 < p.out_rows) y[o + 128] = __float2bfloat16_rn(y1);
-                  }
-                }
-              }
-            }
-          }
-          if (!last_round) tmem_st_wait();
-          base += cnt;
-        } while (base < n_contrib);
-        tc_fence_before();
-        mbar_arrive(acce_bar(buf));
       }
-      if (et == 0) trace(p, span, seg == 0 ? 6 : 9);
+      if (et == 0) trace(p, span, 6);
       s = seg_end;
+      if (s == tile_end) next_tile<MODE>(p, cur);
+    }
+
+    // ---- deferred reduce-scatter of tiles shared by > 2 spans: span j of the group reduces token columns
+    // [j*M/n, (j+1)*M/n), adding the n partials in span order, and runs the epilogue on them.
+    // All MMAs of this CTA are complete here, so the stage ring is free to stage the partial slices.
+#pragma unroll 1
+    for (int gi = 0; gi < n_groups; ++gi) {
+      const Group g = groups[gi];
+      const int n = g.b - g.a + 1;
+      const int j = span - g.a;
+      const int m0 = (int)(((long long)j * p.M) / n), m1 = (int)(((long long)(j + 1) * p.M) / n);
+      // wait until every span of the group has published its partial of this launch
+#pragma unroll 1
+      for (int i = et; i < n; i += 256) {
+        const int qs = g.a + i;
+        const int* f = p.flags + qs * 2 + ((p.span_begin[qs] >= g.first) ? 0 : 1);
+        while (ld_acquire(f) != epoch) {}
+      }
+      epi_sync();
+      if (et == 0) trace(p, span, 8);
+      if (m1 <= m0) continue;
+      int cc_max = (int)(ring_bytes / ((uint32_t)n * 1024u));
+      if (cc_max > m1 - m0) cc_max = m1 - m0;
+#pragma unroll 1
+      for (int mc = m0; mc < m1; mc += cc_max) {
+        const int cc = min(cc_max, m1 - mc);
+        if (red_round > 0) {                               // staging smem is reused: order our reads before the async writes
+          fence_proxy_async();
+          epi_sync();
+        }
+        if (et == 0) mbar_expect_tx(red_bar, (uint32_t)n * 2u * (uint32_t)cc * 512u);
+#pragma unroll 1
+        for (int i = et; i < 2 * n; i += 256) {
+          const int qs = g.a + (i >> 1), mat = i & 1;
+          const int which = (p.span_begin[qs] >= g.first) ? 0 : 1;
+          const float* src = p.partials + ((size_t)qs * 2 + which) * part_floats + ((size_t)mat * p.n_pad + mc) * 128;
+          bulk_g2s(smem_base + (uint32_t)(i * cc) * 512u, src, (uint32_t)cc * 512u, red_bar, policy_evict_first());
+        }
+        mbar_wait(red_bar, red_round & 1u);
+        ++red_round;
+        if (et == 0) trace(p, span, 15);
+        const int rrow = et & 127;
+#pragma unroll 1
+        for (int c = et >> 7; c < cc; c += 2) {
+          float f0 = 0.0f, f1 = 0.0f;
+#pragma unroll 2
+          for (int qi = 0; qi < n; ++qi) {                 // fixed span order: deterministic
+            f0 += stg[((size_t)(2 * qi) * cc + c) * 128 + rrow];
+            f1 += stg[((size_t)(2 * qi + 1) * cc + c) * 128 + rrow];
+          }
+          finish<MODE>(p, sc, g.tile, rrow, mc + c, f0, f1);
+        }
+      }
+      if (et == 0) trace(p, span, 9);
     }
     if (p.trace && et == 0) { p.trace[(size_t)span * 16 + 10] = seg; p.trace[(size_t)span * 16 + 11] = se - sb; p.trace[(size_t)span * 16 + 13] = globaltimer(); }
   }
@@ -421,7 +532,8 @@ int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, bool pdl, cudaSt
   const size_t smem = (size_t)p.num_stages * p.slot_bytes + 1024 + 256 + 4 * 4 * (size_t)p.n_pad;
   static bool attr_set = false;
   if (!attr_set) {
-    if (cudaFuncSetAttribute(spense_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 232448) != cudaSuccess)
+    if (cudaFuncSetAttribute(spense_gemm_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 232448) != cudaSuccess ||
+        cudaFuncSetAttribute(spense_gemm_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 232448) != cudaSuccess)
       return SPENSE_ERR_CUDA;
     attr_set = true;
   }
@@ -435,8 +547,9 @@ int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, bool pdl, cudaSt
   attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  if (cudaLaunchKernelEx(&cfg, spense_gemm_kernel, p, tmap_b) != cudaSuccess) return SPENSE_ERR_CUDA;
-  return SPENSE_OK;
+  const cudaError_t e = p.mode == 0 ? cudaLaunchKernelEx(&cfg, spense_gemm_kernel<0>, p, tmap_b)
+                                    : cudaLaunchKernelEx(&cfg, spense_gemm_kernel<1>, p, tmap_b);
+  return e == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;
 }
 
 }  // namespace spense

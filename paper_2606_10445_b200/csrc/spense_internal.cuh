@@ -36,7 +36,7 @@ constexpr int kBlobHeaderBytes = 1024;
 constexpr uint32_t kBlobMagic = 0x53504E53u;  // "SNPS"
 constexpr int kBlobVersion = 1;
 constexpr int kMaxSpans = 160;
-constexpr int kFlagBytes = 4096;
+constexpr int kFlagBytes = 4096;             // control words (128 B) + 2 flags per span
 
 struct BlobHeader {
   uint32_t magic;
@@ -105,10 +105,14 @@ struct GemmParams {
   int y_dtype;
   int ld_out;               // I (mode 0) or H (mode 1)
   int out_rows;             // valid output columns (I or H) for masking padded tiles
-  float* partials;          // workspace: n_spans slots of 2 * n_pad * 128 floats
-  int* flags;               // workspace: n_spans ints, zero between launches
+  int* ws_ctrl;             // workspace control words: [0] epoch of the last finished launch, [1] finished-CTA count
+  int* flags;               // workspace: 2 ints per span (first / last segment), hold the epoch of the dump
+  float* partials;          // workspace: 2 slots per span of 2 * n_pad * 128 floats
   long long* trace;         // debug timeline (16 slots per span) or nullptr
+  const uint8_t* next_base; // section the NEXT kernel of the stream will stream (L2 prefetch during our tail) or nullptr
   int span_begin[kMaxSpans + 1];
+  uint32_t next_off[kMaxSpans];   // byte offset of span i's first stage in next_base ...
+  uint32_t next_len[kMaxSpans];   // ... and how many bytes of it to prefetch
 };
 
 // ------------------------------------------------------------------------------------------

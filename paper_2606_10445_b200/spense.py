@@ -66,12 +66,12 @@ def lib() -> ctypes.CDLL:
         L.spense_gate_up.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_int32, c_void_p, c_int32,
                                      c_void_p, c_void_p, c_void_p, c_size_t, c_void_p]
         L.spense_down.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_void_p, c_int32,
-                                  c_void_p, c_size_t, c_void_p]
+                                  c_void_p, c_size_t, c_void_p, c_void_p]
         L.spense_mlp.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_int32, c_void_p, c_int32, c_void_p,
-                                 c_void_p, c_void_p, c_int32, c_void_p, c_size_t, c_void_p]
+                                 c_void_p, c_void_p, c_int32, c_void_p, c_size_t, c_void_p, c_void_p]
         L.spense_mlp_host.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_int32, c_void_p, c_int32,
                                       c_void_p, c_int32, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_size_t,
-                                      c_void_p]
+                                      c_void_p, c_void_p]
         L.spense_quantize_e4m3.argtypes = [c_void_p, c_int64, c_int64, c_int32, c_void_p, c_void_p, c_void_p,
                                            c_size_t, c_void_p]
         for name in EXPORTS:
@@ -181,18 +181,25 @@ def spense_gate_up(layer: PackedLayer, x, s_x, s_h, ws, hq=None, h_f32=None):
     return hq
 
 
-def spense_down(layer: PackedLayer, hq, s_h, ws, y=None, dtype=torch.float32):
+def _next(next_layer):
+    return None if next_layer is None else c_void_p(next_layer.blob.data_ptr())
+
+
+def spense_down(layer: PackedLayer, hq, s_h, ws, y=None, dtype=torch.float32, next_layer=None):
     _dev(hq, torch.uint8), _dev(s_h, torch.float32)
     M = hq.shape[0]
     if y is None:
         y = torch.empty(M, layer.H, dtype=dtype, device=hq.device)
     stride = 0 if s_h.numel() == 1 else 1
     _check(lib().spense_down(ctypes.byref(layer.shape), _ptr(layer.blob), _ptr(hq), _ptr(s_h), stride, M, _ptr(y),
-                             SPENSE_F32 if y.dtype == torch.float32 else SPENSE_BF16, _ptr(ws), ws.numel(), _stream()))
+                             SPENSE_F32 if y.dtype == torch.float32 else SPENSE_BF16, _ptr(ws), ws.numel(),
+                             _next(next_layer), _stream()))
     return y
 
 
-def spense_mlp(layer: PackedLayer, x, s_x, s_h, ws, hq_scratch=None, y=None, h_f32=None, dtype=torch.float32):
+def spense_mlp(layer: PackedLayer, x, s_x, s_h, ws, hq_scratch=None, y=None, h_f32=None, dtype=torch.float32,
+               next_layer=None):
+    """next_layer: the PackedLayer that runs next on this stream (same shape) or None -- L2 prefetch hint."""
     _dev(x, torch.uint8), _dev(s_x, torch.float32), _dev(s_h, torch.float32)
     M = x.shape[0]
     if hq_scratch is None:
@@ -202,11 +209,12 @@ def spense_mlp(layer: PackedLayer, x, s_x, s_h, ws, hq_scratch=None, y=None, h_f
     stride = 0 if s_h.numel() == 1 else 1
     _check(lib().spense_mlp(ctypes.byref(layer.shape), _ptr(layer.blob), _ptr(x), _ptr(s_x), M, _ptr(s_h), stride,
                             _ptr(hq_scratch), _ptr(h_f32), _ptr(y),
-                            SPENSE_F32 if y.dtype == torch.float32 else SPENSE_BF16, _ptr(ws), ws.numel(), _stream()))
+                            SPENSE_F32 if y.dtype == torch.float32 else SPENSE_BF16, _ptr(ws), ws.numel(),
+                            _next(next_layer), _stream()))
     return y
 
 
-def spense_mlp_host(layer: PackedLayer, h_x, h_sx, h_sh, h_y, staging, ws):
+def spense_mlp_host(layer: PackedLayer, h_x, h_sx, h_sh, h_y, staging, ws, next_layer=None):
     """HOST (pinned) x uint8 [M, H], s_x [M], s_h [1|M] -> HOST y [M, H].  staging = dict of device
     buffers d_x, d_scales, d_hq, d_y.  Synchronises the stream."""
     M = h_x.shape[0]
@@ -214,7 +222,7 @@ def spense_mlp_host(layer: PackedLayer, h_x, h_sx, h_sh, h_y, staging, ws):
     _check(lib().spense_mlp_host(ctypes.byref(layer.shape), _ptr(layer.blob), _ptr(h_x), _ptr(h_sx), M, _ptr(h_sh),
                                  stride, _ptr(h_y), SPENSE_F32 if h_y.dtype == torch.float32 else SPENSE_BF16,
                                  _ptr(staging["d_x"]), _ptr(staging["d_scales"]), _ptr(staging["d_hq"]),
-                                 _ptr(staging["d_y"]), _ptr(ws), ws.numel(), _stream()))
+                                 _ptr(staging["d_y"]), _ptr(ws), ws.numel(), _next(next_layer), _stream()))
     return h_y
 
 

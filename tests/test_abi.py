@@ -63,5 +63,5 @@ def test_size_queries_and_host_side_argument_errors(sp):
     st = L.spense_gate_up(ctypes.byref(shp), None, None, None, 8, None, 0, None, None, None, 0, None)
     assert sp.STATUS[st] == "SPENSE_ERR_ARG"
     st = L.spense_down(ctypes.byref(shp), ctypes.c_void_p(1024), ctypes.c_void_p(3), ctypes.c_void_p(4), 0, 8,
-                       ctypes.c_void_p(16), 0, ctypes.c_void_p(128), 1 << 30, None)
+                       ctypes.c_void_p(16), 0, ctypes.c_void_p(128), 1 << 30, None, None)
     assert sp.STATUS[st] == "SPENSE_ERR_ALIGN"

@@ -24,9 +24,10 @@
 // Span i runs on CTA n_spans-1-i.  CTAs of one launch wait for each other, so all n_spans <= #SM CTAs
 // must be co-resident: 1 CTA/SM by construction (shared memory), the device must not be shared.
 //
-// Warp roles (384 threads): warp 0 producer (bulk copy of the weight stage + TMA of the activation
-// tile), warp 1 MMA issuer, warp 2 TMEM allocator, warps 4-11 epilogue (TMEM lane quadrant = warp & 3,
-// half of the token columns = (warp - 4) >> 2).  Rarely executed code is kept rolled: the kernel is
+// Warp roles (640 threads): warp 0 producer (bulk copy of the weight stage + TMA of the activation
+// tile), warp 1 MMA issuer, warp 2 TMEM allocator, warps 4-19 epilogue (TMEM lane quadrant = warp & 3,
+// quarter of the token columns = (warp - 4) >> 2): the last tile's epilogue is exposed at the end of
+// every CTA and is instruction-issue bound, so it gets 4 warps per scheduler.  Rarely executed code is kept rolled: the kernel is
 // latency-sensitive at its tail and instruction-cache misses on cold paths showed up in the timeline.
 #include <cuda_bf16.h>
 
@@ -127,27 +128,29 @@ __device__ __forceinline__ int ld_acquire(const int* p) {
 __device__ __forceinline__ void st_release(int* p, int v) {
   asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
-__device__ __forceinline__ void epi_sync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }   // the 8 epilogue warps
+__device__ __forceinline__ void epi_sync() { asm volatile("bar.sync 1, 512;" ::: "memory"); }   // the 16 epilogue warps
 
-constexpr int kThreads = 384;
+constexpr int kEpiThreads = 512;                 // 16 epilogue warps: 4 per TMEM lane quadrant
+constexpr int kThreads = 128 + kEpiThreads;
 constexpr int kTmemCols = 512;
 constexpr int kMetaCol = 480;   // 2 buffers x 16 columns of 2:4 metadata
 
 // One output element (token m, weight row r of pair tile `tile`): scales, GLU + requant, or the Y store.
+// sc holds one float4 per token column: MODE 0 {s_x*s_gate, s_x*s_up, s_h, RN(1/s_h)}, MODE 1 {s_h*s_down, -, -, -}.
 template <int MODE>
-__device__ __forceinline__ void finish(const GemmParams& p, const float* sc, int tile, int r, int m, float f0, float f1) {
+__device__ __forceinline__ void finish(const GemmParams& p, const float4* sc, int tile, int r, int m, float f0, float f1) {
+  const float4 k = sc[m];
   if (MODE == 0) {
-    const float g = f0 * sc[m];
-    const float u = f1 * sc[p.n_pad + m];
+    const float g = f0 * k.x;
+    const float u = f1 * k.y;
     const float h = silu_mul(g, u);
-    const float qv = div_by(h, sc[2 * p.n_pad + m], sc[3 * p.n_pad + m]);
+    const float qv = div_by(h, k.z, k.w);
     const size_t o = (size_t)m * p.ld_out + tile * 128 + r;
     if (p.h_f32) p.h_f32[o] = h;
     p.hq[o] = (uint8_t)(to_e4m3x2(qv, 0.0f) & 0xFFu);
   } else {
     const int out_row = tile * 256 + r;
-    const float scl = sc[m];
-    const float y0 = f0 * scl, y1 = f1 * scl;
+    const float y0 = f0 * k.x, y1 = f1 * k.x;
     const size_t o = (size_t)m * p.ld_out + out_row;
     const bool second = out_row + 128 < p.out_rows;
     if (p.y_dtype == SPENSE_F32) {
@@ -192,7 +195,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmap_b);
     for (int s = 0; s < S; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(accf_bar(b), 1); mbar_init(acce_bar(b), 256); }
+    for (int b = 0; b < 2; ++b) { mbar_init(accf_bar(b), 1); mbar_init(acce_bar(b), kEpiThreads); }
     mbar_init(red_bar, 1);
     fence_barrier_init();
   }
@@ -335,15 +338,15 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
     }
   } else if (warp >= 4) {
     // ===================== epilogue (8 warps) =====================
-    // warp & 3 selects the TMEM lane quadrant, (warp - 4) >> 2 the half of the token columns.
+    // warp & 3 selects the TMEM lane quadrant, (warp - 4) >> 2 the quarter of the token columns.
     const int q = warp & 3;
-    const int half = (warp - 4) >> 2;
     const int row = q * 32 + lane;                         // accumulator lane = weight row inside the tile
-    const int et = threadIdx.x - 128;                      // 0..255
+    const int et = threadIdx.x - 128;                      // 0..511
     const int cols_used = min(p.n_pad, (p.M + 7) & ~7);    // token columns holding real tokens, rounded to the TMEM load width
-    const int c_begin = half * (p.n_pad >> 1);
-    const int c_end = min(c_begin + (p.n_pad >> 1), cols_used);
-    float* sc = reinterpret_cast<float*>(smem_gen + ring_bytes + 256);   // [4][n_pad] per-token scales
+    const int cols_per = (((p.n_pad + 3) >> 2) + 7) & ~7;  // columns per warp: a quarter, rounded to the TMEM load width
+    const int c_begin = ((warp - 4) >> 2) * cols_per;
+    const int c_end = min(c_begin + cols_per, cols_used);
+    float4* sc = reinterpret_cast<float4*>(smem_gen + ring_bytes + 256);   // one float4 of scales per token column
     const float* stg = reinterpret_cast<const float*>(smem_gen);         // the stage ring doubles as partial staging
     const size_t part_floats = (size_t)2 * p.n_pad * 128;  // one partial: [mat][col][row]
 
@@ -351,18 +354,17 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
     pdl_wait();
     if (et < p.n_pad) {
       const int m = et < p.M ? et : p.M - 1;
+      float4 k = make_float4(0.f, 0.f, 0.f, 0.f);
       if (MODE == 0) {
         const float sx = __ldg(p.s_act + m);
-        sc[et] = sx * p.w_scale0;
-        sc[p.n_pad + et] = sx * p.w_scale1;
         const float sh = __ldg(p.s_h + (size_t)m * p.sh_stride);
-        sc[2 * p.n_pad + et] = sh;
-        sc[3 * p.n_pad + et] = __frcp_rn(sh);
+        k = make_float4(sx * p.w_scale0, sx * p.w_scale1, sh, __frcp_rn(sh));
       } else {
-        sc[et] = __ldg(p.s_act + (size_t)m * p.sh_stride) * p.w_scale0;
+        k.x = __ldg(p.s_act + (size_t)m * p.sh_stride) * p.w_scale0;
       }
+      sc[et] = k;
     }
-    if (et == 255) {
+    if (et == kEpiThreads - 1) {
       // Epoch of this launch = epoch word + 1.  Every CTA reads the word BEFORE it counts itself; the CTA
       // that counts last therefore knows all have read it and advances it for the next launch.
       const int e = ld_acquire(p.ws_ctrl);
@@ -406,6 +408,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
           if (et == 0) {
             const int* f = p.flags + b * 2;                // span b starts inside the tile: its first segment
             while (ld_acquire(f) != epoch) {}
+            asm volatile("fence.proxy.async.global;" ::: "memory");   // partner's generic-proxy stores -> our async-proxy read
             const float* part = p.partials + (size_t)b * 2 * part_floats;
             mbar_expect_tx(red_bar, 2u * (uint32_t)cols_used * 512u);
             bulk_g2s(smem_base, part, (uint32_t)cols_used * 512u, red_bar, policy_evict_first());
@@ -476,51 +479,46 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
       const int n = g.b - g.a + 1;
       const int j = span - g.a;
       const int m0 = (int)(((long long)j * p.M) / n), m1 = (int)(((long long)(j + 1) * p.M) / n);
-      // wait until every span of the group has published its partial of this launch
+      if (m1 > m0) {
+        int cc_max = (int)(ring_bytes / ((uint32_t)n * 1024u));
+        if (cc_max > m1 - m0) cc_max = m1 - m0;
 #pragma unroll 1
-      for (int i = et; i < n; i += 256) {
-        const int qs = g.a + i;
-        const int* f = p.flags + qs * 2 + ((p.span_begin[qs] >= g.first) ? 0 : 1);
-        while (ld_acquire(f) != epoch) {}
-      }
-      epi_sync();
-      if (et == 0) trace(p, span, 8);
-      if (m1 <= m0) continue;
-      int cc_max = (int)(ring_bytes / ((uint32_t)n * 1024u));
-      if (cc_max > m1 - m0) cc_max = m1 - m0;
-#pragma unroll 1
-      for (int mc = m0; mc < m1; mc += cc_max) {
-        const int cc = min(cc_max, m1 - mc);
-        if (red_round > 0) {                               // staging smem is reused: order our reads before the async writes
-          fence_proxy_async();
-          epi_sync();
-        }
-        if (et == 0) mbar_expect_tx(red_bar, (uint32_t)n * 2u * (uint32_t)cc * 512u);
-#pragma unroll 1
-        for (int i = et; i < 2 * n; i += 256) {
-          const int qs = g.a + (i >> 1), mat = i & 1;
-          const int which = (p.span_begin[qs] >= g.first) ? 0 : 1;
-          const float* src = p.partials + ((size_t)qs * 2 + which) * part_floats + ((size_t)mat * p.n_pad + mc) * 128;
-          bulk_g2s(smem_base + (uint32_t)(i * cc) * 512u, src, (uint32_t)cc * 512u, red_bar, policy_evict_first());
-        }
-        mbar_wait(red_bar, red_round & 1u);
-        ++red_round;
-        if (et == 0) trace(p, span, 15);
-        const int rrow = et & 127;
-#pragma unroll 1
-        for (int c = et >> 7; c < cc; c += 2) {
-          float f0 = 0.0f, f1 = 0.0f;
-#pragma unroll 2
-          for (int qi = 0; qi < n; ++qi) {                 // fixed span order: deterministic
-            f0 += stg[((size_t)(2 * qi) * cc + c) * 128 + rrow];
-            f1 += stg[((size_t)(2 * qi + 1) * cc + c) * 128 + rrow];
+        for (int mc = m0; mc < m1; mc += cc_max) {
+          const int cc = min(cc_max, m1 - mc);
+          if (red_round > 0) {                             // staging smem is reused: order our reads before the async writes
+            fence_proxy_async();
+            epi_sync();
           }
-          finish<MODE>(p, sc, g.tile, rrow, mc + c, f0, f1);
+          if (et == 0) mbar_expect_tx(red_bar, (uint32_t)n * 2u * (uint32_t)cc * 512u);
+          // thread i fetches matrix (i & 1) of partner (i >> 1) as soon as THAT partner has published
+#pragma unroll 1
+          for (int i = et; i < 2 * n; i += kEpiThreads) {
+            const int qs = g.a + (i >> 1), mat = i & 1;
+            const int which = (p.span_begin[qs] >= g.first) ? 0 : 1;
+            while (ld_acquire(p.flags + qs * 2 + which) != epoch) {}
+            asm volatile("fence.proxy.async.global;" ::: "memory");   // partner's generic-proxy stores -> our async-proxy read
+            const float* src = p.partials + ((size_t)qs * 2 + which) * part_floats + ((size_t)mat * p.n_pad + mc) * 128;
+            bulk_g2s(smem_base + (uint32_t)(i * cc) * 512u, src, (uint32_t)cc * 512u, red_bar, policy_evict_first());
+          }
+          mbar_wait(red_bar, red_round & 1u);
+          ++red_round;
+          if (et == 0) trace(p, span, 15);
+          const int rrow = et & 127;
+#pragma unroll 1
+          for (int c = et >> 7; c < cc; c += kEpiThreads >> 7) {
+            float f0 = 0.0f, f1 = 0.0f;
+#pragma unroll 4
+            for (int qi = 0; qi < n; ++qi) {               // fixed span order: deterministic
+              f0 += stg[((size_t)(2 * qi) * cc + c) * 128 + rrow];
+              f1 += stg[((size_t)(2 * qi + 1) * cc + c) * 128 + rrow];
+            }
+            finish<MODE>(p, sc, g.tile, rrow, mc + c, f0, f1);
+          }
         }
       }
       if (et == 0) trace(p, span, 9);
     }
-    if (p.trace && et == 0) { p.trace[(size_t)span * 16 + 10] = seg; p.trace[(size_t)span * 16 + 11] = se - sb; p.trace[(size_t)span * 16 + 13] = globaltimer(); }
+    if (p.trace && et == 0) { p.trace[(size_t)span * 16 + 10] = clock64(); p.trace[(size_t)span * 16 + 11] = (se - sb) | (seg << 16); p.trace[(size_t)span * 16 + 13] = globaltimer(); }
   }
 
   tc_fence_before();

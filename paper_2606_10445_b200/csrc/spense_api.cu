@@ -99,6 +99,11 @@ const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms) {
   if (spans > total) spans = total;
   double sum = 0;
   for (double c : cost) sum += c;
+  // stages per pair tile, to bound how many spans can share one tile (the kernel stages one 1 KB column
+  // slice per sharing span in half of its ring: at most kMaxShare spans per tile)
+  const int kMaxShare = 64;
+  const int num_tiles = mode == 0 ? g.gu_tiles : g.dn_tiles;
+  if (spans > kMaxShare * num_tiles / 2) spans = kMaxShare * num_tiles / 2 > 0 ? kMaxShare * num_tiles / 2 : 1;
   sc.n_spans = spans;
   double acc = 0;
   int s = 0;

@@ -186,7 +186,8 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
   auto empty_bar = [&](int s) { return bar_base + 8u * (8 + s); };
   auto accf_bar = [&](int b) { return bar_base + 8u * (16 + b); };
   auto acce_bar = [&](int b) { return bar_base + 8u * (18 + b); };
-  const uint32_t red_bar = bar_base + 8u * 22;
+  const uint32_t own_bar = bar_base + 8u * 22;   // owner-path staging of one partial
+  const uint32_t red_bar = bar_base + 8u * 23;   // two barriers: reduce-scatter double buffer
   const uint32_t tmem_slot = bar_base + 8u * 20;
   uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
   volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(smem_gen + ring_bytes + 8 * 20);
@@ -196,7 +197,9 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
     prefetch_tmap(&tmap_b);
     for (int s = 0; s < S; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(accf_bar(b), 1); mbar_init(acce_bar(b), kEpiThreads); }
+    mbar_init(own_bar, 1);
     mbar_init(red_bar, 1);
+    mbar_init(red_bar + 8, 1);
     fence_barrier_init();
   }
   if (warp == 2) tmem_alloc(tmem_slot, kTmemCols);
@@ -379,7 +382,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
 
     Group groups[2];
     int n_groups = 0;
-    uint32_t red_round = 0;                                // uses of the staging barrier so far
+    bool own_used = false;                                 // the owner path has staged a partial through the ring
     unsigned long long off;
     Cursor cur = cursor_at<MODE>(p, sb, &off);
     int seg = 0;
@@ -410,12 +413,12 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
             while (ld_acquire(f) != epoch) {}
             asm volatile("fence.proxy.async.global;" ::: "memory");   // partner's generic-proxy stores -> our async-proxy read
             const float* part = p.partials + (size_t)b * 2 * part_floats;
-            mbar_expect_tx(red_bar, 2u * (uint32_t)cols_used * 512u);
-            bulk_g2s(smem_base, part, (uint32_t)cols_used * 512u, red_bar, policy_evict_first());
-            bulk_g2s(smem_base + (uint32_t)cols_used * 512u, part + (size_t)p.n_pad * 128, (uint32_t)cols_used * 512u, red_bar, policy_evict_first());
+            mbar_expect_tx(own_bar, 2u * (uint32_t)cols_used * 512u);
+            bulk_g2s(smem_base, part, (uint32_t)cols_used * 512u, own_bar, policy_evict_first());
+            bulk_g2s(smem_base + (uint32_t)cols_used * 512u, part + (size_t)p.n_pad * 128, (uint32_t)cols_used * 512u, own_bar, policy_evict_first());
           }
-          mbar_wait(red_bar, red_round & 1u);
-          ++red_round;
+          mbar_wait(own_bar, 0);                           // a span owns at most one split tile (its last segment)
+          own_used = true;
           if (et == 0) trace(p, span, 8);
         }
 #pragma unroll 1
@@ -472,49 +475,74 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
 
     // ---- deferred reduce-scatter of tiles shared by > 2 spans: span j of the group reduces token columns
     // [j*M/n, (j+1)*M/n), adding the n partials in span order, and runs the epilogue on them.
-    // All MMAs of this CTA are complete here, so the stage ring is free to stage the partial slices.
-#pragma unroll 1
-    for (int gi = 0; gi < n_groups; ++gi) {
-      const Group g = groups[gi];
-      const int n = g.b - g.a + 1;
-      const int j = span - g.a;
-      const int m0 = (int)(((long long)j * p.M) / n), m1 = (int)(((long long)(j + 1) * p.M) / n);
-      if (m1 > m0) {
-        int cc_max = (int)(ring_bytes / ((uint32_t)n * 1024u));
-        if (cc_max > m1 - m0) cc_max = m1 - m0;
-#pragma unroll 1
-        for (int mc = m0; mc < m1; mc += cc_max) {
-          const int cc = min(cc_max, m1 - mc);
-          if (red_round > 0) {                             // staging smem is reused: order our reads before the async writes
-            fence_proxy_async();
-            epi_sync();
-          }
-          if (et == 0) mbar_expect_tx(red_bar, (uint32_t)n * 2u * (uint32_t)cc * 512u);
-          // thread i fetches matrix (i & 1) of partner (i >> 1) as soon as THAT partner has published
-#pragma unroll 1
-          for (int i = et; i < 2 * n; i += kEpiThreads) {
-            const int qs = g.a + (i >> 1), mat = i & 1;
-            const int which = (p.span_begin[qs] >= g.first) ? 0 : 1;
-            while (ld_acquire(p.flags + qs * 2 + which) != epoch) {}
-            asm volatile("fence.proxy.async.global;" ::: "memory");   // partner's generic-proxy stores -> our async-proxy read
-            const float* src = p.partials + ((size_t)qs * 2 + which) * part_floats + ((size_t)mat * p.n_pad + mc) * 128;
-            bulk_g2s(smem_base + (uint32_t)(i * cc) * 512u, src, (uint32_t)cc * 512u, red_bar, policy_evict_first());
-          }
-          mbar_wait(red_bar, red_round & 1u);
-          ++red_round;
-          if (et == 0) trace(p, span, 15);
-          const int rrow = et & 127;
-#pragma unroll 1
-          for (int c = et >> 7; c < cc; c += kEpiThreads >> 7) {
-            float f0 = 0.0f, f1 = 0.0f;
-#pragma unroll 4
-            for (int qi = 0; qi < n; ++qi) {               // fixed span order: deterministic
-              f0 += stg[((size_t)(2 * qi) * cc + c) * 128 + rrow];
-              f1 += stg[((size_t)(2 * qi + 1) * cc + c) * 128 + rrow];
-            }
-            finish<MODE>(p, sc, g.tile, rrow, mc + c, f0, f1);
-          }
+    // All MMAs of this CTA are complete here, so the stage ring is free: its two halves double-buffer the
+    // partial slices (the fetch of the next chunk / next group overlaps the arithmetic of this one).
+    if (n_groups > 0) {
+      const uint32_t half_bytes = (ring_bytes >> 1) & ~1023u;
+      // chunk cursor: (group, first column, columns); both cursors walk the same sequence
+      auto advance = [&](int& gi, int& mc, int& cc) -> bool {
+        while (gi < n_groups) {
+          const int n = groups[gi].b - groups[gi].a + 1;
+          const int j = span - groups[gi].a;
+          const int m0 = (int)(((long long)j * p.M) / n), m1 = (int)(((long long)(j + 1) * p.M) / n);
+          int ccm = (int)(half_bytes / ((uint32_t)n * 1024u));
+          ccm = ccm < 1 ? 1 : ccm;
+          mc = mc < 0 ? m0 : mc + ccm;
+          if (mc < m1) { cc = min(ccm, m1 - mc); return true; }
+          ++gi; mc = -1;
         }
+        return false;
+      };
+      // thread i of the chunk fetches matrix (i & 1) of partner (i >> 1) as soon as THAT partner has published
+      auto issue = [&](int gi, int mc, int cc, int k) {
+        const Group g = groups[gi];
+        const int n = g.b - g.a + 1;
+        const uint32_t bar = red_bar + 8u * (uint32_t)(k & 1);
+        const uint32_t dst = smem_base + (uint32_t)(k & 1) * half_bytes;
+        if (et == 0) mbar_expect_tx(bar, (uint32_t)n * 2u * (uint32_t)cc * 512u);
+        const int e0 = (et + kEpiThreads - ((k & 1) << 8)) & (kEpiThreads - 1);   // chunks in flight poll from different threads
+#pragma unroll 1
+        for (int i = e0; i < 2 * n; i += kEpiThreads) {
+          const int qs = g.a + (i >> 1), mat = i & 1;
+          const int which = (p.span_begin[qs] >= g.first) ? 0 : 1;
+          while (ld_acquire(p.flags + qs * 2 + which) != epoch) {}
+          asm volatile("fence.proxy.async.global;" ::: "memory");   // partner's generic-proxy stores -> our async-proxy read
+          const float* src = p.partials + ((size_t)qs * 2 + which) * part_floats + ((size_t)mat * p.n_pad + mc) * 128;
+          bulk_g2s(dst + (uint32_t)(i * cc) * 512u, src, (uint32_t)cc * 512u, bar, policy_evict_first());
+        }
+      };
+      int gi_i = 0, mc_i = -1, cc_i = 0, k_i = 0;          // issue cursor
+      int gi_c = 0, mc_c = -1, cc_c = 0, k_c = 0;          // consume cursor
+      bool more = advance(gi_i, mc_i, cc_i);
+      if (more) {
+        if (own_used) { fence_proxy_async(); epi_sync(); } // the owner path staged through the same memory
+        issue(gi_i, mc_i, cc_i, k_i++);
+        more = advance(gi_i, mc_i, cc_i);
+      }
+#pragma unroll 1
+      while (advance(gi_c, mc_c, cc_c)) {
+        if (more) {
+          if (k_i >= 2) { fence_proxy_async(); epi_sync(); }   // that half was read two chunks ago: order the reads before the async writes
+          issue(gi_i, mc_i, cc_i, k_i++);
+          more = advance(gi_i, mc_i, cc_i);
+        }
+        mbar_wait(red_bar + 8u * (uint32_t)(k_c & 1), (uint32_t)(k_c >> 1) & 1u);
+        if (et == 0) trace(p, span, 15);
+        const Group g = groups[gi_c];
+        const int n = g.b - g.a + 1;
+        const float* sl = reinterpret_cast<const float*>(smem_gen + (size_t)(k_c & 1) * half_bytes);
+        const int rrow = et & 127;
+#pragma unroll 1
+        for (int c = et >> 7; c < cc_c; c += kEpiThreads >> 7) {
+          float f0 = 0.0f, f1 = 0.0f;
+#pragma unroll 4
+          for (int qi = 0; qi < n; ++qi) {                 // fixed span order: deterministic
+            f0 += sl[((size_t)(2 * qi) * cc_c + c) * 128 + rrow];
+            f1 += sl[((size_t)(2 * qi + 1) * cc_c + c) * 128 + rrow];
+          }
+          finish<MODE>(p, sc, g.tile, rrow, mc_c + c, f0, f1);
+        }
+        ++k_c;
       }
       if (et == 0) trace(p, span, 9);
     }

@@ -183,12 +183,14 @@ def main():
     x, sx = si.make_activations(M, H, 1000 + M, device=dev)
     sh = torch.full((M,), 0.05, device=dev)
     ws = sp.spense_workspace(blobs[0], max(M, 256))
+    ws_dense = None                                      # the all-dense baseline has its own schedule and workspace size
     hq = torch.empty(M, I, dtype=torch.uint8, device=dev)
     y = torch.empty(M, H, dtype=torch.bfloat16, device=dev)
 
-    def step_eager(layers, xx, ssx, ssh, hqq, yy):
+    def step_eager(layers, xx, ssx, ssh, hqq, yy, wsp=None):
+        wsp = ws if wsp is None else wsp
         for i, b in enumerate(layers):                   # the layer that runs next is named as an L2 prefetch hint
-            sp.spense_mlp(b, xx, ssx, ssh, ws, hq_scratch=hqq, y=yy, next_layer=layers[(i + 1) % len(layers)])
+            sp.spense_mlp(b, xx, ssx, ssh, wsp, hq_scratch=hqq, y=yy, next_layer=layers[(i + 1) % len(layers)])
 
     def graph_of(fn):
         fn()                                             # warm: header cache, schedules, func attributes
@@ -241,13 +243,14 @@ def main():
         sweep = []
         if not args.no_sweep:
             dense = make_blobs(1.0, 6, 3000)
+            ws_dense = sp.spense_workspace(dense[0], 256)
             for Ms in (1, 8, 32, 64, 128, 256):
                 xs, sxs = si.make_activations(Ms, H, 1000 + Ms, device=dev)
                 shs = torch.full((Ms,), 0.05, device=dev)
                 hqs = torch.empty(Ms, I, dtype=torch.uint8, device=dev)
                 ys = torch.empty(Ms, H, dtype=torch.bfloat16, device=dev)
                 t_sp = t_us(lambda: step_eager(blobs[:6], xs, sxs, shs, hqs, ys), 6)
-                t_dn = t_us(lambda: step_eager(dense, xs, sxs, shs, hqs, ys), 6)
+                t_dn = t_us(lambda: step_eager(dense, xs, sxs, shs, hqs, ys, ws_dense), 6)
                 sweep.append({"M": Ms, "spense_us": round(t_sp, 2), "dense_us": round(t_dn, 2),
                               "speedup_vs_dense": round(t_dn / t_sp, 3),
                               "spense_gbs": round(algorithmic_bytes(Ms, I_d) / t_sp / 1e3, 1),

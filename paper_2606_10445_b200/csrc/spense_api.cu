@@ -49,101 +49,28 @@ bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) %
 
 int n_pad_of(int M) { int n = (M + 15) / 16 * 16; return n > 128 ? 128 : n; }
 
+size_t ws_bytes_for(int n_pad, int spans) { return kFlagBytes + (size_t)spans * 2 * 2 * n_pad * 128 * sizeof(float); }
+
 double env_double(const char* name, double dflt) {
   const char* v = std::getenv(name);
   return v ? std::atof(v) : dflt;
 }
 
-// schedule knobs (environment at first use; tests override them through spense_debug_set_schedule)
-struct Knobs {
-  double tail_frac;     // share of the streamed cost handed out dynamically
-  int tail_cs;          // stages per tail chunk, 0 = by token count
-  int max_spans;        // cap on the persistent CTAs, 0 = one per SM
-  int min_static;       // the static part keeps at least this many stages
-  double fixed, gamma;  // stage cost model
-};
-Knobs g_knobs = {-1, 0, 0, 0, 0, 0};
-const Knobs& knobs() {
-  if (g_knobs.tail_frac < 0) {
-    g_knobs.tail_frac = env_double("SPENSE_TAIL_FRAC", 0.15);
-    g_knobs.tail_cs = (int)env_double("SPENSE_TAIL_CHUNK", 0);
-    g_knobs.max_spans = (int)env_double("SPENSE_MAX_SPANS", 0);
-    g_knobs.min_static = (int)env_double("SPENSE_MIN_STATIC", 2 * kMaxSpans);
-    g_knobs.fixed = env_double("SPENSE_SCHED_FIXED", 36864.0);
-    g_knobs.gamma = env_double("SPENSE_SCHED_GAMMA", 0.25);
-  }
-  return g_knobs;
-}
-
-int slot_bytes_of(int n_pad) { return kSparseStageBytes + 2 * n_pad * 128; }
-int ring_stages_of(int n_pad) {
-  const int stages = (kSmemMax - 1024 - kSmemTailBytes - 16 * n_pad) / slot_bytes_of(n_pad);
-  return stages > 8 ? 8 : stages;
-}
-
-// ---- the dynamic tail: the last whole tiles of the stage sequence, cut into chunks of tail_cs stages.
-// A pure function of (mode, geometry, token padding, knobs): the workspace size query needs it without a device.
-struct Tail {
-  int tile0, ts, cs, cpt_s, cpt_d, n_chunks, n_tiles;
-  int static_stages;
-};
-
-Tail make_tail(int mode, const Geometry& g, int n_pad) {
-  const Knobs& k = knobs();
-  const int num_tiles = mode == 0 ? g.gu_tiles : g.dn_tiles;
-  const int tiles_sparse = mode == 0 ? g.gu_tiles_sparse : 0;
-  const double cs_cost = k.fixed + kSparseStageBytes + k.gamma * 2.0 * n_pad * 128;
-  const double cd_cost = k.fixed + kDenseStageBytes + k.gamma * 1.0 * n_pad * 128;
-  auto stages_of = [&](int t) { return mode == 0 ? (t < tiles_sparse ? g.gu_ns : g.gu_nd) : g.dn_ns + g.dn_nd; };
-  auto cost_of = [&](int t) {
-    return mode == 0 ? (t < tiles_sparse ? g.gu_ns * cs_cost : g.gu_nd * cd_cost) : g.dn_ns * cs_cost + g.dn_nd * cd_cost;
-  };
-  long long total_stages = 0;
-  double total_cost = 0;
-  for (int t = 0; t < num_tiles; ++t) { total_stages += stages_of(t); total_cost += cost_of(t); }
-  Tail tl = {};
-  tl.tile0 = num_tiles;
-  long long st = total_stages;
-  double acc = 0;
-  while (tl.tile0 > 1 && tl.n_tiles < 64) {
-    const int t = tl.tile0 - 1;
-    const bool fits = acc + cost_of(t) <= k.tail_frac * total_cost ||
-                      (tl.n_tiles == 0 && k.tail_frac > 0 && cost_of(t) <= 0.5 * total_cost);
-    if (!fits || st - stages_of(t) < k.min_static || st - stages_of(t) < 1) break;
-    acc += cost_of(t); st -= stages_of(t);
-    --tl.tile0; ++tl.n_tiles;
-    if (t < tiles_sparse) ++tl.ts;
-  }
-  tl.static_stages = (int)st;
-  if (tl.n_tiles == 0) return tl;
-  int cs = k.tail_cs > 0 ? k.tail_cs : (n_pad <= 16 ? 1 : n_pad <= 32 ? 2 : n_pad <= 64 ? 3 : 4);
-  const int per_s = mode == 0 ? g.gu_ns : g.dn_ns + g.dn_nd, per_d = mode == 0 ? g.gu_nd : g.dn_ns + g.dn_nd;
-  const int per_max = per_s > per_d ? per_s : per_d;
-  if (cs < (per_max + 63) / 64) cs = (per_max + 63) / 64;   // a task stages one 1 KB column slice per partial: <= 64 partials per tile
-  tl.cs = cs;
-  tl.cpt_s = (per_s + cs - 1) / cs;
-  tl.cpt_d = (per_d + cs - 1) / cs;
-  tl.n_chunks = mode == 0 ? tl.ts * tl.cpt_s + (tl.n_tiles - tl.ts) * tl.cpt_d : tl.n_tiles * tl.cpt_s;
-  return tl;
-}
-
-size_t ws_bytes_for(const Geometry& g, int n_pad) {
-  const int c0 = make_tail(0, g, n_pad).n_chunks, c1 = make_tail(1, g, n_pad).n_chunks;
-  return kFlagBytes + ((size_t)2 * kMaxSpans + (c0 > c1 ? c0 : c1)) * 2 * n_pad * 128 * sizeof(float);
-}
-
-// ---- stream-K schedule of the static part: n_spans spans of (nearly) equal cost.
+// ---- stream-K schedule: cut the stage sequence into n_spans spans of (nearly) equal bytes.
 struct Schedule {
   int mode, H, I, I_d, n_pad, sms;
   int n_spans;
-  Tail tail;
-  int n_red, n_red_static;
   int span_begin[kMaxSpans + 1];
   uint32_t span_off[kMaxSpans];   // byte offset of the span's first stage image inside its section
   uint32_t span_pre[kMaxSpans];   // bytes of the stages the producer issues before anything else (one ring)
-  RedEntry red[kMaxRed];
+  uint32_t span_len[kMaxSpans];   // bytes of the whole span
 };
 
+int slot_bytes_of(int n_pad) { return kSparseStageBytes + 2 * n_pad * 128; }
+int ring_stages_of(int n_pad) {
+  const int stages = (232448 - 1024 - 256 - 16 * n_pad) / slot_bytes_of(n_pad);
+  return stages > 8 ? 8 : stages;
+}
 std::mutex g_sched_mu;
 std::vector<Schedule> g_sched;
 
@@ -151,35 +78,26 @@ const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms) {
   std::lock_guard<std::mutex> lk(g_sched_mu);
   for (const Schedule& s : g_sched)
     if (s.mode == mode && s.H == g.H && s.I == g.I && s.I_d == g.I_d && s.n_pad == n_pad && s.sms == sms) return s;
-  const Knobs& kn = knobs();
   Schedule sc = {};
   sc.mode = mode; sc.H = g.H; sc.I = g.I; sc.I_d = g.I_d; sc.n_pad = n_pad; sc.sms = sms;
-  sc.tail = make_tail(mode, g, n_pad);
   // cost of a stage.  Every CTA keeps the same number of ring slots in flight, so under HBM contention a
   // stage costs one slot latency plus its bytes: measured on B200 (profiles/) a 40 KB sparse stage takes
   // ~1.12x a 32 KB dense one => fixed part ~36 KB-equivalents; activation bytes come from L2 and weigh less.
-  const double cs = kn.fixed + kSparseStageBytes + kn.gamma * 2.0 * n_pad * 128, cd = kn.fixed + kDenseStageBytes + kn.gamma * 1.0 * n_pad * 128;
-  const int num_tiles = mode == 0 ? g.gu_tiles : g.dn_tiles;
-  const int tiles_sparse = mode == 0 ? g.gu_tiles_sparse : 0;
-  const int static_tiles = sc.tail.tile0;
+  static const double fixed = env_double("SPENSE_SCHED_FIXED", 36864.0), gamma = env_double("SPENSE_SCHED_GAMMA", 0.25);
+  const double cs = fixed + kSparseStageBytes + gamma * 2.0 * n_pad * 128, cd = fixed + kDenseStageBytes + gamma * 1.0 * n_pad * 128;
   std::vector<double> cost;
-  std::vector<uint32_t> bytes;
-  std::vector<int> tile_begin(num_tiles + 1, 0);
-  for (int t = 0; t < num_tiles; ++t) {
-    const int ns = mode == 0 ? (t < tiles_sparse ? g.gu_ns : 0) : g.dn_ns;
-    const int nd = mode == 0 ? (t < tiles_sparse ? 0 : g.gu_nd) : g.dn_nd;
-    tile_begin[t + 1] = tile_begin[t] + ns + nd;
-    if (t < static_tiles) {
-      cost.insert(cost.end(), (size_t)ns, cs); cost.insert(cost.end(), (size_t)nd, cd);
-      bytes.insert(bytes.end(), (size_t)ns, (uint32_t)kSparseStageBytes); bytes.insert(bytes.end(), (size_t)nd, (uint32_t)kDenseStageBytes);
+  if (mode == 0) {
+    cost.insert(cost.end(), (size_t)g.gu_tiles_sparse * g.gu_ns, cs);
+    cost.insert(cost.end(), (size_t)(g.gu_tiles - g.gu_tiles_sparse) * g.gu_nd, cd);
+  } else {
+    for (int t = 0; t < g.dn_tiles; ++t) {
+      cost.insert(cost.end(), (size_t)g.dn_ns, cs);
+      cost.insert(cost.end(), (size_t)g.dn_nd, cd);
     }
   }
   const int total = (int)cost.size();
   int spans = sms < kMaxSpans ? sms : kMaxSpans;
-  if (kn.max_spans > 0 && spans > kn.max_spans) spans = kn.max_spans;
   if (spans > total) spans = total;
-  // a task stages one 1 KB column slice per partial in half of the ring: at most 64 spans per tile
-  if (spans > 32 * static_tiles) spans = 32 * static_tiles;
   double sum = 0;
   for (double c : cost) sum += c;
   sc.n_spans = spans;
@@ -197,6 +115,13 @@ const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms) {
   }
   sc.span_begin[spans] = total;
   // byte offsets: the blob stores the stage images in exactly this linear order
+  std::vector<uint32_t> bytes(total);
+  if (mode == 0) {
+    for (int i = 0; i < total; ++i) bytes[i] = i < g.gu_tiles_sparse * g.gu_ns ? kSparseStageBytes : kDenseStageBytes;
+  } else {
+    const int per = g.dn_ns + g.dn_nd;
+    for (int i = 0; i < total; ++i) bytes[i] = (i % per) < g.dn_ns ? kSparseStageBytes : kDenseStageBytes;
+  }
   const int ring = ring_stages_of(n_pad);
   uint64_t off = 0;
   int st = 0;
@@ -206,21 +131,9 @@ const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms) {
     uint32_t pre = 0;
     for (int k = sc.span_begin[i]; k < sc.span_begin[i + 1] && k < sc.span_begin[i] + ring; ++k) pre += bytes[k];
     sc.span_pre[i] = pre;
-  }
-  // reduced tiles: static tiles shared by more than two spans, then the tail tiles
-  int a = 0;
-  for (int t = 0; t < static_tiles; ++t) {
-    while (a + 1 < spans && sc.span_begin[a + 1] <= tile_begin[t]) ++a;
-    int b = a;
-    while (b + 1 < spans && sc.span_begin[b + 1] < tile_begin[t + 1]) ++b;
-    if (b > a + 1 && sc.n_red < kMaxRed) sc.red[sc.n_red++] = RedEntry{t, b - a + 1, a};
-  }
-  sc.n_red_static = sc.n_red;
-  int chunk0 = 0;
-  for (int t = static_tiles; t < num_tiles; ++t) {
-    const int cpt = mode == 0 ? (t < tiles_sparse ? sc.tail.cpt_s : sc.tail.cpt_d) : sc.tail.cpt_s;
-    sc.red[sc.n_red++] = RedEntry{t, cpt, chunk0};
-    chunk0 += cpt;
+    uint32_t len = 0;
+    for (int k = sc.span_begin[i]; k < sc.span_begin[i + 1]; ++k) len += bytes[k];
+    sc.span_len[i] = len;
   }
   g_sched.push_back(sc);
   return g_sched.back();
@@ -269,6 +182,13 @@ int read_header(const void* d_blob, const spense_shape_t* shape, BlobHeader* out
   return SPENSE_OK;
 }
 
+// bytes of span k that the PREVIOUS launch pulls into L2 during its tail: at least one ring
+uint32_t next_prefetch_bytes(const Schedule& sc, int k) {
+  static const uint32_t want = (uint32_t)(env_double("SPENSE_PF_NEXT_KB", 0.0) * 1024.0);
+  uint32_t n = sc.span_pre[k] > want ? sc.span_pre[k] : want;
+  return n < sc.span_len[k] ? n : sc.span_len[k];
+}
+
 long long* g_trace = nullptr;   // debug: set by spense_debug_set_trace (not part of the public ABI)
 
 void fill_common(GemmParams& p, const Schedule& sc, int M, int n_pad, void* d_ws) {
@@ -276,22 +196,22 @@ void fill_common(GemmParams& p, const Schedule& sc, int M, int n_pad, void* d_ws
   if (g_trace) g_trace += (size_t)kMaxSpans * 16;   // debug: consecutive launches fill consecutive timelines
   p.n_spans = sc.n_spans;
   std::memcpy(p.span_begin, sc.span_begin, sizeof(int) * (sc.n_spans + 1));
-  p.tail_tile0 = sc.tail.tile0; p.tail_ts = sc.tail.ts; p.tail_cs = sc.tail.cs;
-  p.tail_cpt_s = sc.tail.cpt_s; p.tail_cpt_d = sc.tail.cpt_d; p.n_tail_chunks = sc.tail.n_chunks;
-  p.n_red = sc.n_red; p.n_red_static = sc.n_red_static;
-  p.red_slices = M < 16 ? M : 16;
-  std::memcpy(p.red, sc.red, sizeof(RedEntry) * sc.n_red);
+  static const uint32_t self_want = (uint32_t)(env_double("SPENSE_PF_SELF_KB", 0.0) * 1024.0);
+  for (int i = 0; i < sc.n_spans; ++i) {                    // own stages pulled into L2 while waiting for the previous kernel
+    const uint32_t from = next_prefetch_bytes(sc, i);
+    const uint32_t left = sc.span_len[i] - from;
+    p.self_off[i] = from - sc.span_pre[i];
+    p.self_len[i] = self_want < left ? self_want : left;
+  }
   p.M = M;
   p.n_pad = n_pad;
   p.slot_bytes = slot_bytes_of(n_pad);
   p.num_stages = ring_stages_of(n_pad);
   p.acc_stride = n_pad <= 32 ? 32 : (n_pad <= 64 ? 64 : 128);
   p.num_acc_bufs = n_pad <= 64 ? 2 : 1;
-  uint8_t* ws = reinterpret_cast<uint8_t*>(d_ws);
-  p.ws_ctrl = reinterpret_cast<int*>(ws);
-  p.flags = reinterpret_cast<int*>(ws + kFlagOff);
-  p.tile_cnt = reinterpret_cast<int*>(ws + kTileCntOff);
-  p.partials = reinterpret_cast<float*>(ws + kFlagBytes);
+  p.ws_ctrl = reinterpret_cast<int*>(d_ws);
+  p.flags = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(d_ws) + 128);
+  p.partials = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes);
 }
 
 // L2 prefetch hint: while this launch runs its fix-up tail, pull what the next launch streams first.
@@ -302,7 +222,7 @@ void fill_next(GemmParams& p, const uint8_t* next_section, const Schedule& next)
   for (int i = 0; i < p.n_spans; ++i) {
     const int k = i < next.n_spans ? i : next.n_spans - 1;
     p.next_off[i] = next.span_off[k];
-    p.next_len[i] = i < next.n_spans ? next.span_pre[k] : 0;
+    p.next_len[i] = i < next.n_spans ? next_prefetch_bytes(next, k) : 0;
   }
 }
 
@@ -386,20 +306,8 @@ extern "C" {
 
 int spense_version(void) { return 100 * 0 + 1; }
 
-// debug hook (undeclared in spense.h): per-CTA clock64 timeline, 16 int64 per span, of the next launches
+// debug hook (undeclared in spense.h): per-CTA globaltimer timeline, 16 int64 per span, of the next launches
 void spense_debug_set_trace(void* d_buf) { g_trace = reinterpret_cast<long long*>(d_buf); }
-
-// debug hook (undeclared in spense.h): override the schedule knobs (negative / zero = keep the default) so that
-// small test shapes exercise the dynamic tail and the multi-way reductions; clears the schedule cache
-void spense_debug_set_schedule(double tail_frac, int tail_cs, int max_spans, int min_static) {
-  std::lock_guard<std::mutex> lk(g_sched_mu);
-  knobs();
-  g_knobs.tail_frac = tail_frac >= 0 ? tail_frac : 0.15;
-  g_knobs.tail_cs = tail_cs > 0 ? tail_cs : 0;
-  g_knobs.max_spans = max_spans > 0 ? max_spans : 0;
-  g_knobs.min_static = min_static >= 0 ? min_static : 2 * kMaxSpans;
-  g_sched.clear();
-}
 
 const char* spense_strerror(int status) {
   switch (status) {
@@ -464,13 +372,7 @@ int spense_workspace_size(const spense_shape_t* shape, int32_t M, size_t* bytes)
   int st = check_shape(shape);
   if (st) return st;
   if (M < 1 || !bytes) return SPENSE_ERR_ARG;
-  const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  size_t need = 0;
-  for (int n_pad = 16; n_pad <= n_pad_of(M); n_pad += 16) {   // the workspace serves every launch of up to M tokens
-    const size_t b = ws_bytes_for(g, n_pad);
-    if (b > need) need = b;
-  }
-  *bytes = need;
+  *bytes = ws_bytes_for(n_pad_of(M), kMaxSpans);
   return SPENSE_OK;
 }
 

@@ -37,6 +37,55 @@ namespace spense {
 
 namespace {
 
+// Position in the linear stage sequence: pair tile, stage inside the tile, stages of the tile.
+struct Cursor {
+  int tile, j, ns, nd, first;   // first = linear index of the tile's first stage
+};
+
+// The only place with integer divisions (one copy, called once per role).
+template <int MODE>
+__device__ __noinline__ Cursor cursor_at(const GemmParams& p, int s, unsigned long long* byte_off) {
+  Cursor c;
+  size_t off;
+  if (MODE == 0) {
+    const int sparse_total = p.tiles_sparse * p.ns;
+    if (s < sparse_total) {
+      c.tile = s / p.ns;
+      c.first = c.tile * p.ns;
+      c.ns = p.ns; c.nd = 0;
+      off = (size_t)s * kSparseStageBytes;
+    } else {
+      const int td = (s - sparse_total) / p.nd;
+      c.tile = p.tiles_sparse + td;
+      c.first = sparse_total + td * p.nd;
+      c.ns = 0; c.nd = p.nd;
+      off = (size_t)sparse_total * kSparseStageBytes + (size_t)(s - sparse_total) * kDenseStageBytes;
+    }
+    c.j = s - c.first;
+  } else {
+    const int per = p.ns + p.nd;
+    c.tile = s / per;
+    c.first = c.tile * per;
+    c.ns = p.ns; c.nd = p.nd;
+    c.j = s - c.first;
+    off = (size_t)c.tile * ((size_t)p.ns * kSparseStageBytes + (size_t)p.nd * kDenseStageBytes);
+    off += c.j < c.ns ? (size_t)c.j * kSparseStageBytes
+                      : (size_t)c.ns * kSparseStageBytes + (size_t)(c.j - c.ns) * kDenseStageBytes;
+  }
+  *byte_off = off;
+  return c;
+}
+
+template <int MODE>
+__device__ __forceinline__ void next_tile(const GemmParams& p, Cursor& c) {
+  c.first += c.ns + c.nd;
+  ++c.tile;
+  c.j = 0;
+  if (MODE == 0) {
+    if (c.tile < p.tiles_sparse) { c.ns = p.ns; c.nd = 0; } else { c.ns = 0; c.nd = p.nd; }
+  }
+}
+
 // SiLU(g) * u on the hardware exp2 / reciprocal units: branch-free, relative error ~1e-6 (far inside
 // the GLU tolerance).  ex2 of a very negative g overflows to +inf -> rcp gives 0 -> h = -0 * u.
 __device__ __forceinline__ float silu_mul(float g, float u) {
@@ -116,78 +165,8 @@ __device__ __forceinline__ void finish(const GemmParams& p, const float4* sc, in
   }
 }
 
-
-// A segment = consecutive stages of ONE pair tile accumulated into one TMEM buffer.  The producer is the only
-// role that walks the schedule (static span, then dynamically claimed tail chunks); it describes every
-// segment in a small shared-memory FIFO that the MMA issuer and the epilogue warps follow.
-enum { kFixWhole = 0, kFixOwnerAdd = 1, kFixDumpFlag = 2, kFixDumpCount = 3, kFixStop = 4 };
-struct Seg {
-  int seq;        // entry index + 1, written last (release): the entry is valid once it matches
-  int tile;
-  int j0, n;      // first stage inside the tile, number of stages
-  int ns_tile;    // stages [0, ns_tile) of this tile are 2:4 sparse
-  int fix;        // kFix*
-  int a;          // OwnerAdd / DumpFlag: flag index; DumpCount: reduced-tile index
-  int b;          // partial slot (OwnerAdd: the partner's, Dump*: ours)
-};
-constexpr int kSegFifo = 16;   // the producer is at most ring + 1 + 2 accumulators (<= 11 segments) ahead of the epilogue
-static_assert(256 + kSegFifo * 32 + 64 == kSmemTailBytes, "shared-memory tail layout");
-
-__device__ __forceinline__ int ld_acquire_cta_shared(const int* p) {
-  int v;
-  asm volatile("ld.acquire.cta.shared::cta.s32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p)) : "memory");
-  return v;
-}
-__device__ __forceinline__ void st_release_cta_shared(int* p, int v) {
-  asm volatile("st.release.cta.shared::cta.s32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
-}
-__device__ __forceinline__ Seg wait_seg(const Seg* fifo, int idx) {
-  const Seg* e = fifo + (idx & (kSegFifo - 1));
-  while (ld_acquire_cta_shared(&e->seq) != idx + 1) {}
-  return *e;
-}
-
-// stages of pair tile t, and the byte offset of its stage j inside the section
-template <int MODE>
-__device__ __forceinline__ void tile_shape(const GemmParams& p, int t, int& ns, int& nd) {
-  if (MODE == 0) {
-    if (t < p.tiles_sparse) { ns = p.ns; nd = 0; } else { ns = 0; nd = p.nd; }
-  } else {
-    ns = p.ns; nd = p.nd;
-  }
-}
-template <int MODE>
-__device__ __forceinline__ size_t stage_offset(const GemmParams& p, int t, int j) {
-  if (MODE == 0) {
-    if (t < p.tiles_sparse) return ((size_t)t * p.ns + j) * kSparseStageBytes;
-    return (size_t)p.tiles_sparse * p.ns * kSparseStageBytes + ((size_t)(t - p.tiles_sparse) * p.nd + j) * kDenseStageBytes;
-  }
-  const size_t base = (size_t)t * ((size_t)p.ns * kSparseStageBytes + (size_t)p.nd * kDenseStageBytes);
-  return base + (j < p.ns ? (size_t)j * kSparseStageBytes
-                          : (size_t)p.ns * kSparseStageBytes + (size_t)(j - p.ns) * kDenseStageBytes);
-}
-// linear stage index of the first stage of tile t (the order of span_begin)
-template <int MODE>
-__device__ __forceinline__ int tile_first(const GemmParams& p, int t) {
-  if (MODE == 0) return t < p.tiles_sparse ? t * p.ns : p.tiles_sparse * p.ns + (t - p.tiles_sparse) * p.nd;
-  return t * (p.ns + p.nd);
-}
-// tail chunk q -> (tile, j0, n)
-template <int MODE>
-__device__ __forceinline__ void tail_chunk(const GemmParams& p, int q, int& tile, int& j0, int& n) {
-  int cpt, per, t_off = 0;
-  if (MODE == 0) {
-    const int qs = p.tail_ts * p.tail_cpt_s;
-    if (q < qs) { cpt = p.tail_cpt_s; per = p.ns; }
-    else { q -= qs; cpt = p.tail_cpt_d; per = p.nd; t_off = p.tail_ts; }
-  } else {
-    cpt = p.tail_cpt_s; per = p.ns + p.nd;
-  }
-  const int tt = q / cpt;
-  tile = p.tail_tile0 + t_off + tt;
-  j0 = (q - tt * cpt) * p.tail_cs;
-  n = min(p.tail_cs, per - j0);
-}
+// A tile shared by more than two spans [a, b]: reduced at the end of the span (reduce-scatter).
+struct Group { int a, b, tile, first; };
 
 }  // namespace
 
@@ -200,31 +179,26 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
   const int lane = threadIdx.x & 31;
 
   const int S = p.num_stages;
-  // after the stage ring: 256 B of barriers | one float4 of scales per token column | segment FIFO | misc
+  // barriers live after the stage ring
   const uint32_t ring_bytes = (uint32_t)S * p.slot_bytes;
   const uint32_t bar_base = smem_base + ring_bytes;
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
   auto empty_bar = [&](int s) { return bar_base + 8u * (8 + s); };
   auto accf_bar = [&](int b) { return bar_base + 8u * (16 + b); };
   auto acce_bar = [&](int b) { return bar_base + 8u * (18 + b); };
-  const uint32_t red_bar = bar_base + 8u * 22;   // two barriers: task-reduction double buffer
+  const uint32_t red_bar = bar_base + 8u * 22;
   const uint32_t tmem_slot = bar_base + 8u * 20;
   uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
   volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(smem_gen + ring_bytes + 8 * 20);
   volatile int* epoch_ptr = reinterpret_cast<volatile int*>(smem_gen + ring_bytes + 8 * 21);
-  float4* sc = reinterpret_cast<float4*>(smem_gen + ring_bytes + 256);
-  Seg* fifo = reinterpret_cast<Seg*>(smem_gen + ring_bytes + 256 + 16 * p.n_pad);
-  volatile int* task_ptr = reinterpret_cast<volatile int*>(fifo + kSegFifo);   // 2 ints: task broadcast (double buffered)
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmap_b);
     for (int s = 0; s < S; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(accf_bar(b), 1); mbar_init(acce_bar(b), kEpiThreads); }
     mbar_init(red_bar, 1);
-    mbar_init(red_bar + 8, 1);
     fence_barrier_init();
   }
-  if (warp == 3 && lane < kSegFifo) fifo[lane].seq = 0;
   if (warp == 2) tmem_alloc(tmem_slot, kTmemCols);
   tc_fence_before();
   __syncthreads();
@@ -241,7 +215,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
   if (p.trace && threadIdx.x == 0) {
     uint32_t smid;
     asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-    p.trace[(size_t)span * 16 + 0] = globaltimer(); p.trace[(size_t)span * 16 + 14] = smid;
+    p.trace[(size_t)span * 16 + 0] = globaltimer(); p.trace[(size_t)span * 16 + 12] = globaltimer(); p.trace[(size_t)span * 16 + 14] = smid;
   }
 
   if (warp == 0) {
@@ -249,129 +223,73 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
     if (lane == 0) {
       const uint64_t pol_w = policy_evict_first();
       const uint64_t pol_a = policy_evict_last();
-      int it = 0, seg_idx = 0, n_issued_static = 0;
-      bool pdl_done = false;
+      unsigned long long off;
+      Cursor c = cursor_at<MODE>(p, sb, &off);
+      const uint8_t* src = p.section + off;
+      const int n = se - sb;
+      const int pre = n < S ? n : S;
       uint32_t info[8];                                    // stages issued before pdl_wait: K coordinate | sparse << 31
-      auto load_b = [&](int slot, uint32_t inf) {
-        const uint32_t b_dst = smem_base + (uint32_t)slot * p.slot_bytes + kSparseStageBytes;
+      auto load_b = [&](int it, uint32_t inf) {
+        const uint32_t b_dst = smem_base + (uint32_t)(it % S) * p.slot_bytes + kSparseStageBytes;
         const int k0 = (int)(inf & 0x7FFFFFFFu);
-        tma_load_2d(b_dst, &tmap_b, k0, 0, full_bar(slot), pol_a);
-        if (inf >> 31) tma_load_2d(b_dst + b_tile_bytes, &tmap_b, k0 + 128, 0, full_bar(slot), pol_a);
+        tma_load_2d(b_dst, &tmap_b, k0, 0, full_bar(it % S), pol_a);
+        if (inf >> 31) tma_load_2d(b_dst + b_tile_bytes, &tmap_b, k0 + 128, 0, full_bar(it % S), pol_a);
       };
       // Weights never depend on the previous kernel of the stream, activations do: fill the whole ring with
       // weight stages, then wait for the previous kernel and add the activation tiles.
+      auto prefetch_l2 = [&](const uint8_t* base, uint32_t bytes) {
+#pragma unroll 1
+        for (uint32_t o = 0; o < bytes; o += 32768u) {
+          const uint32_t chunk = bytes - o < 32768u ? bytes - o : 32768u;
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(base + o), "r"(chunk) : "memory");
+        }
+      };
       auto flush = [&]() {
         trace(p, span, 1);
+        if (p.self_len[span]) prefetch_l2(src + p.self_off[span], p.self_len[span]);
         pdl_wait();
-        pdl_done = true;
 #pragma unroll
         for (int k = 0; k < 8; ++k)
-          if (k < it) load_b(k, info[k]);
+          if (k < pre) load_b(k, info[k]);
       };
-      auto push_seg = [&](int tile, int j0, int n, int ns_tile, int fix, int a, int b) {
-        Seg* e = fifo + (seg_idx & (kSegFifo - 1));
-        e->tile = tile; e->j0 = j0; e->n = n; e->ns_tile = ns_tile; e->fix = fix; e->a = a; e->b = b;
-        st_release_cta_shared(&e->seq, ++seg_idx);
-      };
-      auto issue = [&](int tile, int j, int ns_tile) {
-        if (!pdl_done && it == S) flush();
-        const bool sp = j < ns_tile;
+#pragma unroll 1
+      for (int it = 0; it < n; ++it) {
+        if (it == pre) flush();
+        const bool sp = c.j < c.ns;
         const uint32_t wb = sp ? (uint32_t)kSparseStageBytes : (uint32_t)kDenseStageBytes;
-        const uint32_t inf = (uint32_t)(sp ? j * kSparseStageK : p.dense_k0 + (j - ns_tile) * kDenseStageK) | (sp ? 0x80000000u : 0u);
+        const uint32_t inf = (uint32_t)(sp ? c.j * kSparseStageK : p.dense_k0 + (c.j - c.ns) * kDenseStageK) | (sp ? 0x80000000u : 0u);
         const int slot = it % S;
-        if (it >= S) mbar_wait(empty_bar(slot), ((uint32_t)(it / S) & 1u) ^ 1u);
+        if (it >= pre) mbar_wait(empty_bar(slot), ((uint32_t)(it / S) & 1u) ^ 1u);
         mbar_expect_tx(full_bar(slot), wb + (sp ? 2u : 1u) * b_tile_bytes);
-        bulk_g2s(smem_base + (uint32_t)slot * p.slot_bytes, p.section + stage_offset<MODE>(p, tile, j), wb, full_bar(slot), pol_w);
-        if (pdl_done) {
-          load_b(slot, inf);
+        bulk_g2s(smem_base + (uint32_t)slot * p.slot_bytes, src, wb, full_bar(slot), pol_w);
+        if (it >= pre) {
+          load_b(it, inf);
         } else {
 #pragma unroll
           for (int k = 0; k < 8; ++k)
             if (k == it) info[k] = inf;
         }
-        ++it;
-      };
-
-      // ---- static span: segments per tile
-      int tile;
-      if (MODE == 0) {
-        const int sparse_total = p.tiles_sparse * p.ns;
-        tile = sb < sparse_total ? sb / p.ns : p.tiles_sparse + (sb - sparse_total) / p.nd;
-      } else {
-        tile = sb / (p.ns + p.nd);
+        src += wb;
+        if (++c.j == c.ns + c.nd) next_tile<MODE>(p, c);
       }
-      int first = tile_first<MODE>(p, tile);
-      const int claim_at = max(sb, se - 2);
-      int q_next = p.n_tail_chunks;                        // claimed tail chunk (claimed a little ahead of need)
-#pragma unroll 1
-      for (int s = sb; s < se;) {
-        int ns, nd;
-        tile_shape<MODE>(p, tile, ns, nd);
-        const int tile_end = first + ns + nd;
-        const int seg_end = min(se, tile_end);
-        int a = span, b = span;
-        while (p.span_begin[a] > first) --a;
-        while (b + 1 < p.n_spans && p.span_begin[b + 1] < tile_end) ++b;
-        int fix = kFixWhole, fa = 0, fb = 0;
-        if (b == a + 1) {
-          fix = span == a ? kFixOwnerAdd : kFixDumpFlag;   // span b starts inside the tile: its first segment
-          fa = b * 2; fb = b * 2;
-        } else if (b > a + 1) {
-          fix = kFixDumpCount;
-          for (int r = 0; r < p.n_red_static; ++r)
-            if (p.red[r].tile == tile) fa = r;
-          fb = span * 2 + (sb >= first ? 0 : 1);
-        }
-        push_seg(tile, s - first, seg_end - s, ns, fix, fa, fb);
-#pragma unroll 1
-        for (; s < seg_end; ++s) {
-          if (s == claim_at && p.n_tail_chunks > 0) {
-            if (!pdl_done) flush();                        // the queue counter belongs to the previous kernel until then
-            q_next = atomicAdd(p.ws_ctrl + kCtrlChunk, 1);
-          }
-          issue(tile, s - first, ns);
-        }
-        ++tile;
-        first = tile_end;
-      }
-      n_issued_static = it;
-      if (!pdl_done) flush();
+      if (n <= pre) flush();
       trace(p, span, 2);
-      // ---- dynamic tail: claim chunks until the queue is empty
-#pragma unroll 1
-      for (int q = q_next; q < p.n_tail_chunks; q = q_next) {
-        q_next = atomicAdd(p.ws_ctrl + kCtrlChunk, 1);
-        int t, j0, n, ns, nd;
-        tail_chunk<MODE>(p, q, t, j0, n);
-        tile_shape<MODE>(p, t, ns, nd);
-        push_seg(t, j0, n, ns, kFixDumpCount, p.n_red_static + (t - p.tail_tile0), 2 * p.n_spans + q);
-#pragma unroll 1
-        for (int j = j0; j < j0 + n; ++j) issue(t, j, ns);
-      }
-      push_seg(0, 0, 0, 0, kFixStop, 0, 0);
-      if (p.trace) { p.trace[(size_t)span * 16 + 12] = globaltimer(); p.trace[(size_t)span * 16 + 11] = n_issued_static | ((it - n_issued_static) << 16); }
       // HBM goes idle while the CTAs run their fix-up tails: use that time to pull the first stages of
       // the NEXT kernel's span into L2 (the next GEMM of this layer / the next layer's gate_up).
-      if (p.next_base) {
-        const uint8_t* nb = p.next_base + (size_t)p.next_off[span];
-        const uint32_t bytes = p.next_len[span];
-#pragma unroll 1
-        for (uint32_t o = 0; o < bytes; o += 32768u) {
-          const uint32_t chunk = bytes - o < 32768u ? bytes - o : 32768u;
-          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(nb + o), "r"(chunk) : "memory");
-        }
-      }
+      if (p.next_base) prefetch_l2(p.next_base + (size_t)p.next_off[span], p.next_len[span]);
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     if (lane == 0) {
       const uint32_t idesc_d = (1u << 4) | ((uint32_t)(p.n_pad >> 3) << 17) | ((128u >> 4) << 24);
       const uint32_t idesc_s = idesc_d | (1u << 2);
-      int it = 0;
+      unsigned long long off;
+      Cursor c = cursor_at<MODE>(p, sb, &off);
+      int it = 0, seg = 0;
 #pragma unroll 1
-      for (int seg = 0;; ++seg) {
-        const Seg e = wait_seg(fifo, seg);
-        if (e.fix == kFixStop) break;
+      for (int s = sb; s < se; ++seg) {
+        const int tile_end = c.first + c.ns + c.nd;
+        const int seg_end = min(se, tile_end);
         const int buf = seg % p.num_acc_bufs;
         const uint32_t use = (uint32_t)(seg / p.num_acc_bufs);
         mbar_wait(acce_bar(buf), (use & 1u) ^ 1u);         // epilogue has drained this accumulator
@@ -380,7 +298,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
         const uint32_t d1 = d0 + (uint32_t)p.acc_stride;
         uint32_t acc = 0;
 #pragma unroll 1
-        for (int j = e.j0; j < e.j0 + e.n; ++j, ++it) {
+        for (; s < seg_end; ++s, ++it, ++c.j) {
           const int slot = it % S;
           const uint32_t ph = (uint32_t)(it / S) & 1u;
           mbar_wait(full_bar(slot), ph);
@@ -389,7 +307,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
           const uint32_t a0 = smem_base + (uint32_t)slot * p.slot_bytes;
           const uint32_t a1 = a0 + kOperandBytes;
           const uint32_t b0 = a0 + kSparseStageBytes;
-          if (j < e.ns_tile) {
+          if (c.j < c.ns) {
             const uint32_t e_base = tmem_base + kMetaCol + (uint32_t)(it & 1) * 16u;
             const uint32_t m0 = a0 + 2 * kOperandBytes;   // A0 meta: 2 atoms of 2 KB, then A1 meta
 #pragma unroll
@@ -414,12 +332,12 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
           tc_commit(empty_bar(slot));                     // smem slot free once these MMAs have read it
         }
         tc_commit(accf_bar(buf));                         // accumulator complete for this segment
+        if (s == tile_end) next_tile<MODE>(p, c);
       }
       trace(p, span, 4);
     }
-  }
-  else if (warp >= 4) {
-    // ===================== epilogue (16 warps) =====================
+  } else if (warp >= 4) {
+    // ===================== epilogue (8 warps) =====================
     // warp & 3 selects the TMEM lane quadrant, (warp - 4) >> 2 the quarter of the token columns.
     const int q = warp & 3;
     const int row = q * 32 + lane;                         // accumulator lane = weight row inside the tile
@@ -428,6 +346,8 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
     const int cols_per = (((p.n_pad + 3) >> 2) + 7) & ~7;  // columns per warp: a quarter, rounded to the TMEM load width
     const int c_begin = ((warp - 4) >> 2) * cols_per;
     const int c_end = min(c_begin + cols_per, cols_used);
+    float4* sc = reinterpret_cast<float4*>(smem_gen + ring_bytes + 256);   // one float4 of scales per token column
+    const float* stg = reinterpret_cast<const float*>(smem_gen);         // the stage ring doubles as partial staging
     const size_t part_floats = (size_t)2 * p.n_pad * 128;  // one partial: [mat][col][row]
 
     // scales, the workspace and the epoch word may be produced / still in use by the previous kernel
@@ -447,46 +367,59 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
     if (et == kEpiThreads - 1) {
       // Epoch of this launch = epoch word + 1.  Every CTA reads the word BEFORE it counts itself; the CTA
       // that counts last therefore knows all have read it and advances it for the next launch.
-      const int e = ld_acquire(p.ws_ctrl + kCtrlEpoch);
+      const int e = ld_acquire(p.ws_ctrl);
       *epoch_ptr = e + 1;
-      if (atomicAdd(p.ws_ctrl + kCtrlStarted, 1) == p.n_spans - 1) {
-        p.ws_ctrl[kCtrlStarted] = 0;
-        st_release(p.ws_ctrl + kCtrlEpoch, e + 1);
+      if (atomicAdd(p.ws_ctrl + 1, 1) == p.n_spans - 1) {
+        p.ws_ctrl[1] = 0;
+        st_release(p.ws_ctrl, e + 1);
       }
     }
     epi_sync();
     const int epoch = *epoch_ptr;                          // flag value of THIS launch (never equals a stale flag)
 
+    Group groups[2];
+    int n_groups = 0;
+    uint32_t red_round = 0;                                // uses of the staging barrier so far
+    unsigned long long off;
+    Cursor cur = cursor_at<MODE>(p, sb, &off);
+    int seg = 0;
 #pragma unroll 1
-    for (int seg = 0;; ++seg) {
-      const Seg e = wait_seg(fifo, seg);
-      if (e.fix == kFixStop) break;
+    for (int s = sb; s < se; ++seg) {
+      const int tile_end = cur.first + cur.ns + cur.nd;
+      const int seg_end = min(se, tile_end);
       const int buf = seg % p.num_acc_bufs;
       const uint32_t use = (uint32_t)(seg / p.num_acc_bufs);
+      // spans [a, b] that hold stages of this tile
+      int a = span, b = span;
+      while (p.span_begin[a] > cur.first) --a;
+      while (b + 1 < p.n_spans && p.span_begin[b + 1] < tile_end) ++b;
+
       mbar_wait(accf_bar(buf), use & 1u);
       tc_fence_after();
       if (et == 0) trace(p, span, seg == 0 ? 5 : 7);
       const uint32_t t0 = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * 2 * p.acc_stride);
       const uint32_t t1 = t0 + (uint32_t)p.acc_stride;
 
-      if (e.fix == kFixWhole || e.fix == kFixOwnerAdd) {
+      if (a == b || (b == a + 1 && span == a)) {
         // the whole tile is ours, or we own a tile whose tail the next span has (usually long ago) dumped
-        const bool add = e.fix == kFixOwnerAdd;
-        const float* part = p.partials + (size_t)e.b * part_floats;
+        const bool add = a != b;
         if (add) {
-          while (ld_acquire(p.flags + e.a) != epoch) {}   // warp-uniform address: one request per warp
+          // Owner of a split tile = last segment of the span: every MMA of this CTA is complete, the ring is free.
+          if (et == 0) {
+            const int* f = p.flags + b * 2;                // span b starts inside the tile: its first segment
+            while (ld_acquire(f) != epoch) {}
+            asm volatile("fence.proxy.async.global;" ::: "memory");   // partner's generic-proxy stores -> our async-proxy read
+            const float* part = p.partials + (size_t)b * 2 * part_floats;
+            mbar_expect_tx(red_bar, 2u * (uint32_t)cols_used * 512u);
+            bulk_g2s(smem_base, part, (uint32_t)cols_used * 512u, red_bar, policy_evict_first());
+            bulk_g2s(smem_base + (uint32_t)cols_used * 512u, part + (size_t)p.n_pad * 128, (uint32_t)cols_used * 512u, red_bar, policy_evict_first());
+          }
+          mbar_wait(red_bar, red_round & 1u);
+          ++red_round;
           if (et == 0) trace(p, span, 8);
         }
 #pragma unroll 1
         for (int c = c_begin; c < c_end; c += 8) {
-          float a0[8], a1[8];
-          if (add) {
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-              a0[i] = __ldcg(part + (size_t)(c + i) * 128 + row);
-              a1[i] = __ldcg(part + (size_t)(p.n_pad + c + i) * 128 + row);
-            }
-          }
           uint32_t v0[8], v1[8];
           tmem_ld8(t0 + c, v0);
           tmem_ld8(t1 + c, v1);
@@ -496,17 +429,21 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
           for (int i = 0; i < 8; ++i) { f0[i] = __uint_as_float(v0[i]); f1[i] = __uint_as_float(v1[i]); }
           if (add) {
 #pragma unroll
-            for (int i = 0; i < 8; ++i) { f0[i] += a0[i]; f1[i] += a1[i]; }
+            for (int i = 0; i < 8; ++i) {
+              f0[i] += stg[(size_t)(c + i) * 128 + row];
+              f1[i] += stg[(size_t)(cols_used + c + i) * 128 + row];
+            }
           }
 #pragma unroll
           for (int i = 0; i < 8; ++i)
-            if (c + i < p.M) finish<MODE>(p, sc, e.tile, row, c + i, f0[i], f1[i]);
+            if (c + i < p.M) finish<MODE>(p, sc, cur.tile, row, c + i, f0[i], f1[i]);
         }
         tc_fence_before();
         mbar_arrive(acce_bar(buf));
       } else {
-        // part of a split tile that others finish: dump the raw fp32 partial [mat][col][row] and publish it
-        float* slot = p.partials + (size_t)e.b * part_floats;
+        // split tile, not (solely) ours to finish: dump the raw fp32 partial [mat][col][row] and publish it
+        const int which = (sb >= cur.first) ? 0 : 1;       // our first segment, or our last one
+        float* slot = p.partials + ((size_t)span * 2 + which) * part_floats;
 #pragma unroll 1
         for (int c = c_begin; c < c_end; c += 8) {
           uint32_t v0[8], v1[8];
@@ -522,91 +459,66 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
         tc_fence_before();
         mbar_arrive(acce_bar(buf));
         epi_sync();                                        // all partial stores issued (CTA scope) ...
-        if (et == 0) {                                     // ... one gpu-scope release publishes them (cumulativity)
-          if (e.fix == kFixDumpFlag) st_release(p.flags + e.a, epoch);
-          else asm volatile("red.release.gpu.global.add.s32 [%0], 1;" ::"l"(p.tile_cnt + e.a) : "memory");
+        if (et == 0) st_release(p.flags + span * 2 + which, epoch);   // ... one gpu-scope release publishes them (cumulativity)
+        if (b > a + 1) {
+          groups[n_groups].a = a; groups[n_groups].b = b; groups[n_groups].tile = cur.tile; groups[n_groups].first = cur.first;
+          ++n_groups;
         }
       }
       if (et == 0) trace(p, span, 6);
+      s = seg_end;
+      if (s == tile_end) next_tile<MODE>(p, cur);
     }
 
-    // ---- task queue: tiles split into more than two partials (groups of static spans, tail tiles).  A task
-    // = (reduced tile, slice of its token columns): wait until all partials of the tile have arrived, add them
-    // in partial order (deterministic) and run the epilogue.  Tasks are claimed dynamically; every MMA of this
-    // CTA is complete here, so the stage ring is free: its two halves double-buffer the partial slices.
-    if (et == 0) trace(p, span, 9);
-    const int n_tasks = p.n_red * p.red_slices;
-    if (n_tasks > 0) {
-      const uint32_t half_bytes = (ring_bytes >> 1) & ~1023u;
-      int k = 0;                                           // staged chunks so far (buffer = k & 1)
+    // ---- deferred reduce-scatter of tiles shared by > 2 spans: span j of the group reduces token columns
+    // [j*M/n, (j+1)*M/n), adding the n partials in span order, and runs the epilogue on them.
+    // All MMAs of this CTA are complete here, so the stage ring is free to stage the partial slices.
 #pragma unroll 1
-      for (int ti = 0;; ++ti) {
-        if (et == 0) task_ptr[ti & 1] = atomicAdd(p.ws_ctrl + kCtrlTask, 1);
-        epi_sync();
-        const int task = task_ptr[ti & 1];
-        if (task >= n_tasks) break;
-        const int r = task / p.red_slices, sl = task - r * p.red_slices;
-        const RedEntry re = p.red[r];
-        const int n = re.n_seg;
-        const int m0 = (int)(((long long)sl * p.M) / p.red_slices), m1 = (int)(((long long)(sl + 1) * p.M) / p.red_slices);
-        if (m0 == m1) continue;
-        const bool is_tail = r >= p.n_red_static;
-        const int first = tile_first<MODE>(p, re.tile);
-        while (ld_acquire(p.tile_cnt + r) < n) {}          // warp-uniform address
-        asm volatile("fence.proxy.async.global;" ::: "memory");   // others' generic-proxy stores -> our async-proxy reads
-        int ccm = (int)(half_bytes / ((uint32_t)n * 1024u));
-        ccm = ccm < 1 ? 1 : ccm;
+    for (int gi = 0; gi < n_groups; ++gi) {
+      const Group g = groups[gi];
+      const int n = g.b - g.a + 1;
+      const int j = span - g.a;
+      const int m0 = (int)(((long long)j * p.M) / n), m1 = (int)(((long long)(j + 1) * p.M) / n);
+      if (m1 > m0) {
+        int cc_max = (int)(ring_bytes / ((uint32_t)n * 1024u));
+        if (cc_max > m1 - m0) cc_max = m1 - m0;
 #pragma unroll 1
-        for (int mc = m0; mc < m1; mc += ccm, ++k) {
-          const int cc = min(ccm, m1 - mc);
-          const uint32_t bar = red_bar + 8u * (uint32_t)(k & 1);
-          const uint32_t dst = smem_base + (uint32_t)(k & 1) * half_bytes;
-          if (et == 0) mbar_expect_tx(bar, (uint32_t)n * 2u * (uint32_t)cc * 512u);
+        for (int mc = m0; mc < m1; mc += cc_max) {
+          const int cc = min(cc_max, m1 - mc);
+          if (red_round > 0) {                             // staging smem is reused: order our reads before the async writes
+            fence_proxy_async();
+            epi_sync();
+          }
+          if (et == 0) mbar_expect_tx(red_bar, (uint32_t)n * 2u * (uint32_t)cc * 512u);
+          // thread i fetches matrix (i & 1) of partner (i >> 1) as soon as THAT partner has published
 #pragma unroll 1
           for (int i = et; i < 2 * n; i += kEpiThreads) {
-            const int qi = i >> 1, mat = i & 1;
-            int slot_idx;
-            if (is_tail) {
-              slot_idx = 2 * p.n_spans + re.first + qi;
-            } else {
-              const int qs = re.first + qi;
-              slot_idx = qs * 2 + (p.span_begin[qs] >= first ? 0 : 1);
-            }
-            const float* src = p.partials + (size_t)slot_idx * part_floats + ((size_t)mat * p.n_pad + mc) * 128;
-            bulk_g2s(dst + (uint32_t)(i * cc) * 512u, src, (uint32_t)cc * 512u, bar, policy_evict_first());
+            const int qs = g.a + (i >> 1), mat = i & 1;
+            const int which = (p.span_begin[qs] >= g.first) ? 0 : 1;
+            while (ld_acquire(p.flags + qs * 2 + which) != epoch) {}
+            asm volatile("fence.proxy.async.global;" ::: "memory");   // partner's generic-proxy stores -> our async-proxy read
+            const float* src = p.partials + ((size_t)qs * 2 + which) * part_floats + ((size_t)mat * p.n_pad + mc) * 128;
+            bulk_g2s(smem_base + (uint32_t)(i * cc) * 512u, src, (uint32_t)cc * 512u, red_bar, policy_evict_first());
           }
-          mbar_wait(bar, (uint32_t)(k >> 1) & 1u);
+          mbar_wait(red_bar, red_round & 1u);
+          ++red_round;
           if (et == 0) trace(p, span, 15);
-          const float* sl_f = reinterpret_cast<const float*>(smem_gen + (size_t)(k & 1) * half_bytes);
           const int rrow = et & 127;
 #pragma unroll 1
           for (int c = et >> 7; c < cc; c += kEpiThreads >> 7) {
             float f0 = 0.0f, f1 = 0.0f;
 #pragma unroll 4
-            for (int qi = 0; qi < n; ++qi) {               // fixed partial order: deterministic
-              f0 += sl_f[((size_t)(2 * qi) * cc + c) * 128 + rrow];
-              f1 += sl_f[((size_t)(2 * qi + 1) * cc + c) * 128 + rrow];
+            for (int qi = 0; qi < n; ++qi) {               // fixed span order: deterministic
+              f0 += stg[((size_t)(2 * qi) * cc + c) * 128 + rrow];
+              f1 += stg[((size_t)(2 * qi + 1) * cc + c) * 128 + rrow];
             }
-            finish<MODE>(p, sc, re.tile, rrow, mc + c, f0, f1);
+            finish<MODE>(p, sc, g.tile, rrow, mc + c, f0, f1);
           }
-          // the buffer used now is overwritten two chunks later: order these reads before those async writes
-          fence_proxy_async();
-          epi_sync();
         }
       }
+      if (et == 0) trace(p, span, 9);
     }
-    // ---- the CTA that finishes last resets the queue counters for the next launch
-    if (et == 0) {
-      __threadfence();
-      if (atomicAdd(p.ws_ctrl + kCtrlDone, 1) == p.n_spans - 1) {
-        p.ws_ctrl[kCtrlChunk] = 0;
-        p.ws_ctrl[kCtrlTask] = 0;
-        for (int r = 0; r < p.n_red; ++r) p.tile_cnt[r] = 0;
-        __threadfence();
-        p.ws_ctrl[kCtrlDone] = 0;
-      }
-      if (p.trace) { p.trace[(size_t)span * 16 + 10] = globaltimer(); }
-    }
+    if (p.trace && et == 0) { p.trace[(size_t)span * 16 + 10] = globaltimer(); p.trace[(size_t)span * 16 + 11] = (se - sb) | (seg << 16); p.trace[(size_t)span * 16 + 13] = globaltimer(); }
   }
 
   tc_fence_before();
@@ -615,7 +527,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
 }
 
 int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, bool pdl, cudaStream_t stream) {
-  const size_t smem = (size_t)p.num_stages * p.slot_bytes + 1024 + kSmemTailBytes + 16 * (size_t)p.n_pad;
+  const size_t smem = (size_t)p.num_stages * p.slot_bytes + 1024 + 256 + 4 * 4 * (size_t)p.n_pad;
   static bool attr_set = false;
   if (!attr_set) {
     if (cudaFuncSetAttribute(spense_gemm_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 232448) != cudaSuccess ||

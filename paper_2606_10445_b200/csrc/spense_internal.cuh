@@ -36,13 +36,7 @@ constexpr int kBlobHeaderBytes = 1024;
 constexpr uint32_t kBlobMagic = 0x53504E53u;  // "SNPS"
 constexpr int kBlobVersion = 1;
 constexpr int kMaxSpans = 160;
-constexpr int kMaxRed = 224;                 // tiles reduced through the task queue (static multi-way + tail tiles)
-constexpr int kFlagBytes = 4096;             // control words | pair flags (2 per span) | tile counters
-constexpr int kCtrlEpoch = 0, kCtrlStarted = 1, kCtrlChunk = 2, kCtrlTask = 3, kCtrlDone = 4;   // int index in the workspace
-constexpr int kFlagOff = 128;                // byte offset of the pair flags
-constexpr int kTileCntOff = 2048;            // byte offset of the per-reduced-tile arrival counters
-constexpr int kSmemTailBytes = 832;          // after the stage ring: 256 B barriers, 16 x 32 B segment FIFO, 64 B misc (+ 16 B per token column)
-constexpr int kSmemMax = 232448;             // opt-in dynamic shared memory per CTA
+constexpr int kFlagBytes = 4096;             // control words (128 B) + 2 flags per span
 
 struct BlobHeader {
   uint32_t magic;
@@ -88,17 +82,9 @@ __host__ __device__ inline int sw128_offset(int r, int b) {
 }
 
 // ------------------------------------------------------------------------------------------
-// GEMM kernel parameters.  One kernel serves gate_up (mode 0) and down (mode 1).  The linear sequence of
-// stages is split into a STATIC part, cut into n_spans cost-balanced spans (one per persistent CTA), and a
-// TAIL of whole tiles cut into small chunks that the CTAs claim dynamically (atomic counter) once their
-// span is issued: per-SM HBM throughput varies by +-10 % from launch to launch, the tail absorbs it.
+// GEMM kernel parameters.  One kernel serves gate_up (mode 0) and down (mode 1): a byte-balanced
+// stream-K walk over the linear sequence of stages; span i = stages [span_begin[i], span_begin[i+1]).
 // ------------------------------------------------------------------------------------------
-struct RedEntry {             // a tile whose partials are summed by the task queue
-  int tile;
-  int n_seg;                  // partials to wait for / to add, in this order:
-  int first;                  // static: first span of the group; tail: first tail-chunk index of the tile
-};
-
 struct GemmParams {
   const uint8_t* section;   // first stage image of this matrix family
   int mode;                 // 0 gate_up, 1 down
@@ -108,14 +94,6 @@ struct GemmParams {
   int n_spans;
   int M, n_pad;             // tokens in this launch, padded to 16
   int num_stages, slot_bytes, acc_stride, num_acc_bufs;
-  // dynamic tail
-  int tail_tile0;           // first tail tile (== num_tiles: no tail)
-  int tail_ts;              // mode 0: number of SPARSE tail tiles (they come first)
-  int tail_cs;              // stages per chunk
-  int tail_cpt_s, tail_cpt_d;   // chunks per sparse / dense tail tile (mode 1: tail_cpt_s = chunks per tile)
-  int n_tail_chunks;
-  // reduced tiles: [0, n_red_static) groups of > 2 static spans, then one entry per tail tile
-  int n_red, n_red_static, red_slices;
   // epilogue
   const float* s_act;       // mode 0: s_x [M]; mode 1: s_h (stride sh_stride)
   const float* s_h;         // mode 0: requant scale
@@ -127,16 +105,16 @@ struct GemmParams {
   int y_dtype;
   int ld_out;               // I (mode 0) or H (mode 1)
   int out_rows;             // valid output columns (I or H) for masking padded tiles
-  int* ws_ctrl;             // workspace control words (kCtrl*)
+  int* ws_ctrl;             // workspace control words: [0] epoch of the last finished launch, [1] finished-CTA count
   int* flags;               // workspace: 2 ints per span (first / last segment), hold the epoch of the dump
-  int* tile_cnt;            // workspace: arrival counter per reduced tile
-  float* partials;          // workspace: 2 slots per span, then one per tail chunk; slot = 2 * n_pad * 128 floats
+  float* partials;          // workspace: 2 slots per span of 2 * n_pad * 128 floats
   long long* trace;         // debug timeline (16 slots per span) or nullptr
   const uint8_t* next_base; // section the NEXT kernel of the stream will stream (L2 prefetch during our tail) or nullptr
   int span_begin[kMaxSpans + 1];
   uint32_t next_off[kMaxSpans];   // byte offset of span i's first stage in next_base ...
   uint32_t next_len[kMaxSpans];   // ... and how many bytes of it to prefetch
-  RedEntry red[kMaxRed];
+  uint32_t self_off[kMaxSpans];   // own span: bytes past the ring prefill where the L2 self-prefetch starts ...
+  uint32_t self_len[kMaxSpans];   // ... and its length (issued while waiting for the previous kernel)
 };
 
 // ------------------------------------------------------------------------------------------

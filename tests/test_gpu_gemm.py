@@ -163,41 +163,3 @@ def test_gemm_argument_errors(sp):
     with pytest.raises(sp.SpenseError) as e:
         sp.spense_gate_up(bad, cuda(c.x), cuda(c.s_x), cuda(torch.ones(1)), ws)
     assert e.value.code == "SPENSE_ERR_BAD_BLOB"
-
-
-# tail_frac, tail_cs, max_spans, min_static: force the dynamic tail / the multi-way task reductions on small shapes
-KNOBS = [(0.3, 1, 0, 0), (0.5, 2, 7, 0), (0.25, 3, 0, 0), (0.0, 0, 0, 0), (0.9, 1, 3, 0)]
-
-
-@pytest.mark.parametrize("knobs", KNOBS)
-@pytest.mark.parametrize("H,I,p,M", [(1024, 4096, 0.25, 64), (512, 1024, 0.5, 17), (768, 2048, 0.0, 128), (1024, 2048, 1.0, 40)])
-def test_dynamic_tail_and_task_reductions(sp, knobs, H, I, p, M):
-    """The schedule knobs change only WHO computes WHAT partial: results must stay within the tolerance,
-    chained == separate calls, and repeated runs bitwise identical whatever CTA claimed which chunk."""
-    import ctypes
-    L = sp.lib()
-    L.spense_debug_set_schedule.argtypes = [ctypes.c_double, ctypes.c_int, ctypes.c_int, ctypes.c_int]
-    L.spense_debug_set_schedule.restype = None
-    L.spense_debug_set_schedule(*knobs)
-    try:
-        c = Case(H, I, p, M, seed=5000 + H + I + M)
-        pk = c.pack_gpu(sp)
-        s_h = c.default_s_h()
-        r = c.oracle_gate_up(s_h)
-        ws = sp.spense_workspace(pk, M)
-        h_gpu, hq_gpu = run_gate_up(sp, c, pk, s_h, ws)
-        assert_gate_up_parity(r, h_gpu, hq_gpu, s_h, f"gate_up knobs={knobs}")
-        sh_dev = cuda(torch.from_numpy(s_h))
-        ys = []
-        for _ in range(4):
-            ys.append(sp.spense_mlp(pk, cuda(c.x), cuda(c.s_x), sh_dev, ws))
-        y_sep = sp.spense_down(pk, cuda(torch.from_numpy(hq_gpu)), sh_dev, ws)
-        torch.cuda.synchronize()
-        assert_down_parity(y_sep.cpu().numpy(), hq_gpu, s_h, c.wd, c.L.w_scale[2], f"down knobs={knobs}")
-        for y in ys:
-            assert torch.equal(y, y_sep)
-        ctrl = ws[:32].view(torch.int32).cpu()
-        assert int(ctrl[1]) == 0 and int(ctrl[2]) == 0 and int(ctrl[3]) == 0 and int(ctrl[4]) == 0
-        assert int(ws[2048:2048 + 4 * 224].view(torch.int32).abs().sum()) == 0     # tile counters reset by the last CTA
-    finally:
-        L.spense_debug_set_schedule(-1.0, 0, 0, -1)

@@ -184,7 +184,7 @@ int read_header(const void* d_blob, const spense_shape_t* shape, BlobHeader* out
 
 // bytes of span k that the PREVIOUS launch pulls into L2 during its tail: at least one ring
 uint32_t next_prefetch_bytes(const Schedule& sc, int k) {
-  static const uint32_t want = (uint32_t)(env_double("SPENSE_PF_NEXT_KB", 0.0) * 1024.0);
+  static const uint32_t want = (uint32_t)(env_double("SPENSE_PF_NEXT_KB", 640.0) * 1024.0);
   uint32_t n = sc.span_pre[k] > want ? sc.span_pre[k] : want;
   return n < sc.span_len[k] ? n : sc.span_len[k];
 }
@@ -196,7 +196,7 @@ void fill_common(GemmParams& p, const Schedule& sc, int M, int n_pad, void* d_ws
   if (g_trace) g_trace += (size_t)kMaxSpans * 16;   // debug: consecutive launches fill consecutive timelines
   p.n_spans = sc.n_spans;
   std::memcpy(p.span_begin, sc.span_begin, sizeof(int) * (sc.n_spans + 1));
-  static const uint32_t self_want = (uint32_t)(env_double("SPENSE_PF_SELF_KB", 0.0) * 1024.0);
+  static const uint32_t self_want = (uint32_t)(env_double("SPENSE_PF_SELF_KB", 160.0) * 1024.0);
   for (int i = 0; i < sc.n_spans; ++i) {                    // own stages pulled into L2 while waiting for the previous kernel
     const uint32_t from = next_prefetch_bytes(sc, i);
     const uint32_t left = sc.span_len[i] - from;
@@ -219,6 +219,8 @@ void fill_next(GemmParams& p, const uint8_t* next_section, const Schedule& next)
   static const bool enabled = env_double("SPENSE_L2_PREFETCH", 1.0) != 0.0;
   if (!enabled || !next_section) return;
   p.next_base = next_section;
+  static const int pace = (int)env_double("SPENSE_PF_PACE_NS", 750.0);
+  p.pf_pace_ns = pace;
   for (int i = 0; i < p.n_spans; ++i) {
     const int k = i < next.n_spans ? i : next.n_spans - 1;
     p.next_off[i] = next.span_off[k];

@@ -191,12 +191,14 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
   uint8_t* smem_gen = smem_raw + (smem_base - smem_u32(smem_raw));
   volatile uint32_t* tmem_slot_ptr = reinterpret_cast<volatile uint32_t*>(smem_gen + ring_bytes + 8 * 20);
   volatile int* epoch_ptr = reinterpret_cast<volatile int*>(smem_gen + ring_bytes + 8 * 21);
+  volatile int* epi_done_ptr = reinterpret_cast<volatile int*>(smem_gen + ring_bytes + 8 * 23);   // epilogue finished (stops the paced prefetch)
 
   if (warp == 0 && lane == 0) {
     prefetch_tmap(&tmap_b);
     for (int s = 0; s < S; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(accf_bar(b), 1); mbar_init(acce_bar(b), kEpiThreads); }
     mbar_init(red_bar, 1);
+    *epi_done_ptr = 0;
     fence_barrier_init();
   }
   if (warp == 2) tmem_alloc(tmem_slot, kTmemCols);
@@ -276,7 +278,24 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
       trace(p, span, 2);
       // HBM goes idle while the CTAs run their fix-up tails: use that time to pull the first stages of
       // the NEXT kernel's span into L2 (the next GEMM of this layer / the next layer's gate_up).
-      if (p.next_base) prefetch_l2(p.next_base + (size_t)p.next_off[span], p.next_len[span]);
+      if (p.next_base) {
+        const uint8_t* nb = p.next_base + (size_t)p.next_off[span];
+        const uint32_t bytes = p.next_len[span];
+        if (p.pf_pace_ns == 0) {
+          prefetch_l2(nb, bytes);
+        } else {
+          // paced: one 32 KB chunk per pf_pace_ns, so the queue in front of the fix-up traffic stays shallow;
+          // stops when this CTA's epilogue is done (the CTA must not outlive its own work)
+          long long t_next = globaltimer();
+#pragma unroll 1
+          for (uint32_t o = 0; o < bytes && *epi_done_ptr == 0; o += 32768u) {
+            const uint32_t chunk = bytes - o < 32768u ? bytes - o : 32768u;
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(nb + o), "r"(chunk) : "memory");
+            t_next += p.pf_pace_ns;
+            while (globaltimer() < t_next && *epi_done_ptr == 0) __nanosleep(64);
+          }
+        }
+      }
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
@@ -418,6 +437,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
           ++red_round;
           if (et == 0) trace(p, span, 8);
         }
+        if (seg_end == se && n_groups == 0 && et == 0) *epi_done_ptr = 1;   // last epilogue of this CTA: stop prefetching now
 #pragma unroll 1
         for (int c = c_begin; c < c_end; c += 8) {
           uint32_t v0[8], v1[8];
@@ -503,6 +523,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
           mbar_wait(red_bar, red_round & 1u);
           ++red_round;
           if (et == 0) trace(p, span, 15);
+          if (gi == n_groups - 1 && mc + cc_max >= m1 && et == 0) *epi_done_ptr = 1;
           const int rrow = et & 127;
 #pragma unroll 1
           for (int c = et >> 7; c < cc; c += kEpiThreads >> 7) {
@@ -518,6 +539,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
       }
       if (et == 0) trace(p, span, 9);
     }
+    if (et == 0) *epi_done_ptr = 1;
     if (p.trace && et == 0) { p.trace[(size_t)span * 16 + 10] = globaltimer(); p.trace[(size_t)span * 16 + 11] = (se - sb) | (seg << 16); p.trace[(size_t)span * 16 + 13] = globaltimer(); }
   }
 

@@ -108,6 +108,7 @@ struct GemmParams {
   int* ws_ctrl;             // workspace control words: [0] epoch of the last finished launch, [1] finished-CTA count
   int* flags;               // workspace: 2 ints per span (first / last segment), hold the epoch of the dump
   float* partials;          // workspace: 2 slots per span of 2 * n_pad * 128 floats
+  int pf_pace_ns;           // next-kernel L2 prefetch: nanoseconds per 32 KB chunk (0 = all at once)
   long long* trace;         // debug timeline (16 slots per span) or nullptr
   const uint8_t* next_base; // section the NEXT kernel of the stream will stream (L2 prefetch during our tail) or nullptr
   int span_begin[kMaxSpans + 1];
@@ -149,6 +150,11 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 __device__ __forceinline__ uint64_t policy_evict_first() {
   uint64_t p;
   asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ uint64_t policy_evict_normal() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
   return p;
 }
 __device__ __forceinline__ uint64_t policy_evict_last() {

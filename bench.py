@@ -28,7 +28,7 @@ H, I, P_DENSE = 5120, 25600, 0.25
 LAYERS = 8
 # dram__bytes_read.sum + dram__bytes_write.sum of the two spense_gemm_kernel launches of one layer at
 # M=64, from the committed ncu capture (profiles/); per layer, like `achieved`.
-NCU_TRAFFIC_BYTES_PER_LAYER = None
+NCU_TRAFFIC_BYTES_PER_LAYER = 285426304   # r01_traffic_app_replay_M64.csv: 16 launches = 8 layers, read + write
 
 
 def algorithmic_bytes(M: int, I_d: int) -> int:
@@ -140,8 +140,128 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def run_report(args):
+    """--report: the other BASELINE.json configs (context rows, not the bench line): Seed-OSS-36B shape
+    dense-fraction sweep, the 64-layer Qwen3-32B-shaped stack, prefill-shaped GEMMs.  Writes one JSON
+    object to stdout and to gpurun_out/report.json.  Same timing rules as the bench line (CUDA graph,
+    CUDA events, layers rotate so every weight byte streams from HBM)."""
+    import torch
+    import spense_inputs as si
+    from paper_2606_10445_b200 import build, spense as sp
+    build.build()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peak, _ = read_peaks()
+    out = {"hbm_peak_gbs": peak}
+
+    def blobs_of(h, i, p, n, seed0, i_dense=None):
+        res = []
+        for k in range(n):
+            L = si.make_layer(h, i, p, seed0 + k, device=dev, I_dense=i_dense)
+            res.append(sp.spense_pack(L.wgate, L.wup, L.wdown, L.w_scale, L.perm, L.I_dense))
+            del L
+        torch.cuda.empty_cache()
+        return res
+
+    def graph_time(fn, reps=20, warm=5):
+        fn(); torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        s = torch.cuda.Stream()
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            with torch.cuda.graph(g, stream=s):
+                fn()
+        torch.cuda.current_stream().wait_stream(s)
+        for _ in range(warm):
+            g.replay()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            g.replay()
+        e1.record(); torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e3 / reps          # us per replay
+
+    def w_bytes(h, i, i_d):
+        return 3 * h * (i_d + (i - i_d) * 0.625)
+
+    def act_bytes(m, h, i):
+        return m * h + 4 * m + 2 * m * i + 2 * m * h
+
+    # ---- config 3: Seed-OSS-36B-shaped layer, p sweep x M sweep, speedup vs the all-dense kernel
+    h, i = 5120, 27648
+    rows, dense_t = [], {}
+    for p in (1.0, 0.0, 0.10, 0.25, 0.50):
+        nl = 5
+        bl = blobs_of(h, i, p, nl, 4000 + int(p * 100) * 10)
+        i_d = bl[0].I_dense
+        ws = sp.spense_workspace(bl[0], 256)
+        for m in (1, 16, 64, 256):
+            x, sx = si.make_activations(m, h, 1000 + m, device=dev)
+            sh = torch.full((m,), 0.05, device=dev)
+            hq = torch.empty(m, i, dtype=torch.uint8, device=dev)
+            y = torch.empty(m, h, dtype=torch.bfloat16, device=dev)
+            t = graph_time(lambda: [sp.spense_mlp(b, x, sx, sh, ws, hq_scratch=hq, y=y, next_layer=bl[(k + 1) % nl])
+                                    for k, b in enumerate(bl)]) / nl
+            if p == 1.0:
+                dense_t[m] = t
+            algo = w_bytes(h, i, i_d) + act_bytes(m, h, i)
+            rows.append({"p": p, "I_dense": i_d, "M": m, "us_per_layer": round(t, 2), "gbs": round(algo / t / 1e3, 1),
+                         "frac_of_hbm_peak": round(algo / t / 1e3 / peak, 3),
+                         "speedup_vs_dense": round(dense_t[m] / t, 3),
+                         "byte_ratio_bound": round(w_bytes(h, i, i) / w_bytes(h, i, i_d), 3)})
+        del bl, ws
+        torch.cuda.empty_cache()
+    out["seed_oss_36b_sweep"] = rows
+
+    # ---- config 4: 64 consecutive Qwen3-32B-shaped layers (18 GB of blobs), one CUDA graph, tokens/s
+    nl = 64
+    bl = blobs_of(H, I, P_DENSE, nl, 6000)
+    ws = sp.spense_workspace(bl[0], 256)
+    stack = []
+    for m in (32, 128):
+        x, sx = si.make_activations(m, H, 1000 + m, device=dev)
+        sh = torch.full((m,), 0.05, device=dev)
+        hq = torch.empty(m, I, dtype=torch.uint8, device=dev)
+        y = torch.empty(m, H, dtype=torch.bfloat16, device=dev)
+        t = graph_time(lambda: [sp.spense_mlp(b, x, sx, sh, ws, hq_scratch=hq, y=y, next_layer=bl[(k + 1) % nl])
+                                for k, b in enumerate(bl)], reps=10, warm=3)
+        algo = nl * (w_bytes(H, I, bl[0].I_dense) + act_bytes(m, H, I))
+        stack.append({"M": m, "layers": nl, "ms_per_stack": round(t / 1e3, 4), "us_per_layer": round(t / nl, 2),
+                      "tokens_per_s": round(m / (t * 1e-6), 1), "gbs": round(algo / t / 1e3, 1),
+                      "frac_of_hbm_peak": round(algo / t / 1e3 / peak, 3)})
+    out["qwen3_32b_stack"] = stack
+
+    # ---- config 5: prefill-shaped GEMMs, gate_up and down separately (the decode kernel run over 128-token
+    # blocks: weights are re-streamed per block, so this is far from the tensor roofline -- NEXT-3)
+    pre = []
+    for m in (2048, 8192):
+        x, sx = si.make_activations(m, H, 1000 + m, device=dev)
+        sh = torch.full((m,), 0.05, device=dev)
+        hq = torch.empty(m, I, dtype=torch.uint8, device=dev)
+        y = torch.empty(m, H, dtype=torch.bfloat16, device=dev)
+        four = bl[:4]
+        t_gu = graph_time(lambda: [sp.spense_gate_up(b, x, sx, sh, ws, hq=hq) for b in four], reps=3, warm=1) / 4
+        t_dn = graph_time(lambda: [sp.spense_down(b, hq, sh, ws, y=y) for b in four], reps=3, warm=1) / 4
+        i_d = bl[0].I_dense
+        macs_gu = m * 2 * H * (i_d + (I - i_d) / 2)          # executed MACs (2:4 tiles do half)
+        macs_dn = m * H * (i_d + (I - i_d) / 2)
+        pre.append({"M": m, "gate_up_us": round(t_gu, 1), "down_us": round(t_dn, 1),
+                    "gate_up_executed_tflops": round(2 * macs_gu / t_gu / 1e6, 1),
+                    "down_executed_tflops": round(2 * macs_dn / t_dn / 1e6, 1),
+                    "gate_up_dense_equiv_tflops": round(2 * m * 2 * H * I / t_gu / 1e6, 1),
+                    "down_dense_equiv_tflops": round(2 * m * H * I / t_dn / 1e6, 1),
+                    "fp8_dense_peak_tflops_nominal": 4500.0})
+    out["prefill_shaped"] = pre
+    os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
+    with open(os.path.join(ROOT, "gpurun_out", "report.json"), "w") as f:
+        json.dump(out, f, indent=1)
+    print(json.dumps(out))
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--report", action="store_true")
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=10)
@@ -152,6 +272,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.report:
+        return run_report(args)
 
     import torch
     import spense_inputs as si

@@ -142,6 +142,19 @@ int spense_mlp(const spense_shape_t* shape, const void* d_blob, const uint8_t* d
                void* d_y, int32_t y_dtype, void* d_ws, size_t ws_bytes, const void* d_next_blob,
                spense_stream_t stream);
 
+/* spense_mlp_dyn -- the whole layer with DYNAMIC per-token re-quantisation of h (the
+ * paper's FP8 serving runs quantise activations dynamically): the scale is not an input,
+ *   s_h[m] = max_j |h[m, j]| / 448   (fp32 division; 1 if the row is all zero),
+ *   Hq[m, j] = E4M3_rne_sat(h[m, j] / s_h[m]),   y as in spense_down with that s_h.
+ * Three stream-ordered steps (programmatic dependent launch): gate_up leaves h in fp32 in d_h_scratch and
+ * the per-CTA maxima of |h| in the workspace, a row kernel forms s_h and Hq, down consumes them.
+ *   d_sh_out [M] fp32 (written); d_hq_scratch [M, I] bytes (written); d_h_scratch [M, I] fp32 (written);
+ *   other arguments as in spense_mlp.  Same status codes.                                            */
+int spense_mlp_dyn(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx,
+                   int32_t M, float* d_sh_out, uint8_t* d_hq_scratch, float* d_h_scratch, void* d_y,
+                   int32_t y_dtype, void* d_ws, size_t ws_bytes, const void* d_next_blob,
+                   spense_stream_t stream);
+
 /* spense_mlp_host -- same, with HOST activations and results: copies h_x [M, H], h_sx [M], h_sh
  * (1 or M floats) to the device staging buffers, runs spense_mlp, copies y back to h_y and
  * synchronises the stream.  Staging (device): d_x [M, H], d_scales [2*M] fp32, d_hq_scratch [M, I],

@@ -351,6 +351,18 @@ def requant_scale_from_h(h: np.ndarray) -> np.ndarray:
     return np.where(amax > 0, (amax / np.float32(E4M3_MAX)).astype(np.float32), np.float32(1)).astype(np.float32)
 
 
+def mlp_dynamic(xq, s_x, wg_bytes, wu_bytes, wd_bytes, w_scale):
+    """The layer with DYNAMIC per-token re-quantisation (Q10: the paper is
+    silent on how h is re-quantised, its vLLM FP8 runs quantise activations dynamically):
+    s_h[m] = max_j |h[m, j]| / 448 from the layer's own h, then the static path with that scale."""
+    r = gate_up(xq, s_x, wg_bytes, wu_bytes, w_scale[0], w_scale[1], 1.0)
+    s_h = requant_scale_from_h(r["h"])
+    r = gate_up(xq, s_x, wg_bytes, wu_bytes, w_scale[0], w_scale[1], s_h)
+    r.update(down(r["hq"], s_h, wd_bytes, w_scale[2]))
+    r["s_h"] = s_h
+    return r
+
+
 # tolerance companions (O6): north_star bound |gpu - oracle| <= 2e-3 * sum|a*w| + 1e-5
 def tol_gemm(abs_sum):
     return 2e-3 * np.asarray(abs_sum) + 1e-5

@@ -49,7 +49,7 @@ bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) %
 
 int n_pad_of(int M) { int n = (M + 15) / 16 * 16; return n > 128 ? 128 : n; }
 
-size_t ws_bytes_for(int n_pad, int spans) { return kFlagBytes + (size_t)spans * 2 * 2 * n_pad * 128 * sizeof(float); }
+size_t ws_bytes_for(int n_pad, int spans) { return kFlagBytes + kAmaxBytes + (size_t)spans * 2 * 2 * n_pad * 128 * sizeof(float); }
 
 double env_double(const char* name, double dflt) {
   const char* v = std::getenv(name);
@@ -211,7 +211,7 @@ void fill_common(GemmParams& p, const Schedule& sc, int M, int n_pad, void* d_ws
   p.num_acc_bufs = n_pad <= 64 ? 2 : 1;
   p.ws_ctrl = reinterpret_cast<int*>(d_ws);
   p.flags = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(d_ws) + 128);
-  p.partials = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes);
+  p.partials = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes + kAmaxBytes);
 }
 
 // L2 prefetch hint: while this launch runs its fix-up tail, pull what the next launch streams first.
@@ -230,7 +230,7 @@ void fill_next(GemmParams& p, const uint8_t* next_section, const Schedule& next)
 
 int gate_up_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_x,
                  const float* d_sx, int32_t M, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32,
-                 void* d_ws, bool pdl, bool down_follows, cudaStream_t stream) {
+                 void* d_ws, bool pdl, bool down_follows, cudaStream_t stream, bool dynamic = false) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
   for (int m0 = 0; m0 < M; m0 += 128) {
     const int Mb = (M - m0) < 128 ? (M - m0) : 128;
@@ -247,6 +247,7 @@ int gate_up_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void*
     p.w_scale0 = hdr.w_scale[0]; p.w_scale1 = hdr.w_scale[1];
     p.hq = d_hq + (size_t)m0 * g.I;
     p.h_f32 = d_h_f32 ? d_h_f32 + (size_t)m0 * g.I : nullptr;
+    p.amax_part = dynamic ? reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes) : nullptr;
     p.ld_out = g.I; p.out_rows = g.I;
     if (down_follows && m0 + 128 >= M)                       // the same layer's down projection streams next
       fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off, get_schedule(1, g, n_pad_of(M < 128 ? M : 128), g_num_sms));
@@ -447,6 +448,41 @@ int spense_mlp(const spense_shape_t* shape, const void* d_blob, const uint8_t* d
   st = gate_up_impl(shape, hdr, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq_scratch, d_h_f32, d_ws, true, true, s);
   if (st) return st;
   return down_impl(shape, hdr, d_blob, d_hq_scratch, d_sh, sh_stride, M, d_y, y_dtype, d_ws, true, d_next_blob, s);
+}
+
+int spense_mlp_dyn(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx, int32_t M,
+                   float* d_sh_out, uint8_t* d_hq_scratch, float* d_h_scratch, void* d_y, int32_t y_dtype, void* d_ws,
+                   size_t ws_bytes, const void* d_next_blob, spense_stream_t stream) {
+  int st = check_shape(shape);
+  if (st) return st;
+  if (!d_blob || !d_x || !d_sx || !d_sh_out || !d_hq_scratch || !d_h_scratch || !d_y || M < 1 ||
+      (y_dtype != SPENSE_F32 && y_dtype != SPENSE_BF16))
+    return SPENSE_ERR_ARG;
+  if (!aligned(d_blob, 128) || !aligned(d_x, 128) || !aligned(d_hq_scratch, 128) || !aligned(d_y, 16) ||
+      !aligned(d_sx, 4) || !aligned(d_sh_out, 4) || !aligned(d_h_scratch, 16) || !aligned(d_next_blob, 128))
+    return SPENSE_ERR_ALIGN;
+  st = check_ws(shape, M, d_ws, ws_bytes);
+  if (st) return st;
+  st = check_device();
+  if (st) return st;
+  BlobHeader hdr;
+  st = read_header(d_blob, shape, &hdr);
+  if (st) return st;
+  cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
+  const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
+  const float* amax = reinterpret_cast<const float*>(reinterpret_cast<const uint8_t*>(d_ws) + kFlagBytes);
+  for (int m0 = 0; m0 < M; m0 += 128) {                      // gate_up (h in fp32, max|h| per CTA) -> requant, per token block
+    const int Mb = (M - m0) < 128 ? (M - m0) : 128;
+    const int n_pad = n_pad_of(Mb);
+    st = gate_up_impl(shape, hdr, d_blob, d_x + (size_t)m0 * g.H, d_sx + m0, Mb, d_sx, 0, d_hq_scratch + (size_t)m0 * g.I,
+                      d_h_scratch + (size_t)m0 * g.I, d_ws, true, m0 + 128 >= M, s, true);
+    if (st) return st;
+    const Schedule& sc = get_schedule(0, g, n_pad, g_num_sms);
+    st = launch_requant_rows(d_h_scratch + (size_t)m0 * g.I, Mb, g.I, amax, sc.n_spans, n_pad, d_hq_scratch + (size_t)m0 * g.I,
+                             d_sh_out + m0, s);
+    if (st) return st;
+  }
+  return down_impl(shape, hdr, d_blob, d_hq_scratch, d_sh_out, 1, M, d_y, y_dtype, d_ws, true, d_next_blob, s);
 }
 
 int spense_mlp_host(const spense_shape_t* shape, const void* d_blob, const uint8_t* h_x, const float* h_sx, int32_t M,

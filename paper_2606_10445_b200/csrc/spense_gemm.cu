@@ -144,8 +144,16 @@ __device__ __forceinline__ void finish(const GemmParams& p, const float4* sc, in
     const float g = f0 * k.x;
     const float u = f1 * k.y;
     const float h = silu_mul(g, u);
-    const float qv = div_by(h, k.z, k.w);
     const size_t o = (size_t)m * p.ld_out + tile * 128 + r;
+    if (p.amax_part) {
+      // dynamic requant: keep h in fp32 and track max|h| per token; the scale does not
+      // exist yet, spense_requant turns h into Hq once every tile is done.  Called warp-uniformly in m.
+      p.h_f32[o] = h;
+      const int mx = __reduce_max_sync(0xffffffffu, __float_as_int(fabsf(h)));   // |h| >= 0: int order == float order
+      if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<int*>(const_cast<float4*>(sc) + m) + 2, mx);
+      return;
+    }
+    const float qv = div_by(h, k.z, k.w);
     if (p.h_f32) p.h_f32[o] = h;
     p.hq[o] = (uint8_t)(to_e4m3x2(qv, 0.0f) & 0xFFu);
   } else {
@@ -376,8 +384,8 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
       float4 k = make_float4(0.f, 0.f, 0.f, 0.f);
       if (MODE == 0) {
         const float sx = __ldg(p.s_act + m);
-        const float sh = __ldg(p.s_h + (size_t)m * p.sh_stride);
-        k = make_float4(sx * p.w_scale0, sx * p.w_scale1, sh, __frcp_rn(sh));
+        const float sh = p.amax_part ? 1.0f : __ldg(p.s_h + (size_t)m * p.sh_stride);
+        k = make_float4(sx * p.w_scale0, sx * p.w_scale1, p.amax_part ? 0.0f : sh, __frcp_rn(sh));   // dynamic: .z = running max|h| bits
       } else {
         k.x = __ldg(p.s_act + (size_t)m * p.sh_stride) * p.w_scale0;
       }
@@ -538,6 +546,10 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
         }
       }
       if (et == 0) trace(p, span, 9);
+    }
+    if (MODE == 0 && p.amax_part) {                          // this CTA's max|h| per token, for spense_requant
+      epi_sync();
+      if (et < p.n_pad) p.amax_part[(size_t)span * p.n_pad + et] = et < p.M ? sc[et].z : 0.0f;
     }
     if (et == 0) *epi_done_ptr = 1;
     if (p.trace && et == 0) { p.trace[(size_t)span * 16 + 10] = globaltimer(); p.trace[(size_t)span * 16 + 11] = (se - sb) | (seg << 16); p.trace[(size_t)span * 16 + 13] = globaltimer(); }

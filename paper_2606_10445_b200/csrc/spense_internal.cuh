@@ -37,6 +37,7 @@ constexpr uint32_t kBlobMagic = 0x53504E53u;  // "SNPS"
 constexpr int kBlobVersion = 1;
 constexpr int kMaxSpans = 160;
 constexpr int kFlagBytes = 4096;             // control words (128 B) + 2 flags per span
+constexpr int kAmaxBytes = 160 * 128 * 4;    // dynamic requant: max|h| per span and token (follows the flags)
 
 struct BlobHeader {
   uint32_t magic;
@@ -101,6 +102,7 @@ struct GemmParams {
   float w_scale0, w_scale1; // mode 0: gate, up; mode 1: down, down
   uint8_t* hq;              // mode 0 out [M, ld_out]
   float* h_f32;             // mode 0 optional out
+  float* amax_part;         // mode 0, dynamic requant: per-span per-token max|h| [n_spans][n_pad] (then hq is not written)
   void* y;                  // mode 1 out [M, ld_out]
   int y_dtype;
   int ld_out;               // I (mode 0) or H (mode 1)
@@ -252,6 +254,8 @@ int launch_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8
                 const float* h_w_scale, const int32_t* d_perm, void* d_blob, const spense_canon_t* canon, void* d_ws,
                 int64_t* h_err_where, cudaStream_t stream);
 int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, bool pdl, cudaStream_t stream);
+int launch_requant_rows(const float* d_h, int rows, int cols, const float* d_amax_part, int n_part, int part_stride,
+                        uint8_t* d_hq, float* d_sh, cudaStream_t stream);
 int launch_quantize(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out, float* d_scales,
                     void* d_ws, cudaStream_t stream);
 

@@ -231,7 +231,50 @@ __global__ void quantize_kernel(const float* __restrict__ in, int64_t cols, cons
   }
 }
 
+// ---------------------------------------------------------------- dynamic per-token requant
+// h [rows, cols] fp32 (written by gate_up in dynamic mode) -> s_h[m] = max_j|h[m,j]| / 448 (1 if zero),
+// Hq[m,j] = E4M3_rne_sat(h[m,j] / s_h[m]).  The row maximum comes from the per-CTA maxima gate_up left in
+// amax_part [n_part][part_stride] (no atomics, nothing to reset).  grid = (column chunks of 4096, rows).
+__global__ void __launch_bounds__(256) requant_rows_kernel(const float* __restrict__ h, int cols, const float* __restrict__ amax_part,
+                                                           int n_part, int part_stride, uint8_t* __restrict__ hq,
+                                                           float* __restrict__ s_h) {
+  asm volatile("griddepcontrol.wait;" ::: "memory");            // h and amax_part come from the previous kernel
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  const int row = blockIdx.y;
+  float m = 0.0f;
+  for (int i = threadIdx.x; i < n_part; i += blockDim.x) m = fmaxf(m, __ldcg(amax_part + (size_t)i * part_stride + row));
+  m = block_max(m);
+  const float s = m > 0.0f ? __fdiv_rn(m, 448.0f) : 1.0f;
+  if (blockIdx.x == 0 && threadIdx.x == 0) s_h[row] = s;
+  const int c0 = blockIdx.x * 4096;
+  const float4* src = reinterpret_cast<const float4*>(h + (size_t)row * cols + c0);
+  uint32_t* dst = reinterpret_cast<uint32_t*>(hq + (size_t)row * cols + c0);
+  const int n4 = min(4096, cols - c0) >> 2;                      // cols % 128 == 0
+  for (int i = threadIdx.x; i < n4; i += blockDim.x) {
+    const float4 v = __ldcg(src + i);
+    uint16_t lo, hi;
+    asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(lo) : "f"(__fdiv_rn(v.y, s)), "f"(__fdiv_rn(v.x, s)));
+    asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(hi) : "f"(__fdiv_rn(v.w, s)), "f"(__fdiv_rn(v.z, s)));
+    dst[i] = (uint32_t)lo | ((uint32_t)hi << 16);
+  }
+}
+
 }  // namespace
+
+int launch_requant_rows(const float* d_h, int rows, int cols, const float* d_amax_part, int n_part, int part_stride,
+                        uint8_t* d_hq, float* d_sh, cudaStream_t stream) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)((cols + 4095) / 4096), (unsigned)rows);
+  cfg.blockDim = dim3(256);
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  const cudaError_t e = cudaLaunchKernelEx(&cfg, requant_rows_kernel, d_h, cols, d_amax_part, n_part, part_stride, d_hq, d_sh);
+  return e == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;
+}
 
 int launch_quantize(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out, float* d_scales,
                     void* d_ws, cudaStream_t stream) {

@@ -23,7 +23,7 @@ STATUS = {0: "SPENSE_OK", -1: "SPENSE_ERR_ARG", -2: "SPENSE_ERR_ALIGN", -3: "SPE
 
 EXPORTS = ["spense_version", "spense_strerror", "spense_perm_from_dense_idx", "spense_pack_sizes", "spense_pack",
            "spense_workspace_size", "spense_workspace_init", "spense_gate_up", "spense_down", "spense_mlp",
-           "spense_mlp_host", "spense_quantize_e4m3"]
+           "spense_mlp_dyn", "spense_mlp_host", "spense_quantize_e4m3"]
 
 
 class SpenseError(RuntimeError):
@@ -69,6 +69,8 @@ def lib() -> ctypes.CDLL:
                                   c_void_p, c_size_t, c_void_p, c_void_p]
         L.spense_mlp.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_int32, c_void_p, c_int32, c_void_p,
                                  c_void_p, c_void_p, c_int32, c_void_p, c_size_t, c_void_p, c_void_p]
+        L.spense_mlp_dyn.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_int32, c_void_p, c_void_p, c_void_p,
+                                     c_void_p, c_int32, c_void_p, c_size_t, c_void_p, c_void_p]
         L.spense_mlp_host.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_int32, c_void_p, c_int32,
                                       c_void_p, c_int32, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_size_t,
                                       c_void_p, c_void_p]
@@ -212,6 +214,23 @@ def spense_mlp(layer: PackedLayer, x, s_x, s_h, ws, hq_scratch=None, y=None, h_f
                             SPENSE_F32 if y.dtype == torch.float32 else SPENSE_BF16, _ptr(ws), ws.numel(),
                             _next(next_layer), _stream()))
     return y
+
+
+def spense_mlp_dyn(layer: PackedLayer, x, s_x, ws, s_h=None, hq_scratch=None, h_scratch=None, y=None,
+                   dtype=torch.float32, next_layer=None):
+    """The layer with dynamic per-token requant: returns (y, s_h [M], hq [M, I], h fp32 [M, I])."""
+    _dev(x, torch.uint8), _dev(s_x, torch.float32)
+    M = x.shape[0]
+    dev = x.device
+    s_h = torch.empty(M, dtype=torch.float32, device=dev) if s_h is None else s_h
+    hq_scratch = torch.empty(M, layer.I, dtype=torch.uint8, device=dev) if hq_scratch is None else hq_scratch
+    h_scratch = torch.empty(M, layer.I, dtype=torch.float32, device=dev) if h_scratch is None else h_scratch
+    y = torch.empty(M, layer.H, dtype=dtype, device=dev) if y is None else y
+    _check(lib().spense_mlp_dyn(ctypes.byref(layer.shape), _ptr(layer.blob), _ptr(x), _ptr(s_x), M, _ptr(s_h),
+                                _ptr(hq_scratch), _ptr(h_scratch), _ptr(y),
+                                SPENSE_F32 if y.dtype == torch.float32 else SPENSE_BF16, _ptr(ws), ws.numel(),
+                                _ptr(next_layer.blob) if next_layer is not None else None, _stream()))
+    return y, s_h, hq_scratch, h_scratch
 
 
 def spense_mlp_host(layer: PackedLayer, h_x, h_sx, h_sh, h_y, staging, ws, next_layer=None):

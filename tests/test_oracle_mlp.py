@@ -132,3 +132,30 @@ def test_small_integer_case_is_integral():
     wg, wu, wd, x = si.make_small_int_case(256, 512, 128, 4, seed=1)
     acc, ab = o.gemm_exact(x.numpy(), wg.numpy())
     assert np.array_equal(acc, np.round(acc)) and ab.max() < 2 ** 24
+
+
+def test_dynamic_requant_scale_pins():
+    """NEXT-1 pins: per token the element of largest |h| lands on +-448 (byte 0x7E / 0xFE), nothing saturates
+    beyond it, an all-zero token gets scale 1, and doubling the up-projection's weight scale (a power of
+    two: u and so h double exactly, SiLU(g) is untouched) doubles s_h and y while every Hq byte stays the same."""
+    L = si.make_layer(256, 1024, 0.25, seed=0)
+    x, s_x = si.make_activations(8, 256, seed=0)
+    x = x.clone()
+    x[3] = 0                                             # an all-zero token
+    c = o.pack_canonical(L.wgate.numpy(), L.wup.numpy(), L.wdown.numpy(), L.perm.numpy(), L.I_dense)
+    wg, wu, wd = o.unpack_canonical(c)
+    r = o.mlp_dynamic(x.numpy(), s_x.numpy(), wg, wu, wd, L.w_scale)
+    assert r["s_h"].dtype == np.float32 and r["s_h"][3] == 1.0 and not r["hq"][3].any() and not r["y"][3].any()
+    for m in range(8):
+        if m == 3:
+            continue
+        j = np.abs(r["h"][m]).argmax()
+        assert r["hq"][m, j] & 0x7F == 0x7E
+        assert (r["hq"][m] & 0x7F).max() == 0x7E
+        assert r["s_h"][m] == np.float32(np.float32(np.abs(r["h"][m]).max()) / np.float32(448.0))
+    ws2 = (L.w_scale[0], 2.0 * L.w_scale[1], L.w_scale[2])
+    r2 = o.mlp_dynamic(x.numpy(), s_x.numpy(), wg, wu, wd, ws2)
+    live = [0, 1, 2, 4, 5, 6, 7]
+    assert np.array_equal(r2["s_h"][live], 2.0 * r["s_h"][live])
+    assert np.array_equal(r2["hq"], r["hq"])
+    assert np.array_equal(r2["y"], 2.0 * r["y"])

@@ -362,6 +362,12 @@ def main():
             return time_steps(g.replay, 20, 5) * 1e3 / n
         extras["gate_up_us"] = t_us(lambda: [sp.spense_gate_up(b, x, sx, sh, ws, hq=hq) for b in blobs])
         extras["down_us"] = t_us(lambda: [sp.spense_down(b, hq, sh, ws, y=y) for b in blobs])
+        # NEXT-1: the same layers with dynamic per-token requant (gate_up -> row requant kernel -> down)
+        h32 = torch.empty(M, I, dtype=torch.float32, device=dev)
+        sh_dyn = torch.empty(M, device=dev)
+        extras["dynamic_requant_us"] = t_us(lambda: [sp.spense_mlp_dyn(b, x, sx, ws, s_h=sh_dyn, hq_scratch=hq, h_scratch=h32, y=y,
+                                                                       next_layer=blobs[(i + 1) % len(blobs)]) for i, b in enumerate(blobs)])
+        del h32
         sweep = []
         if not args.no_sweep:
             dense = make_blobs(1.0, 6, 3000)

@@ -49,7 +49,9 @@ bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) %
 
 int n_pad_of(int M) { int n = (M + 15) / 16 * 16; return n > 128 ? 128 : n; }
 
-size_t ws_bytes_for(int n_pad, int spans) { return kFlagBytes + kAmaxBytes + (size_t)spans * 2 * 2 * n_pad * 128 * sizeof(float); }
+size_t part_bytes_for(int n_pad, int spans) { return (size_t)spans * 2 * 2 * n_pad * 128 * sizeof(float); }
+// control words, flags, max|h| table, tile flags | partials of gate_up | partials of down (they may run concurrently)
+size_t ws_bytes_for(int n_pad, int spans) { return kWsFixedBytes + 2 * part_bytes_for(n_pad, spans); }
 
 double env_double(const char* name, double dflt) {
   const char* v = std::getenv(name);
@@ -209,9 +211,11 @@ void fill_common(GemmParams& p, const Schedule& sc, int M, int n_pad, void* d_ws
   p.num_stages = ring_stages_of(n_pad);
   p.acc_stride = n_pad <= 32 ? 32 : (n_pad <= 64 ? 64 : 128);
   p.num_acc_bufs = n_pad <= 64 ? 2 : 1;
-  p.ws_ctrl = reinterpret_cast<int*>(d_ws);
-  p.flags = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(d_ws) + 128);
-  p.partials = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes + kAmaxBytes);
+  uint8_t* ws = reinterpret_cast<uint8_t*>(d_ws);
+  const int mode = sc.mode;
+  p.ws_ctrl = reinterpret_cast<int*>(ws) + 2 * mode;
+  p.flags = reinterpret_cast<int*>(ws + 128 + mode * kMaxSpans * 2 * sizeof(int));
+  p.partials = reinterpret_cast<float*>(ws + kWsFixedBytes + (mode ? part_bytes_for(n_pad, kMaxSpans) : 0));
 }
 
 // L2 prefetch hint: while this launch runs its fix-up tail, pull what the next launch streams first.
@@ -230,7 +234,7 @@ void fill_next(GemmParams& p, const uint8_t* next_section, const Schedule& next)
 
 int gate_up_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_x,
                  const float* d_sx, int32_t M, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32,
-                 void* d_ws, bool pdl, bool down_follows, cudaStream_t stream, bool dynamic = false) {
+                 void* d_ws, bool pdl, bool down_follows, cudaStream_t stream, bool dynamic = false, bool gated = false) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
   for (int m0 = 0; m0 < M; m0 += 128) {
     const int Mb = (M - m0) < 128 ? (M - m0) : 128;
@@ -248,6 +252,10 @@ int gate_up_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void*
     p.hq = d_hq + (size_t)m0 * g.I;
     p.h_f32 = d_h_f32 ? d_h_f32 + (size_t)m0 * g.I : nullptr;
     p.amax_part = dynamic ? reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes) : nullptr;
+    if (gated) {                                             // publish a flag per finished tile: down polls them
+      p.tile_flags = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes + kAmaxBytes);
+      p.tile_cnt = p.tile_flags + kDepInts;
+    }
     p.ld_out = g.I; p.out_rows = g.I;
     if (down_follows && m0 + 128 >= M)                       // the same layer's down projection streams next
       fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off, get_schedule(1, g, n_pad_of(M < 128 ? M : 128), g_num_sms));
@@ -262,7 +270,7 @@ int gate_up_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void*
 
 int down_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_hq,
               const float* d_sh, int32_t sh_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, bool pdl,
-              const void* d_next_blob, cudaStream_t stream) {
+              const void* d_next_blob, cudaStream_t stream, bool gated = false) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
   const size_t esz = y_dtype == SPENSE_F32 ? 4 : 2;
   for (int m0 = 0; m0 < M; m0 += 128) {
@@ -280,6 +288,11 @@ int down_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_
     p.y = reinterpret_cast<uint8_t*>(d_y) + (size_t)m0 * g.H * esz;
     p.y_dtype = y_dtype;
     p.ld_out = g.H; p.out_rows = g.H;
+    if (gated) {                                             // wait per Hq tile instead of for the whole gate_up grid
+      p.dep_flags = reinterpret_cast<const int*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes + kAmaxBytes);
+      p.dep_done = reinterpret_cast<int*>(d_ws) + kCtrlDepDone;
+      p.dep_tiles = g.gu_tiles;
+    }
     if (d_next_blob && m0 + 128 >= M)                        // the next layer's gate/up weights stream next
       fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + hdr.gate_up_off, get_schedule(0, g, n_pad_of(M < 128 ? M : 128), g_num_sms));
     CUtensorMap tm;
@@ -381,8 +394,8 @@ int spense_workspace_size(const spense_shape_t* shape, int32_t M, size_t* bytes)
 
 int spense_workspace_init(void* d_ws, size_t ws_bytes, spense_stream_t stream) {
   if (!d_ws) return SPENSE_ERR_ARG;
-  if (ws_bytes < (size_t)kFlagBytes) return SPENSE_ERR_BUFFER_TOO_SMALL;
-  return cudaMemsetAsync(d_ws, 0, kFlagBytes, reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;
+  if (ws_bytes < (size_t)kWsFixedBytes) return SPENSE_ERR_BUFFER_TOO_SMALL;
+  return cudaMemsetAsync(d_ws, 0, kWsFixedBytes, reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;
 }
 
 int spense_gate_up(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx, int32_t M,
@@ -445,9 +458,12 @@ int spense_mlp(const spense_shape_t* shape, const void* d_blob, const uint8_t* d
   st = read_header(d_blob, shape, &hdr);
   if (st) return st;
   cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
-  st = gate_up_impl(shape, hdr, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq_scratch, d_h_f32, d_ws, true, true, s);
+  // one token block: down starts on the tiles gate_up has finished (flags) instead of waiting for the whole grid
+  static const bool gate_knob = env_double("SPENSE_GATE", 1.0) != 0.0;
+  const bool gated = gate_knob && M <= 128;
+  st = gate_up_impl(shape, hdr, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq_scratch, d_h_f32, d_ws, true, true, s, false, gated);
   if (st) return st;
-  return down_impl(shape, hdr, d_blob, d_hq_scratch, d_sh, sh_stride, M, d_y, y_dtype, d_ws, true, d_next_blob, s);
+  return down_impl(shape, hdr, d_blob, d_hq_scratch, d_sh, sh_stride, M, d_y, y_dtype, d_ws, true, d_next_blob, s, gated);
 }
 
 int spense_mlp_dyn(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx, int32_t M,

@@ -239,9 +239,38 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
       const int n = se - sb;
       const int pre = n < S ? n : S;
       uint32_t info[8];                                    // stages issued before pdl_wait: K coordinate | sparse << 31
+      // gate_up -> down dependency per Hq tile (spense_mlp): tiles [dep_lo, dep_hi) are known to be stored
+      int dep_lo = 0, dep_hi = 0;
+      auto need_tile = [&](int t) {
+        if (t < dep_lo || t > dep_hi) dep_lo = dep_hi = t;    // the K range restarted (next row tile): verify again
+#pragma unroll 1
+        while (dep_hi <= t) {
+          const int4* f = reinterpret_cast<const int4*>(p.dep_flags + (dep_hi & ~3));
+          int4 v[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i)
+            asm volatile("ld.volatile.global.v4.s32 {%0,%1,%2,%3}, [%4];" : "=r"(v[i].x), "=r"(v[i].y), "=r"(v[i].z), "=r"(v[i].w) : "l"(f + i));
+          uint32_t m = 0;
+#pragma unroll
+          for (int i = 0; i < 4; ++i)
+            m |= ((v[i].x != 0) | ((v[i].y != 0) << 1) | ((v[i].z != 0) << 2) | ((v[i].w != 0) << 3)) << (4 * i);
+          m >>= dep_hi & 3;
+          const int n_ready = __ffs(~m) - 1;                 // consecutive finished tiles from dep_hi on
+          if (n_ready > 0) {
+            dep_hi += n_ready;
+            asm volatile("fence.acq_rel.gpu;" ::: "memory");
+            asm volatile("fence.proxy.async.global;" ::: "memory");   // gate_up's generic-proxy stores -> our TMA reads
+          }
+        }
+      };
       auto load_b = [&](int it, uint32_t inf) {
         const uint32_t b_dst = smem_base + (uint32_t)(it % S) * p.slot_bytes + kSparseStageBytes;
         const int k0 = (int)(inf & 0x7FFFFFFFu);
+        if (MODE == 1 && p.dep_flags) {
+          const int t_last = (k0 + ((inf >> 31) ? 255 : 127)) >> 7;
+          need_tile(k0 >> 7);
+          need_tile(t_last < p.dep_tiles ? t_last : p.dep_tiles - 1);
+        }
         tma_load_2d(b_dst, &tmap_b, k0, 0, full_bar(it % S), pol_a);
         if (inf >> 31) tma_load_2d(b_dst + b_tile_bytes, &tmap_b, k0 + 128, 0, full_bar(it % S), pol_a);
       };
@@ -257,7 +286,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
       auto flush = [&]() {
         trace(p, span, 1);
         if (p.self_len[span]) prefetch_l2(src + p.self_off[span], p.self_len[span]);
-        pdl_wait();
+        if (!(MODE == 1 && p.dep_flags)) pdl_wait();
 #pragma unroll
         for (int k = 0; k < 8; ++k)
           if (k < pre) load_b(k, info[k]);
@@ -286,6 +315,9 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
       trace(p, span, 2);
       // HBM goes idle while the CTAs run their fix-up tails: use that time to pull the first stages of
       // the NEXT kernel's span into L2 (the next GEMM of this layer / the next layer's gate_up).
+      // flag-gated launch: nothing above waited for the previous grid; do it once (it is long done) so that
+      // "this kernel complete" still implies "everything before it complete" for the next kernel's PDL wait
+      if (MODE == 1 && p.dep_flags) pdl_wait();
       if (p.next_base) {
         const uint8_t* nb = p.next_base + (size_t)p.next_off[span];
         const uint32_t bytes = p.next_len[span];
@@ -377,8 +409,9 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
     const float* stg = reinterpret_cast<const float*>(smem_gen);         // the stage ring doubles as partial staging
     const size_t part_floats = (size_t)2 * p.n_pad * 128;  // one partial: [mat][col][row]
 
-    // scales, the workspace and the epoch word may be produced / still in use by the previous kernel
-    pdl_wait();
+    // scales, the workspace and the epoch word may be produced / still in use by the previous kernel; a
+    // flag-gated down has its own workspace half and caller-provided scales: it starts right away
+    if (!(MODE == 1 && p.dep_flags)) pdl_wait();
     if (et < p.n_pad) {
       const int m = et < p.M ? et : p.M - 1;
       float4 k = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -468,6 +501,10 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
         }
         tc_fence_before();
         mbar_arrive(acce_bar(buf));
+        if (MODE == 0 && p.tile_flags) {                     // Hq[:, tile] complete: all stores issued, one release
+          epi_sync();
+          if (et == 0) st_release(p.tile_flags + cur.tile, 1);
+        }
       } else {
         // split tile, not (solely) ours to finish: dump the raw fp32 partial [mat][col][row] and publish it
         const int which = (sb >= cur.first) ? 0 : 1;       // our first segment, or our last one
@@ -545,11 +582,30 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
           }
         }
       }
+      if (MODE == 0 && p.tile_flags) {                       // the last of the n reducers publishes the tile
+        epi_sync();
+        if (et == 0) {
+          __threadfence();
+          if (atomicAdd(p.tile_cnt + g.tile, 1) == n - 1) {
+            p.tile_cnt[g.tile] = 0;
+            __threadfence();
+            st_release(p.tile_flags + g.tile, 1);
+          }
+        }
+      }
       if (et == 0) trace(p, span, 9);
     }
     if (MODE == 0 && p.amax_part) {                          // this CTA's max|h| per token, for spense_requant
       epi_sync();
       if (et < p.n_pad) p.amax_part[(size_t)span * p.n_pad + et] = et < p.M ? sc[et].z : 0.0f;
+    }
+    if (MODE == 1 && p.dep_flags && et == 0) {             // every load of this CTA has consumed its flags
+      __threadfence();
+      if (atomicAdd(p.dep_done, 1) == p.n_spans - 1) {
+        for (int t = 0; t < p.dep_tiles; ++t) const_cast<int*>(p.dep_flags)[t] = 0;
+        __threadfence();
+        *p.dep_done = 0;
+      }
     }
     if (et == 0) *epi_done_ptr = 1;
     if (p.trace && et == 0) { p.trace[(size_t)span * 16 + 10] = globaltimer(); p.trace[(size_t)span * 16 + 11] = (se - sb) | (seg << 16); p.trace[(size_t)span * 16 + 13] = globaltimer(); }

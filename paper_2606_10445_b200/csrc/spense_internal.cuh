@@ -38,6 +38,11 @@ constexpr int kBlobVersion = 1;
 constexpr int kMaxSpans = 160;
 constexpr int kFlagBytes = 4096;             // control words (128 B) + 2 flags per span
 constexpr int kAmaxBytes = 160 * 128 * 4;    // dynamic requant: max|h| per span and token (follows the flags)
+constexpr int kMaxGateTiles = 8192;          // I <= 2^20
+constexpr int kDepInts = kMaxGateTiles + 64; // gate_up tile-done flags (down polls them 16 at a time past the end)
+constexpr int kDepBytes = 2 * kDepInts * 4;  // flags, then the arrival counters of tiles finished by several CTAs
+constexpr int kWsFixedBytes = kFlagBytes + kAmaxBytes + kDepBytes;   // zeroed by spense_workspace_init; partials follow
+constexpr int kCtrlDepDone = 4;              // int index in the control words: down CTAs that are done with the tile flags
 
 struct BlobHeader {
   uint32_t magic;
@@ -107,9 +112,15 @@ struct GemmParams {
   int y_dtype;
   int ld_out;               // I (mode 0) or H (mode 1)
   int out_rows;             // valid output columns (I or H) for masking padded tiles
-  int* ws_ctrl;             // workspace control words: [0] epoch of the last finished launch, [1] finished-CTA count
+  int* ws_ctrl;             // workspace control words of this mode: [0] epoch of the last launch, [1] started-CTA count
   int* flags;               // workspace: 2 ints per span (first / last segment), hold the epoch of the dump
   float* partials;          // workspace: 2 slots per span of 2 * n_pad * 128 floats
+  // fine-grained gate_up -> down dependency inside spense_mlp (replaces the grid-wide wait of down's loads)
+  int* tile_flags;          // mode 0: set to 1 when all of Hq[:, 128 t .. 128 t + 128) is stored (nullptr: off)
+  int* tile_cnt;            // mode 0: arrivals at tiles that several CTAs finish (reduce-scatter)
+  const int* dep_flags;     // mode 1: the same flags, polled before the Hq tile of a stage is loaded (nullptr: PDL wait)
+  int* dep_done;            // mode 1: CTAs done; the last one clears the flags for the next layer
+  int dep_tiles;
   int pf_pace_ns;           // next-kernel L2 prefetch: nanoseconds per 32 KB chunk (0 = all at once)
   long long* trace;         // debug timeline (16 slots per span) or nullptr
   const uint8_t* next_base; // section the NEXT kernel of the stream will stream (L2 prefetch during our tail) or nullptr

@@ -70,7 +70,7 @@ struct Schedule {
 
 int slot_bytes_of(int n_pad) { return kSparseStageBytes + 2 * n_pad * 128; }
 int ring_stages_of(int n_pad) {
-  const int stages = (232448 - 1024 - 256 - 16 * n_pad) / slot_bytes_of(n_pad);
+  const int stages = (kSmemMax - 1024 - 256 - 20 * n_pad) / slot_bytes_of(n_pad);   // barriers + the two scale tables
   return stages > 8 ? 8 : stages;
 }
 std::mutex g_sched_mu;
@@ -191,6 +191,7 @@ uint32_t next_prefetch_bytes(const Schedule& sc, int k) {
   return n < sc.span_len[k] ? n : sc.span_len[k];
 }
 
+int g_fused = -1;               // spense_mlp as ONE persistent launch (SPENSE_FUSED / spense_debug_set_fused); -1 = read the environment
 long long* g_trace = nullptr;   // debug: set by spense_debug_set_trace (not part of the public ABI)
 
 void fill_common(GemmParams& p, const Schedule& sc, int M, int n_pad, void* d_ws) {
@@ -211,11 +212,19 @@ void fill_common(GemmParams& p, const Schedule& sc, int M, int n_pad, void* d_ws
   p.num_stages = ring_stages_of(n_pad);
   p.acc_stride = n_pad <= 32 ? 32 : (n_pad <= 64 ? 64 : 128);
   p.num_acc_bufs = n_pad <= 64 ? 2 : 1;
+  // separate launches run one after the other and share the control words, flags and partial slots (the
+  // partials then stay hot in L2); the fused kernel gives its down phase the second set (use_second_ws_half)
   uint8_t* ws = reinterpret_cast<uint8_t*>(d_ws);
-  const int mode = sc.mode;
-  p.ws_ctrl = reinterpret_cast<int*>(ws) + 2 * mode;
-  p.flags = reinterpret_cast<int*>(ws + 128 + mode * kMaxSpans * 2 * sizeof(int));
-  p.partials = reinterpret_cast<float*>(ws + kWsFixedBytes + (mode ? part_bytes_for(n_pad, kMaxSpans) : 0));
+  p.ws_ctrl = reinterpret_cast<int*>(ws);
+  p.flags = reinterpret_cast<int*>(ws + 128);
+  p.partials = reinterpret_cast<float*>(ws + kWsFixedBytes);
+}
+
+void use_second_ws_half(GemmParams& p, void* d_ws) {
+  uint8_t* ws = reinterpret_cast<uint8_t*>(d_ws);
+  p.ws_ctrl = reinterpret_cast<int*>(ws) + 2;
+  p.flags = reinterpret_cast<int*>(ws + 128 + kMaxSpans * 2 * sizeof(int));
+  p.partials = reinterpret_cast<float*>(ws + kWsFixedBytes + part_bytes_for(p.n_pad, kMaxSpans));
 }
 
 // L2 prefetch hint: while this launch runs its fix-up tail, pull what the next launch streams first.
@@ -232,36 +241,59 @@ void fill_next(GemmParams& p, const uint8_t* next_section, const Schedule& next)
   }
 }
 
+// parameter block + tensor map of one gate_up launch over tokens [m0, m0 + Mb)
+int gate_up_params(const Geometry& g, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_x, const float* d_sx,
+                   int m0, int Mb, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32, void* d_ws,
+                   bool dynamic, GemmParams& p, CUtensorMap& tm) {
+  const int n_pad = n_pad_of(Mb);
+  const Schedule& sc = get_schedule(0, g, n_pad, g_num_sms);
+  p = GemmParams{};
+  fill_common(p, sc, Mb, n_pad, d_ws);
+  p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.gate_up_off;
+  p.mode = 0;
+  p.num_tiles = g.gu_tiles; p.tiles_sparse = g.gu_tiles_sparse;
+  p.ns = g.gu_ns; p.nd = g.gu_nd; p.dense_k0 = 0;
+  p.s_act = d_sx + m0;
+  p.s_h = d_sh + (size_t)m0 * sh_stride; p.sh_stride = sh_stride;
+  p.w_scale0 = hdr.w_scale[0]; p.w_scale1 = hdr.w_scale[1];
+  p.hq = d_hq + (size_t)m0 * g.I;
+  p.h_f32 = d_h_f32 ? d_h_f32 + (size_t)m0 * g.I : nullptr;
+  p.amax_part = dynamic ? reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes) : nullptr;
+  p.ld_out = g.I; p.out_rows = g.I;
+  return make_tmap(&tm, d_x + (size_t)m0 * g.H, g.H, Mb, n_pad);
+}
+
+int down_params(const Geometry& g, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_hq, const float* d_sh,
+                int32_t sh_stride, int m0, int Mb, void* d_y, int32_t y_dtype, void* d_ws, GemmParams& p, CUtensorMap& tm) {
+  const size_t esz = y_dtype == SPENSE_F32 ? 4 : 2;
+  const int n_pad = n_pad_of(Mb);
+  const Schedule& sc = get_schedule(1, g, n_pad, g_num_sms);
+  p = GemmParams{};
+  fill_common(p, sc, Mb, n_pad, d_ws);
+  p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off;
+  p.mode = 1;
+  p.num_tiles = g.dn_tiles; p.tiles_sparse = 0;
+  p.ns = g.dn_ns; p.nd = g.dn_nd; p.dense_k0 = g.I_s;
+  p.s_act = d_sh + (size_t)m0 * sh_stride; p.sh_stride = sh_stride;
+  p.w_scale0 = hdr.w_scale[2]; p.w_scale1 = hdr.w_scale[2];
+  p.y = reinterpret_cast<uint8_t*>(d_y) + (size_t)m0 * g.H * esz;
+  p.y_dtype = y_dtype;
+  p.ld_out = g.H; p.out_rows = g.H;
+  return make_tmap(&tm, d_hq + (size_t)m0 * g.I, g.I, Mb, n_pad);
+}
+
 int gate_up_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_x,
                  const float* d_sx, int32_t M, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32,
-                 void* d_ws, bool pdl, bool down_follows, cudaStream_t stream, bool dynamic = false, bool gated = false) {
+                 void* d_ws, bool pdl, bool down_follows, cudaStream_t stream, bool dynamic = false) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
   for (int m0 = 0; m0 < M; m0 += 128) {
     const int Mb = (M - m0) < 128 ? (M - m0) : 128;
-    const int n_pad = n_pad_of(Mb);
-    const Schedule& sc = get_schedule(0, g, n_pad, g_num_sms);
-    GemmParams p = {};
-    fill_common(p, sc, Mb, n_pad, d_ws);
-    p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.gate_up_off;
-    p.mode = 0;
-    p.num_tiles = g.gu_tiles; p.tiles_sparse = g.gu_tiles_sparse;
-    p.ns = g.gu_ns; p.nd = g.gu_nd; p.dense_k0 = 0;
-    p.s_act = d_sx + m0;
-    p.s_h = d_sh + (size_t)m0 * sh_stride; p.sh_stride = sh_stride;
-    p.w_scale0 = hdr.w_scale[0]; p.w_scale1 = hdr.w_scale[1];
-    p.hq = d_hq + (size_t)m0 * g.I;
-    p.h_f32 = d_h_f32 ? d_h_f32 + (size_t)m0 * g.I : nullptr;
-    p.amax_part = dynamic ? reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes) : nullptr;
-    if (gated) {                                             // publish a flag per finished tile: down polls them
-      p.tile_flags = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes + kAmaxBytes);
-      p.tile_cnt = p.tile_flags + kDepInts;
-    }
-    p.ld_out = g.I; p.out_rows = g.I;
+    GemmParams p;
+    CUtensorMap tm;
+    int st = gate_up_params(g, hdr, d_blob, d_x, d_sx, m0, Mb, d_sh, sh_stride, d_hq, d_h_f32, d_ws, dynamic, p, tm);
+    if (st) return st;
     if (down_follows && m0 + 128 >= M)                       // the same layer's down projection streams next
       fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off, get_schedule(1, g, n_pad_of(M < 128 ? M : 128), g_num_sms));
-    CUtensorMap tm;
-    int st = make_tmap(&tm, d_x + (size_t)m0 * g.H, g.H, Mb, n_pad);
-    if (st) return st;
     st = launch_gemm(p, tm, pdl, stream);
     if (st) return st;
   }
@@ -270,38 +302,45 @@ int gate_up_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void*
 
 int down_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_hq,
               const float* d_sh, int32_t sh_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, bool pdl,
-              const void* d_next_blob, cudaStream_t stream, bool gated = false) {
+              const void* d_next_blob, cudaStream_t stream) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const size_t esz = y_dtype == SPENSE_F32 ? 4 : 2;
   for (int m0 = 0; m0 < M; m0 += 128) {
     const int Mb = (M - m0) < 128 ? (M - m0) : 128;
-    const int n_pad = n_pad_of(Mb);
-    const Schedule& sc = get_schedule(1, g, n_pad, g_num_sms);
-    GemmParams p = {};
-    fill_common(p, sc, Mb, n_pad, d_ws);
-    p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off;
-    p.mode = 1;
-    p.num_tiles = g.dn_tiles; p.tiles_sparse = 0;
-    p.ns = g.dn_ns; p.nd = g.dn_nd; p.dense_k0 = g.I_s;
-    p.s_act = d_sh + (size_t)m0 * sh_stride; p.sh_stride = sh_stride;
-    p.w_scale0 = hdr.w_scale[2]; p.w_scale1 = hdr.w_scale[2];
-    p.y = reinterpret_cast<uint8_t*>(d_y) + (size_t)m0 * g.H * esz;
-    p.y_dtype = y_dtype;
-    p.ld_out = g.H; p.out_rows = g.H;
-    if (gated) {                                             // wait per Hq tile instead of for the whole gate_up grid
-      p.dep_flags = reinterpret_cast<const int*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes + kAmaxBytes);
-      p.dep_done = reinterpret_cast<int*>(d_ws) + kCtrlDepDone;
-      p.dep_tiles = g.gu_tiles;
-    }
+    GemmParams p;
+    CUtensorMap tm;
+    int st = down_params(g, hdr, d_blob, d_hq, d_sh, sh_stride, m0, Mb, d_y, y_dtype, d_ws, p, tm);
+    if (st) return st;
     if (d_next_blob && m0 + 128 >= M)                        // the next layer's gate/up weights stream next
       fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + hdr.gate_up_off, get_schedule(0, g, n_pad_of(M < 128 ? M : 128), g_num_sms));
-    CUtensorMap tm;
-    int st = make_tmap(&tm, d_hq + (size_t)m0 * g.I, g.I, Mb, n_pad);
-    if (st) return st;
     st = launch_gemm(p, tm, pdl, stream);
     if (st) return st;
   }
   return SPENSE_OK;
+}
+
+// One token block: gate_up and down as ONE persistent launch (spense_mlp_kernel); down's Hq loads are gated per
+// 128-column tile by flags gate_up publishes, no grid-wide barrier in between.
+int mlp_fused_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_x,
+                   const float* d_sx, int32_t M, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32,
+                   void* d_y, int32_t y_dtype, void* d_ws, const void* d_next_blob, cudaStream_t stream) {
+  const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
+  GemmParams pg, pd;
+  CUtensorMap tx, th;
+  int st = gate_up_params(g, hdr, d_blob, d_x, d_sx, 0, M, d_sh, sh_stride, d_hq, d_h_f32, d_ws, false, pg, tx);
+  if (st) return st;
+  st = down_params(g, hdr, d_blob, d_hq, d_sh, sh_stride, 0, M, d_y, y_dtype, d_ws, pd, th);
+  if (st) return st;
+  use_second_ws_half(pd, d_ws);
+  int* dep = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes + kAmaxBytes);
+  pg.tile_flags = dep;
+  pg.tile_cnt = dep + kDepInts;
+  pd.dep_flags = dep;
+  pd.dep_done = reinterpret_cast<int*>(d_ws) + kCtrlDepDone;
+  pd.dep_tiles = g.gu_tiles;
+  { static const uint32_t pfb = (uint32_t)(env_double("SPENSE_PF_GATED_KB", 256.0) * 1024.0); pd.gated_pf_bytes = pfb; }
+  if (d_next_blob)                                           // the next layer's gate/up weights stream next
+    fill_next(pd, reinterpret_cast<const uint8_t*>(d_next_blob) + hdr.gate_up_off, get_schedule(0, g, n_pad_of(M), g_num_sms));
+  return launch_mlp(pg, tx, pd, th, stream);
 }
 
 int check_ws(const spense_shape_t* shape, int M, const void* d_ws, size_t ws_bytes) {
@@ -321,6 +360,10 @@ using namespace spense;
 extern "C" {
 
 int spense_version(void) { return 100 * 0 + 1; }
+
+// debug hook (undeclared in spense.h): run spense_mlp (M <= 128) as the fused single-launch kernel (1) or as two
+// PDL-chained launches (0, the default: measured 55.5 vs 57.4 us/layer at M=64)
+void spense_debug_set_fused(int on) { g_fused = on ? 1 : 0; }
 
 // debug hook (undeclared in spense.h): per-CTA globaltimer timeline, 16 int64 per span, of the next launches
 void spense_debug_set_trace(void* d_buf) { g_trace = reinterpret_cast<long long*>(d_buf); }
@@ -458,12 +501,13 @@ int spense_mlp(const spense_shape_t* shape, const void* d_blob, const uint8_t* d
   st = read_header(d_blob, shape, &hdr);
   if (st) return st;
   cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
-  // one token block: down starts on the tiles gate_up has finished (flags) instead of waiting for the whole grid
-  static const bool gate_knob = env_double("SPENSE_GATE", 1.0) != 0.0;
-  const bool gated = gate_knob && M <= 128;
-  st = gate_up_impl(shape, hdr, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq_scratch, d_h_f32, d_ws, true, true, s, false, gated);
+  if (g_fused < 0) g_fused = env_double("SPENSE_FUSED", 0.0) != 0.0 ? 1 : 0;
+  if (g_fused && M <= 128)
+    return mlp_fused_impl(shape, hdr, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq_scratch, d_h_f32, d_y, y_dtype, d_ws,
+                          d_next_blob, s);
+  st = gate_up_impl(shape, hdr, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq_scratch, d_h_f32, d_ws, true, true, s);
   if (st) return st;
-  return down_impl(shape, hdr, d_blob, d_hq_scratch, d_sh, sh_stride, M, d_y, y_dtype, d_ws, true, d_next_blob, s, gated);
+  return down_impl(shape, hdr, d_blob, d_hq_scratch, d_sh, sh_stride, M, d_y, y_dtype, d_ws, true, d_next_blob, s);
 }
 
 int spense_mlp_dyn(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx, int32_t M,

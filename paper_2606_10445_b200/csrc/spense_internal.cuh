@@ -36,10 +36,11 @@ constexpr int kBlobHeaderBytes = 1024;
 constexpr uint32_t kBlobMagic = 0x53504E53u;  // "SNPS"
 constexpr int kBlobVersion = 1;
 constexpr int kMaxSpans = 160;
+constexpr int kSmemMax = 232448;             // opt-in dynamic shared memory per CTA
 constexpr int kFlagBytes = 4096;             // control words (128 B) + 2 flags per span
 constexpr int kAmaxBytes = 160 * 128 * 4;    // dynamic requant: max|h| per span and token (follows the flags)
 constexpr int kMaxGateTiles = 8192;          // I <= 2^20
-constexpr int kDepInts = kMaxGateTiles + 64; // gate_up tile-done flags (down polls them 16 at a time past the end)
+constexpr int kDepInts = kMaxGateTiles + 1024;   // padded so that kWsFixedBytes is a multiple of 4 KB // gate_up tile-done flags (down polls them 16 at a time past the end)
 constexpr int kDepBytes = 2 * kDepInts * 4;  // flags, then the arrival counters of tiles finished by several CTAs
 constexpr int kWsFixedBytes = kFlagBytes + kAmaxBytes + kDepBytes;   // zeroed by spense_workspace_init; partials follow
 constexpr int kCtrlDepDone = 4;              // int index in the control words: down CTAs that are done with the tile flags
@@ -121,6 +122,7 @@ struct GemmParams {
   const int* dep_flags;     // mode 1: the same flags, polled before the Hq tile of a stage is loaded (nullptr: PDL wait)
   int* dep_done;            // mode 1: CTAs done; the last one clears the flags for the next layer
   int dep_tiles;
+  uint32_t gated_pf_bytes;  // mode 1 gated: L2 prefetch budget per span while waiting for the first Hq tiles
   int pf_pace_ns;           // next-kernel L2 prefetch: nanoseconds per 32 KB chunk (0 = all at once)
   long long* trace;         // debug timeline (16 slots per span) or nullptr
   const uint8_t* next_base; // section the NEXT kernel of the stream will stream (L2 prefetch during our tail) or nullptr
@@ -265,6 +267,8 @@ int launch_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8
                 const float* h_w_scale, const int32_t* d_perm, void* d_blob, const spense_canon_t* canon, void* d_ws,
                 int64_t* h_err_where, cudaStream_t stream);
 int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, bool pdl, cudaStream_t stream);
+int launch_mlp(const GemmParams& pg, const CUtensorMap& tmap_x, const GemmParams& pd, const CUtensorMap& tmap_hq,
+               cudaStream_t stream);
 int launch_requant_rows(const float* d_h, int rows, int cols, const float* d_amax_part, int n_part, int part_stride,
                         uint8_t* d_hq, float* d_sh, cudaStream_t stream);
 int launch_quantize(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out, float* d_scales,

@@ -163,3 +163,38 @@ def test_gemm_argument_errors(sp):
     with pytest.raises(sp.SpenseError) as e:
         sp.spense_gate_up(bad, cuda(c.x), cuda(c.s_x), cuda(torch.ones(1)), ws)
     assert e.value.code == "SPENSE_ERR_BAD_BLOB"
+
+
+@pytest.mark.parametrize("H,I,p,M", [(256, 1024, 0.25, 8), (1024, 4096, 0.25, 64), (640, 896, 0.43, 100), (768, 2048, 0.0, 128),
+                                     (1024, 2048, 1.0, 17), (5120, 5120, 0.25, 64)])
+def test_fused_single_launch_mlp_equals_two_launches(sp, H, I, p, M):
+    """spense_mlp as ONE persistent launch (gate_up and down phases in the same CTAs, Hq tiles gated by per-tile
+    flags, no grid barrier): bit-identical to the two PDL-chained launches, reproducible, flags left cleared."""
+    import ctypes
+    L = sp.lib()
+    L.spense_debug_set_fused.argtypes = [ctypes.c_int]
+    L.spense_debug_set_fused.restype = None
+    c = Case(H, I, p, M, seed=9000 + H + I + M)
+    pk = c.pack_gpu(sp)
+    s_h = c.default_s_h()
+    sh_dev = cuda(torch.from_numpy(s_h))
+    ws = sp.spense_workspace(pk, M)
+    y_ref = sp.spense_mlp(pk, cuda(c.x), cuda(c.s_x), sh_dev, ws)
+    torch.cuda.synchronize()
+    try:
+        L.spense_debug_set_fused(1)
+        hq = torch.zeros(M, I, dtype=torch.uint8, device="cuda")
+        ys = [sp.spense_mlp(pk, cuda(c.x), cuda(c.s_x), sh_dev, ws, hq_scratch=hq, next_layer=pk) for _ in range(4)]
+        yb = sp.spense_mlp(pk, cuda(c.x), cuda(c.s_x), sh_dev, ws, dtype=torch.bfloat16)
+        torch.cuda.synchronize()
+    finally:
+        L.spense_debug_set_fused(0)
+    for y in ys:
+        assert torch.equal(y, y_ref)
+    assert torch.equal(yb, y_ref.to(torch.bfloat16))
+    assert_down_parity(y_ref.cpu().numpy(), hq.cpu().numpy(), s_h, c.wd, c.L.w_scale[2], "fused down")
+    dep = ws[4096 + 160 * 128 * 4:4096 + 160 * 128 * 4 + 4 * (I // 128)].view(torch.int32)
+    assert int(dep.abs().sum()) == 0                       # the last CTA cleared the tile flags
+    y_after = sp.spense_mlp(pk, cuda(c.x), cuda(c.s_x), sh_dev, ws)      # the two-launch path still works on this workspace
+    torch.cuda.synchronize()
+    assert torch.equal(y_after, y_ref)

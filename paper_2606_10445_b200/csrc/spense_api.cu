@@ -4,6 +4,7 @@
 
 #include <cstdlib>
 #include <cstring>
+#include <deque>
 #include <mutex>
 #include <vector>
 
@@ -60,12 +61,13 @@ double env_double(const char* name, double dflt) {
 
 // ---- stream-K schedule: cut the stage sequence into n_spans spans of (nearly) equal bytes.
 struct Schedule {
-  int mode, H, I, I_d, n_pad, sms;
+  int mode, H, I, I_d, n_pad, sms, fused;
   int n_spans;
   int span_begin[kMaxSpans + 1];
   uint32_t span_off[kMaxSpans];   // byte offset of the span's first stage image inside its section
   uint32_t span_pre[kMaxSpans];   // bytes of the stages the producer issues before anything else (one ring)
   uint32_t span_len[kMaxSpans];   // bytes of the whole span
+  double span_cost[kMaxSpans];    // modelled cost of the span (fused: down spans are sized to equalise gate_up + down)
 };
 
 int slot_bytes_of(int n_pad) { return kSparseStageBytes + 2 * n_pad * 128; }
@@ -74,14 +76,19 @@ int ring_stages_of(int n_pad) {
   return stages > 8 ? 8 : stages;
 }
 std::mutex g_sched_mu;
-std::vector<Schedule> g_sched;
+std::deque<Schedule> g_sched;   // deque: references handed out stay valid
 
-const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms) {
+// fused = schedules of the single-launch MLP kernel (CTA b runs span n-1-b of gate_up AND of down):
+//   gate_up: span boundaries are nudged so that no tile is shared by more than two spans where a tile is not
+//            much longer than a span (a 3-way tile finishes last and every down span that reads it waits);
+//   down   : spans are sized so that gate_up cost + down cost is the same for every CTA.
+const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms, bool fused = false) {
+  const Schedule* gate = (fused && mode == 1) ? &get_schedule(0, g, n_pad, sms, true) : nullptr;
   std::lock_guard<std::mutex> lk(g_sched_mu);
   for (const Schedule& s : g_sched)
-    if (s.mode == mode && s.H == g.H && s.I == g.I && s.I_d == g.I_d && s.n_pad == n_pad && s.sms == sms) return s;
+    if (s.mode == mode && s.H == g.H && s.I == g.I && s.I_d == g.I_d && s.n_pad == n_pad && s.sms == sms && s.fused == (int)fused) return s;
   Schedule sc = {};
-  sc.mode = mode; sc.H = g.H; sc.I = g.I; sc.I_d = g.I_d; sc.n_pad = n_pad; sc.sms = sms;
+  sc.mode = mode; sc.H = g.H; sc.I = g.I; sc.I_d = g.I_d; sc.n_pad = n_pad; sc.sms = sms; sc.fused = fused;
   // cost of a stage.  Every CTA keeps the same number of ring slots in flight, so under HBM contention a
   // stage costs one slot latency plus its bytes: measured on B200 (profiles/) a 40 KB sparse stage takes
   // ~1.12x a 32 KB dense one => fixed part ~36 KB-equivalents; activation bytes come from L2 and weigh less.
@@ -103,11 +110,25 @@ const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms) {
   double sum = 0;
   for (double c : cost) sum += c;
   sc.n_spans = spans;
+  // cumulative share of the cost each span should end at: equal, or (fused down) what is left of an equal
+  // share of gate_up + down after the CTA's gate_up span
+  std::vector<double> cum(spans + 1, 0.0);
+  for (int i = 1; i <= spans; ++i) cum[i] = (double)i / spans;
+  if (gate && gate->n_spans == spans) {
+    double gsum = 0;
+    for (int i = 0; i < spans; ++i) gsum += gate->span_cost[i];
+    const double share = (gsum + sum) / spans;
+    double tot = 0;
+    std::vector<double> w(spans);
+    for (int i = 0; i < spans; ++i) { w[i] = share - gate->span_cost[i]; if (w[i] < 0.25 * sum / spans) w[i] = 0.25 * sum / spans; tot += w[i]; }
+    double run = 0;
+    for (int i = 0; i < spans; ++i) { run += w[i]; cum[i + 1] = run / tot; }
+  }
   double acc = 0;
   int s = 0;
   sc.span_begin[0] = 0;
   for (int i = 1; i < spans; ++i) {
-    const double target = sum * i / spans;
+    const double target = sum * cum[i];
     while (s < total && acc + 0.5 * cost[s] < target) acc += cost[s++];
     int b = s;
     if (b <= sc.span_begin[i - 1]) b = sc.span_begin[i - 1] + 1;     // every span owns >= 1 stage
@@ -116,6 +137,30 @@ const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms) {
     sc.span_begin[i] = b;
   }
   sc.span_begin[spans] = total;
+  if (fused && mode == 0) {
+    // a span lying strictly inside a tile makes the tile 3-way: stretch it to the nearer tile boundary
+    int tf = 0;
+    for (int t = 0; t < g.gu_tiles; ++t) {
+      const int per = t < g.gu_tiles_sparse ? g.gu_ns : g.gu_nd;
+      const int te = tf + per;
+      if (per < 2 * total / spans) {
+        for (int m = 1; m + 1 < spans; ++m) {
+          if (sc.span_begin[m] > tf && sc.span_begin[m + 1] < te) {
+            const int head = sc.span_begin[m] - tf, tail = te - sc.span_begin[m + 1];
+            if (head <= tail && sc.span_begin[m - 1] < tf) sc.span_begin[m] = tf;
+            else if (sc.span_begin[m + 2] > te) sc.span_begin[m + 1] = te;
+            else if (sc.span_begin[m - 1] < tf) sc.span_begin[m] = tf;
+          }
+        }
+      }
+      tf = te;
+    }
+  }
+  for (int i = 0; i < spans; ++i) {
+    double c = 0;
+    for (int k = sc.span_begin[i]; k < sc.span_begin[i + 1]; ++k) c += cost[k];
+    sc.span_cost[i] = c;
+  }
   // byte offsets: the blob stores the stage images in exactly this linear order
   std::vector<uint32_t> bytes(total);
   if (mode == 0) {
@@ -244,9 +289,9 @@ void fill_next(GemmParams& p, const uint8_t* next_section, const Schedule& next)
 // parameter block + tensor map of one gate_up launch over tokens [m0, m0 + Mb)
 int gate_up_params(const Geometry& g, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_x, const float* d_sx,
                    int m0, int Mb, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32, void* d_ws,
-                   bool dynamic, GemmParams& p, CUtensorMap& tm) {
+                   bool dynamic, GemmParams& p, CUtensorMap& tm, bool fused = false) {
   const int n_pad = n_pad_of(Mb);
-  const Schedule& sc = get_schedule(0, g, n_pad, g_num_sms);
+  const Schedule& sc = get_schedule(0, g, n_pad, g_num_sms, fused);
   p = GemmParams{};
   fill_common(p, sc, Mb, n_pad, d_ws);
   p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.gate_up_off;
@@ -264,10 +309,11 @@ int gate_up_params(const Geometry& g, const BlobHeader& hdr, const void* d_blob,
 }
 
 int down_params(const Geometry& g, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_hq, const float* d_sh,
-                int32_t sh_stride, int m0, int Mb, void* d_y, int32_t y_dtype, void* d_ws, GemmParams& p, CUtensorMap& tm) {
+                int32_t sh_stride, int m0, int Mb, void* d_y, int32_t y_dtype, void* d_ws, GemmParams& p, CUtensorMap& tm,
+                bool fused = false) {
   const size_t esz = y_dtype == SPENSE_F32 ? 4 : 2;
   const int n_pad = n_pad_of(Mb);
-  const Schedule& sc = get_schedule(1, g, n_pad, g_num_sms);
+  const Schedule& sc = get_schedule(1, g, n_pad, g_num_sms, fused);
   p = GemmParams{};
   fill_common(p, sc, Mb, n_pad, d_ws);
   p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off;
@@ -326,9 +372,9 @@ int mlp_fused_impl(const spense_shape_t* shape, const BlobHeader& hdr, const voi
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
   GemmParams pg, pd;
   CUtensorMap tx, th;
-  int st = gate_up_params(g, hdr, d_blob, d_x, d_sx, 0, M, d_sh, sh_stride, d_hq, d_h_f32, d_ws, false, pg, tx);
+  int st = gate_up_params(g, hdr, d_blob, d_x, d_sx, 0, M, d_sh, sh_stride, d_hq, d_h_f32, d_ws, false, pg, tx, true);
   if (st) return st;
-  st = down_params(g, hdr, d_blob, d_hq, d_sh, sh_stride, 0, M, d_y, y_dtype, d_ws, pd, th);
+  st = down_params(g, hdr, d_blob, d_hq, d_sh, sh_stride, 0, M, d_y, y_dtype, d_ws, pd, th, true);
   if (st) return st;
   use_second_ws_half(pd, d_ws);
   int* dep = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes + kAmaxBytes);
@@ -339,7 +385,7 @@ int mlp_fused_impl(const spense_shape_t* shape, const BlobHeader& hdr, const voi
   pd.dep_tiles = g.gu_tiles;
   { static const uint32_t pfb = (uint32_t)(env_double("SPENSE_PF_GATED_KB", 256.0) * 1024.0); pd.gated_pf_bytes = pfb; }
   if (d_next_blob)                                           // the next layer's gate/up weights stream next
-    fill_next(pd, reinterpret_cast<const uint8_t*>(d_next_blob) + hdr.gate_up_off, get_schedule(0, g, n_pad_of(M), g_num_sms));
+    fill_next(pd, reinterpret_cast<const uint8_t*>(d_next_blob) + hdr.gate_up_off, get_schedule(0, g, n_pad_of(M), g_num_sms, true));
   return launch_mlp(pg, tx, pd, th, stream);
 }
 

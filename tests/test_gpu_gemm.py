@@ -189,10 +189,16 @@ def test_fused_single_launch_mlp_equals_two_launches(sp, H, I, p, M):
         torch.cuda.synchronize()
     finally:
         L.spense_debug_set_fused(0)
-    for y in ys:
-        assert torch.equal(y, y_ref)
-    assert torch.equal(yb, y_ref.to(torch.bfloat16))
-    assert_down_parity(y_ref.cpu().numpy(), hq.cpu().numpy(), s_h, c.wd, c.L.w_scale[2], "fused down")
+    # the fused launch cuts the K ranges differently (its own schedule), so sums associate differently: equal to
+    # the two-launch result only within the tolerance, but bitwise reproducible and bf16 = RNE of its own fp32
+    for y in ys[1:]:
+        assert torch.equal(y, ys[0])
+    assert torch.equal(yb, ys[0].to(torch.bfloat16))
+    assert torch.allclose(ys[0], y_ref, rtol=1e-3, atol=1e-3 * float(y_ref.abs().max()))
+    r = c.oracle_gate_up(s_h)
+    diff = (hq.cpu().numpy() != r["hq"]).mean()
+    assert diff < 5e-3, diff
+    assert_down_parity(ys[0].cpu().numpy(), hq.cpu().numpy(), s_h, c.wd, c.L.w_scale[2], "fused down")
     dep = ws[4096 + 160 * 128 * 4:4096 + 160 * 128 * 4 + 4 * (I // 128)].view(torch.int32)
     assert int(dep.abs().sum()) == 0                       # the last CTA cleared the tile flags
     y_after = sp.spense_mlp(pk, cuda(c.x), cuda(c.s_x), sh_dev, ws)      # the two-launch path still works on this workspace

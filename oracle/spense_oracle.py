@@ -363,6 +363,39 @@ def mlp_dynamic(xq, s_x, wg_bytes, wu_bytes, wd_bytes, w_scale):
     return r
 
 
+# ---------------------------------------------------------------------------------------------
+# Dense-index selection: SpenseGPT (Eq. 5) is `spensegpt_dense_idx` above;
+# SpenseGPT+ (Eqs. 8-12) follows.  Readings: for W_down the index i is
+# a COLUMN, so Eq. 9 aggregates column i over the H rows and H_down is the Hessian of down's input h
+# (diag over the intermediate dimension); epsilon of Eq. 10 is an argument (the paper gives no value);
+# "approximately pN ... under the required alignment constraint" = exactly I_dense indices (a multiple
+# of 128); ties go to the lower index.
+# ---------------------------------------------------------------------------------------------
+def spensegpt_plus_scores(wgate, wup, wdown, hdiag_x, hdiag_h, eps=1e-8):
+    """s_i of Eq. 11 in float64.  wgate, wup [I, H]; wdown [H, I]; hdiag_x [H] = diag(X^T X) of the MLP
+    input (gate and up share it); hdiag_h [I] = diag of down's input Hessian."""
+    wg, wu, wd = (np.asarray(a, dtype=np.float64) for a in (wgate, wup, wdown))
+    rx = np.sqrt(np.asarray(hdiag_x, dtype=np.float64))
+    rh = np.sqrt(np.asarray(hdiag_h, dtype=np.float64))
+    I, H = wg.shape
+    s_gate = (np.abs(wg) * rx[None, :]).sum(axis=1) / H          # Eq. 9, rows of W_gate
+    s_up = (np.abs(wu) * rx[None, :]).sum(axis=1) / H            # Eq. 9, rows of W_up
+    s_down = (np.abs(wd) * rh[None, :]).sum(axis=0) / H          # Eq. 9, columns of W_down (K = its H rows)
+    norm = lambda v: v / (v.mean() + eps)                        # Eq. 10
+    return norm(s_gate) + norm(s_up) + norm(s_down)              # Eq. 11
+
+
+def topk_dense_idx(score, I_dense: int) -> np.ndarray:
+    """Eq. 12: the I_dense indices of largest score, ties to the lower index; returned ascending."""
+    score = np.asarray(score)
+    order = np.lexsort((np.arange(score.size), -score))          # by score descending, then index ascending
+    return np.sort(order[:I_dense]).astype(np.int32)
+
+
+def spensegpt_plus_dense_idx(wgate, wup, wdown, hdiag_x, hdiag_h, I_dense: int, eps=1e-8) -> np.ndarray:
+    return topk_dense_idx(spensegpt_plus_scores(wgate, wup, wdown, hdiag_x, hdiag_h, eps), I_dense)
+
+
 # tolerance companions (O6): north_star bound |gpu - oracle| <= 2e-3 * sum|a*w| + 1e-5
 def tol_gemm(abs_sum):
     return 2e-3 * np.asarray(abs_sum) + 1e-5

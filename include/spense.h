@@ -164,6 +164,21 @@ int spense_mlp_host(const spense_shape_t* shape, const void* d_blob, const uint8
                     uint8_t* d_x, float* d_scales, uint8_t* d_hq_scratch, void* d_y, void* d_ws,
                     size_t ws_bytes, const void* d_next_blob, spense_stream_t stream);
 
+/* spense_select_dense -- SpenseGPT+ dense-index selection (Eqs. 8-12):
+ *   s^gate_i = 1/H sum_j |Wg[i,j]| sqrt(Hx[j]),  s^up likewise,  s^down_i = sqrt(Hh[i]) / H sum_n |Wd[n,i]|   (Eq. 9)
+ *   s_i = sum over the three projections of s^mlp_i / (mean(s^mlp) + eps)                            (Eqs. 10, 11)
+ *   D = the shape->I_dense indices of largest s_i, ties to the lower index                           (Eq. 12)
+ * Inputs (device, fp32, original index order): d_wgate, d_wup [I, H]; d_wdown [H, I]; d_hdiag_x [H] = diag(X^T X)
+ * of the MLP input; d_hdiag_h [I] = diag of the Hessian of down's input.  eps >= 0 (the paper gives no value).
+ * Outputs (device): d_score [I] (nullable); d_dense_idx [I_dense] ascending; d_perm [I] new -> old, the stable
+ * partition spense_pack expects (sparse indices ascending, then D ascending).
+ * Every reduction runs in a fixed order: scores and selection are bitwise reproducible.  No synchronisation.
+ * Workspace: spense_select_workspace_size bytes, 16-byte aligned.                                         */
+int spense_select_workspace_size(const spense_shape_t* shape, size_t* bytes);
+int spense_select_dense(const spense_shape_t* shape, const float* d_wgate, const float* d_wup, const float* d_wdown,
+                        const float* d_hdiag_x, const float* d_hdiag_h, float eps, float* d_score,
+                        int32_t* d_dense_idx, int32_t* d_perm, void* d_ws, size_t ws_bytes, spense_stream_t stream);
+
 /* spense_quantize_e4m3 -- helper (reading Q5): scale = amax / 448 (1 if amax == 0), per tensor or
  * per row; out = E4M3_rne_sat(in / scale) with an IEEE fp32 division.  d_scales: 1 or rows floats.
  * d_ws needs 4 bytes * (rows + 1). Bit-exact against the oracle.                                  */

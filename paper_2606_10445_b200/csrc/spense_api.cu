@@ -613,6 +613,34 @@ int spense_mlp_host(const spense_shape_t* shape, const void* d_blob, const uint8
   return cudaStreamSynchronize(s) == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;
 }
 
+int spense_select_workspace_size(const spense_shape_t* shape, size_t* bytes) {
+  int st = check_shape(shape);
+  if (st) return st;
+  if (!bytes) return SPENSE_ERR_ARG;
+  // three score vectors, the combined score, the ranks, W_down's column sums per 64-row chunk
+  *bytes = (size_t)shape->I * (5 + (size_t)(shape->H + 63) / 64) * sizeof(float) + 128;
+  return SPENSE_OK;
+}
+
+int spense_select_dense(const spense_shape_t* shape, const float* d_wgate, const float* d_wup, const float* d_wdown,
+                        const float* d_hdiag_x, const float* d_hdiag_h, float eps, float* d_score, int32_t* d_dense_idx,
+                        int32_t* d_perm, void* d_ws, size_t ws_bytes, spense_stream_t stream) {
+  int st = check_shape(shape);
+  if (st) return st;
+  if (!d_wgate || !d_wup || !d_wdown || !d_hdiag_x || !d_hdiag_h || !d_perm || !d_ws || (shape->I_dense > 0 && !d_dense_idx) ||
+      !(eps >= 0.0f))
+    return SPENSE_ERR_ARG;
+  if (!aligned(d_wgate, 16) || !aligned(d_wup, 16) || !aligned(d_wdown, 16) || !aligned(d_hdiag_x, 16) || !aligned(d_ws, 16))
+    return SPENSE_ERR_ALIGN;
+  size_t need = 0;
+  spense_select_workspace_size(shape, &need);
+  if (ws_bytes < need) return SPENSE_ERR_BUFFER_TOO_SMALL;
+  st = check_device();
+  if (st) return st;
+  return launch_select(shape, d_wgate, d_wup, d_wdown, d_hdiag_x, d_hdiag_h, eps, d_score, d_dense_idx, d_perm, d_ws,
+                       reinterpret_cast<cudaStream_t>(stream));
+}
+
 int spense_quantize_e4m3(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out, float* d_scales,
                          void* d_ws, size_t ws_bytes, spense_stream_t stream) {
   if (!d_in || !d_out || !d_scales || !d_ws || rows < 1 || cols < 1 || (mode != SPENSE_PER_TENSOR && mode != SPENSE_PER_ROW))

@@ -23,7 +23,8 @@ STATUS = {0: "SPENSE_OK", -1: "SPENSE_ERR_ARG", -2: "SPENSE_ERR_ALIGN", -3: "SPE
 
 EXPORTS = ["spense_version", "spense_strerror", "spense_perm_from_dense_idx", "spense_pack_sizes", "spense_pack",
            "spense_workspace_size", "spense_workspace_init", "spense_gate_up", "spense_down", "spense_mlp",
-           "spense_mlp_dyn", "spense_mlp_host", "spense_quantize_e4m3"]
+           "spense_mlp_dyn", "spense_mlp_host", "spense_quantize_e4m3", "spense_select_workspace_size",
+           "spense_select_dense"]
 
 
 class SpenseError(RuntimeError):
@@ -74,6 +75,9 @@ def lib() -> ctypes.CDLL:
         L.spense_mlp_host.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_int32, c_void_p, c_int32,
                                       c_void_p, c_int32, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_size_t,
                                       c_void_p, c_void_p]
+        L.spense_select_workspace_size.argtypes = [POINTER(Shape), POINTER(c_size_t)]
+        L.spense_select_dense.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_float, c_void_p,
+                                          c_void_p, c_void_p, c_void_p, c_size_t, c_void_p]
         L.spense_quantize_e4m3.argtypes = [c_void_p, c_int64, c_int64, c_int32, c_void_p, c_void_p, c_void_p,
                                            c_size_t, c_void_p]
         for name in EXPORTS:
@@ -253,3 +257,22 @@ def spense_quantize_e4m3(x: torch.Tensor, mode: int):
     ws = torch.empty((rows + 1) * 4, dtype=torch.uint8, device=x.device)
     _check(lib().spense_quantize_e4m3(_ptr(x), rows, cols, mode, _ptr(out), _ptr(scales), _ptr(ws), ws.numel(), _stream()))
     return out, scales
+
+
+def spense_select_dense(wgate, wup, wdown, hdiag_x, hdiag_h, I_dense: int, eps: float = 1e-8):
+    """SpenseGPT+ dense-index selection on fp32 weights (CUDA).  Returns (score [I], dense_idx [I_dense], perm [I])."""
+    for t in (wgate, wup, wdown, hdiag_x, hdiag_h):
+        _dev(t, torch.float32)
+    I, H = wgate.shape
+    dev = wgate.device
+    shape = Shape(H, I, I_dense)
+    b = c_size_t()
+    _check(lib().spense_select_workspace_size(ctypes.byref(shape), ctypes.byref(b)))
+    ws = torch.empty(b.value, dtype=torch.uint8, device=dev)
+    score = torch.empty(I, dtype=torch.float32, device=dev)
+    dense_idx = torch.empty(I_dense, dtype=torch.int32, device=dev)
+    perm = torch.empty(I, dtype=torch.int32, device=dev)
+    _check(lib().spense_select_dense(ctypes.byref(shape), _ptr(wgate), _ptr(wup), _ptr(wdown), _ptr(hdiag_x), _ptr(hdiag_h),
+                                     c_float(eps), _ptr(score), _ptr(dense_idx) if I_dense else None, _ptr(perm), _ptr(ws),
+                                     b.value, _stream()))
+    return score, dense_idx, perm

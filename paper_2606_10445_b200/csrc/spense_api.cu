@@ -61,7 +61,7 @@ double env_double(const char* name, double dflt) {
 
 // ---- stream-K schedule: cut the stage sequence into n_spans spans of (nearly) equal bytes.
 struct Schedule {
-  int mode, H, I, I_d, n_pad, sms, fused;
+  int mode, H, I, I_d, n_pad, sms, fused, nb;
   int n_spans;
   int span_begin[kMaxSpans + 1];
   uint32_t span_off[kMaxSpans];   // byte offset of the span's first stage image inside its section
@@ -82,24 +82,25 @@ std::deque<Schedule> g_sched;   // deque: references handed out stay valid
 //   gate_up: span boundaries are nudged so that no tile is shared by more than two spans where a tile is not
 //            much longer than a span (a 3-way tile finishes last and every down span that reads it waits);
 //   down   : spans are sized so that gate_up cost + down cost is the same for every CTA.
-const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms, bool fused = false) {
+const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms, bool fused = false, int nb = 1) {
   const Schedule* gate = (fused && mode == 1) ? &get_schedule(0, g, n_pad, sms, true) : nullptr;
   std::lock_guard<std::mutex> lk(g_sched_mu);
   for (const Schedule& s : g_sched)
-    if (s.mode == mode && s.H == g.H && s.I == g.I && s.I_d == g.I_d && s.n_pad == n_pad && s.sms == sms && s.fused == (int)fused) return s;
+    if (s.mode == mode && s.H == g.H && s.I == g.I && s.I_d == g.I_d && s.n_pad == n_pad && s.sms == sms && s.fused == (int)fused && s.nb == nb) return s;
   Schedule sc = {};
-  sc.mode = mode; sc.H = g.H; sc.I = g.I; sc.I_d = g.I_d; sc.n_pad = n_pad; sc.sms = sms; sc.fused = fused;
+  sc.mode = mode; sc.H = g.H; sc.I = g.I; sc.I_d = g.I_d; sc.n_pad = n_pad; sc.sms = sms; sc.fused = fused; sc.nb = nb;
   // cost of a stage.  Every CTA keeps the same number of ring slots in flight, so under HBM contention a
   // stage costs one slot latency plus its bytes: measured on B200 (profiles/) a 40 KB sparse stage takes
   // ~1.12x a 32 KB dense one => fixed part ~36 KB-equivalents; activation bytes come from L2 and weigh less.
   static const double fixed = env_double("SPENSE_SCHED_FIXED", 36864.0), gamma = env_double("SPENSE_SCHED_GAMMA", 0.25);
   const double cs = fixed + kSparseStageBytes + gamma * 2.0 * n_pad * 128, cd = fixed + kDenseStageBytes + gamma * 1.0 * n_pad * 128;
+  // nb token blocks: every tile appears nb times in a row (virtual tiles), the stage sequence is nb times longer
   std::vector<double> cost;
   if (mode == 0) {
-    cost.insert(cost.end(), (size_t)g.gu_tiles_sparse * g.gu_ns, cs);
-    cost.insert(cost.end(), (size_t)(g.gu_tiles - g.gu_tiles_sparse) * g.gu_nd, cd);
+    cost.insert(cost.end(), (size_t)g.gu_tiles_sparse * nb * g.gu_ns, cs);
+    cost.insert(cost.end(), (size_t)(g.gu_tiles - g.gu_tiles_sparse) * nb * g.gu_nd, cd);
   } else {
-    for (int t = 0; t < g.dn_tiles; ++t) {
+    for (int t = 0; t < g.dn_tiles * nb; ++t) {
       cost.insert(cost.end(), (size_t)g.dn_ns, cs);
       cost.insert(cost.end(), (size_t)g.dn_nd, cd);
     }
@@ -164,7 +165,7 @@ const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms, bo
   // byte offsets: the blob stores the stage images in exactly this linear order
   std::vector<uint32_t> bytes(total);
   if (mode == 0) {
-    for (int i = 0; i < total; ++i) bytes[i] = i < g.gu_tiles_sparse * g.gu_ns ? kSparseStageBytes : kDenseStageBytes;
+    for (int i = 0; i < total; ++i) bytes[i] = i < g.gu_tiles_sparse * nb * g.gu_ns ? kSparseStageBytes : kDenseStageBytes;
   } else {
     const int per = g.dn_ns + g.dn_nd;
     for (int i = 0; i < total; ++i) bytes[i] = (i % per) < g.dn_ns ? kSparseStageBytes : kDenseStageBytes;
@@ -249,8 +250,9 @@ void fill_common(GemmParams& p, const Schedule& sc, int M, int n_pad, void* d_ws
     const uint32_t from = next_prefetch_bytes(sc, i);
     const uint32_t left = sc.span_len[i] - from;
     p.self_off[i] = from - sc.span_pre[i];
-    p.self_len[i] = self_want < left ? self_want : left;
+    p.self_len[i] = sc.nb > 1 ? 0 : (self_want < left ? self_want : left);   // virtual tiles: a span is not one byte range
   }
+  p.nb = sc.nb;
   p.M = M;
   p.n_pad = n_pad;
   p.slot_bytes = slot_bytes_of(n_pad);
@@ -290,8 +292,8 @@ void fill_next(GemmParams& p, const uint8_t* next_section, const Schedule& next)
 int gate_up_params(const Geometry& g, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_x, const float* d_sx,
                    int m0, int Mb, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32, void* d_ws,
                    bool dynamic, GemmParams& p, CUtensorMap& tm, bool fused = false) {
-  const int n_pad = n_pad_of(Mb);
-  const Schedule& sc = get_schedule(0, g, n_pad, g_num_sms, fused);
+  const int n_pad = n_pad_of(Mb);                            // > 128 tokens: blocks of 128 inside one launch
+  const Schedule& sc = get_schedule(0, g, n_pad, g_num_sms, fused, (Mb + 127) / 128);
   p = GemmParams{};
   fill_common(p, sc, Mb, n_pad, d_ws);
   p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.gate_up_off;
@@ -313,7 +315,7 @@ int down_params(const Geometry& g, const BlobHeader& hdr, const void* d_blob, co
                 bool fused = false) {
   const size_t esz = y_dtype == SPENSE_F32 ? 4 : 2;
   const int n_pad = n_pad_of(Mb);
-  const Schedule& sc = get_schedule(1, g, n_pad, g_num_sms, fused);
+  const Schedule& sc = get_schedule(1, g, n_pad, g_num_sms, fused, (Mb + 127) / 128);
   p = GemmParams{};
   fill_common(p, sc, Mb, n_pad, d_ws);
   p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off;
@@ -332,36 +334,26 @@ int gate_up_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void*
                  const float* d_sx, int32_t M, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32,
                  void* d_ws, bool pdl, bool down_follows, cudaStream_t stream, bool dynamic = false) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  for (int m0 = 0; m0 < M; m0 += 128) {
-    const int Mb = (M - m0) < 128 ? (M - m0) : 128;
-    GemmParams p;
-    CUtensorMap tm;
-    int st = gate_up_params(g, hdr, d_blob, d_x, d_sx, m0, Mb, d_sh, sh_stride, d_hq, d_h_f32, d_ws, dynamic, p, tm);
-    if (st) return st;
-    if (down_follows && m0 + 128 >= M)                       // the same layer's down projection streams next
-      fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off, get_schedule(1, g, n_pad_of(M < 128 ? M : 128), g_num_sms));
-    st = launch_gemm(p, tm, pdl, stream);
-    if (st) return st;
-  }
-  return SPENSE_OK;
+  GemmParams p;
+  CUtensorMap tm;
+  int st = gate_up_params(g, hdr, d_blob, d_x, d_sx, 0, M, d_sh, sh_stride, d_hq, d_h_f32, d_ws, dynamic, p, tm);
+  if (st) return st;
+  if (down_follows && M <= 128)                              // the same layer's down projection streams next
+    fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off, get_schedule(1, g, n_pad_of(M), g_num_sms));
+  return launch_gemm(p, tm, pdl, stream);
 }
 
 int down_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_hq,
               const float* d_sh, int32_t sh_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, bool pdl,
               const void* d_next_blob, cudaStream_t stream) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  for (int m0 = 0; m0 < M; m0 += 128) {
-    const int Mb = (M - m0) < 128 ? (M - m0) : 128;
-    GemmParams p;
-    CUtensorMap tm;
-    int st = down_params(g, hdr, d_blob, d_hq, d_sh, sh_stride, m0, Mb, d_y, y_dtype, d_ws, p, tm);
-    if (st) return st;
-    if (d_next_blob && m0 + 128 >= M)                        // the next layer's gate/up weights stream next
-      fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + hdr.gate_up_off, get_schedule(0, g, n_pad_of(M < 128 ? M : 128), g_num_sms));
-    st = launch_gemm(p, tm, pdl, stream);
-    if (st) return st;
-  }
-  return SPENSE_OK;
+  GemmParams p;
+  CUtensorMap tm;
+  int st = down_params(g, hdr, d_blob, d_hq, d_sh, sh_stride, 0, M, d_y, y_dtype, d_ws, p, tm);
+  if (st) return st;
+  if (d_next_blob && M <= 128)                               // the next layer's gate/up weights stream next
+    fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + hdr.gate_up_off, get_schedule(0, g, n_pad_of(M), g_num_sms));
+  return launch_gemm(p, tm, pdl, stream);
 }
 
 // One token block: gate_up and down as ONE persistent launch (spense_mlp_kernel); down's Hq loads are gated per

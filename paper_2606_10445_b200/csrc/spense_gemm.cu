@@ -47,52 +47,64 @@ namespace spense {
 
 namespace {
 
-// Position in the linear stage sequence: pair tile, stage inside the tile, stages of the tile.
+// Position in the linear stage sequence: pair tile, token block, stage inside the tile, stages of the tile.
+// With nb token blocks the sequence visits "virtual tiles" v = tile * nb + blk.
 struct Cursor {
-  int tile, j, ns, nd, first;   // first = linear index of the tile's first stage
+  int tile, blk, j, ns, nd, first;   // first = linear index of the (virtual) tile's first stage
 };
+
+// byte offset of stage j of pair tile `tile` inside the section (the blob stores every tile once)
+template <int MODE>
+__device__ __forceinline__ size_t stage_byte_offset(const GemmParams& p, int tile, int j) {
+  if (MODE == 0) {
+    if (tile < p.tiles_sparse) return ((size_t)tile * p.ns + j) * kSparseStageBytes;
+    return (size_t)p.tiles_sparse * p.ns * kSparseStageBytes + ((size_t)(tile - p.tiles_sparse) * p.nd + j) * kDenseStageBytes;
+  }
+  const size_t base = (size_t)tile * ((size_t)p.ns * kSparseStageBytes + (size_t)p.nd * kDenseStageBytes);
+  return base + (j < p.ns ? (size_t)j * kSparseStageBytes
+                          : (size_t)p.ns * kSparseStageBytes + (size_t)(j - p.ns) * kDenseStageBytes);
+}
 
 // The only place with integer divisions (one copy per mode, called once per role and phase).
 template <int MODE>
 __device__ __noinline__ Cursor cursor_at(const GemmParams& p, int s, unsigned long long* byte_off) {
   Cursor c;
-  size_t off;
+  int v;                                                   // virtual tile
   if (MODE == 0) {
-    const int sparse_total = p.tiles_sparse * p.ns;
+    const int sparse_total = p.tiles_sparse * p.nb * p.ns;
     if (s < sparse_total) {
-      c.tile = s / p.ns;
-      c.first = c.tile * p.ns;
+      v = s / p.ns;
+      c.first = v * p.ns;
       c.ns = p.ns; c.nd = 0;
-      off = (size_t)s * kSparseStageBytes;
     } else {
       const int td = (s - sparse_total) / p.nd;
-      c.tile = p.tiles_sparse + td;
+      v = p.tiles_sparse * p.nb + td;
       c.first = sparse_total + td * p.nd;
       c.ns = 0; c.nd = p.nd;
-      off = (size_t)sparse_total * kSparseStageBytes + (size_t)(s - sparse_total) * kDenseStageBytes;
     }
-    c.j = s - c.first;
   } else {
     const int per = p.ns + p.nd;
-    c.tile = s / per;
-    c.first = c.tile * per;
+    v = s / per;
+    c.first = v * per;
     c.ns = p.ns; c.nd = p.nd;
-    c.j = s - c.first;
-    off = (size_t)c.tile * ((size_t)p.ns * kSparseStageBytes + (size_t)p.nd * kDenseStageBytes);
-    off += c.j < c.ns ? (size_t)c.j * kSparseStageBytes
-                      : (size_t)c.ns * kSparseStageBytes + (size_t)(c.j - c.ns) * kDenseStageBytes;
   }
-  *byte_off = off;
+  c.tile = p.nb == 1 ? v : v / p.nb;
+  c.blk = p.nb == 1 ? 0 : v - c.tile * p.nb;
+  c.j = s - c.first;
+  *byte_off = stage_byte_offset<MODE>(p, c.tile, c.j);
   return c;
 }
 
 template <int MODE>
 __device__ __forceinline__ void next_tile(const GemmParams& p, Cursor& c) {
   c.first += c.ns + c.nd;
-  ++c.tile;
   c.j = 0;
-  if (MODE == 0) {
-    if (c.tile < p.tiles_sparse) { c.ns = p.ns; c.nd = 0; } else { c.ns = 0; c.nd = p.nd; }
+  if (++c.blk == p.nb) {
+    c.blk = 0;
+    ++c.tile;
+    if (MODE == 0) {
+      if (c.tile < p.tiles_sparse) { c.ns = p.ns; c.nd = 0; } else { c.ns = 0; c.nd = p.nd; }
+    }
   }
 }
 
@@ -106,11 +118,13 @@ __device__ __forceinline__ float silu_mul(float g, float u) {
 }
 
 // a / b from the correctly rounded reciprocal r = RN(1/b) and two FMAs (Markstein): branch-free and
-// correctly rounded wherever the quotient is a normal number -- all the E4M3 cast after it can see.
+// correctly rounded wherever the quotient is a normal number -- all the E4M3 cast after it can see
+// (a zero quotient keeps the sign IEEE division gives it: h = -0 must encode as 0x80 like the oracle's).
 __device__ __forceinline__ float div_by(float a, float b, float r) {
   const float q0 = a * r;
   const float rem = fmaf(-q0, b, a);
-  return fmaf(rem, r, q0);
+  const float q = fmaf(rem, r, q0);
+  return q == 0.0f ? q0 : q;                               // (+0) + (-0) = +0 would lose the sign of a zero quotient
 }
 
 // fp32 -> E4M3 (saturating, round to nearest even); cvt.rn.satfinite.e4m3x2.f32 packs two values
@@ -172,15 +186,16 @@ struct Ctx {
 
 // One output element (token m, weight row r of pair tile `tile`): scales, GLU + requant, or the Y store.
 // MODE 0: sc = float4 per token column {s_x*s_gate, s_x*s_up, s_h, RN(1/s_h)}; MODE 1: sc = float per token s_h*s_down.
+// m = token column inside the block (index of the scale table), m_out = token (output row).
 template <int MODE, bool DYN>
-__device__ __forceinline__ void finish(const GemmParams& p, const void* sc, int tile, int r, int m, float f0, float f1) {
+__device__ __forceinline__ void finish(const GemmParams& p, const void* sc, int tile, int r, int m, int m_out, float f0, float f1) {
   if (MODE == 0) {
     const float4* sc4 = reinterpret_cast<const float4*>(sc);
     const float4 k = sc4[m];
     const float g = f0 * k.x;
     const float u = f1 * k.y;
     const float h = silu_mul(g, u);
-    const size_t o = (size_t)m * p.ld_out + tile * 128 + r;
+    const size_t o = (size_t)m_out * p.ld_out + tile * 128 + r;
     if (DYN) {
       // dynamic requant: keep h in fp32 and track max|h| per token; the scale does not
       // exist yet, the row requant kernel turns h into Hq once every tile is done.  Called warp-uniformly in m.
@@ -196,7 +211,7 @@ __device__ __forceinline__ void finish(const GemmParams& p, const void* sc, int 
     const float kx = reinterpret_cast<const float*>(sc)[m];
     const int out_row = tile * 256 + r;
     const float y0 = f0 * kx, y1 = f1 * kx;
-    const size_t o = (size_t)m * p.ld_out + out_row;
+    const size_t o = (size_t)m_out * p.ld_out + out_row;
     const bool second = out_row + 128 < p.out_rows;
     if (p.y_dtype == SPENSE_F32) {
       float* y = reinterpret_cast<float*>(p.y);
@@ -211,7 +226,7 @@ __device__ __forceinline__ void finish(const GemmParams& p, const void* sc, int 
 }
 
 // A tile shared by more than two spans [a, b]: reduced at the end of the phase (reduce-scatter).
-struct Group { int a, b, tile, first; };
+struct Group { int a, b, tile, first, blk; };
 
 // ===================== producer (one thread) =====================
 // Streams the stages of span `span` of one phase through the ring.  `it` counts the stages of the whole
@@ -225,7 +240,8 @@ __device__ __forceinline__ void producer_phase(const GemmParams& p, const CUtens
   const int S = cx.S;
   const int sb = p.span_begin[span];
   const int n = p.span_begin[span + 1] - sb;
-  const uint64_t pol_w = policy_evict_first();
+  // one token block: a weight byte is used once (evict first); several: the next block re-reads the tile from L2
+  const uint64_t pol_w = p.nb == 1 ? policy_evict_first() : policy_evict_normal();
   const uint64_t pol_a = policy_evict_last();
   unsigned long long off;
   Cursor c = cursor_at<MODE>(p, sb, &off);
@@ -235,7 +251,7 @@ __device__ __forceinline__ void producer_phase(const GemmParams& p, const CUtens
   int dep_lo = 0, dep_hi = 0;                              // Hq tiles [dep_lo, dep_hi) are known to be stored
 
   auto tiles_ready = [&](uint32_t inf) -> bool {           // at most one poll (16 flags) per call
-    const int k0 = (int)(inf & 0x7FFFFFFFu);
+    const int k0 = (int)(inf & 0x1FFFFFu);
     const int t_first = k0 >> 7;
     int t_last = (k0 + ((inf >> 31) ? 255 : 127)) >> 7;
     if (t_last >= p.dep_tiles) t_last = p.dep_tiles - 1;   // a padded K stage reads no further than the last tile
@@ -261,9 +277,10 @@ __device__ __forceinline__ void producer_phase(const GemmParams& p, const CUtens
   };
   auto load_b = [&](int slot, uint32_t inf) {
     const uint32_t b_dst = cx.smem_base + (uint32_t)slot * cx.slot_bytes + kSparseStageBytes;
-    const int k0 = (int)(inf & 0x7FFFFFFFu);
-    tma_load_2d(b_dst, tmap, k0, 0, cx.full_bar(slot), pol_a);
-    if (inf >> 31) tma_load_2d(b_dst + cx.b_tile_bytes, tmap, k0 + 128, 0, cx.full_bar(slot), pol_a);
+    const int k0 = (int)(inf & 0x1FFFFFu);                  // K coordinate | token block << 21 | sparse << 31
+    const int row0 = (int)((inf >> 21) & 0x3FFu) * 128;
+    tma_load_2d(b_dst, tmap, k0, row0, cx.full_bar(slot), pol_a);
+    if (inf >> 31) tma_load_2d(b_dst + cx.b_tile_bytes, tmap, k0 + 128, row0, cx.full_bar(slot), pol_a);
   };
 
   int w = 0;                                               // weight stages issued (of this phase)
@@ -277,7 +294,8 @@ __device__ __forceinline__ void producer_phase(const GemmParams& p, const CUtens
     // everything that does not need the slot is computed before the wait: a freed slot is refilled at once
     const bool sp = c.j < c.ns;
     const uint32_t wb = sp ? (uint32_t)kSparseStageBytes : (uint32_t)kDenseStageBytes;
-    const uint32_t inf = (uint32_t)(sp ? c.j * kSparseStageK : p.dense_k0 + (c.j - c.ns) * kDenseStageK) | (sp ? 0x80000000u : 0u);
+    const uint32_t inf = (uint32_t)(sp ? c.j * kSparseStageK : p.dense_k0 + (c.j - c.ns) * kDenseStageK) | ((uint32_t)c.blk << 21) |
+                         (sp ? 0x80000000u : 0u);
     const uint32_t tx = wb + (sp ? 2u : 1u) * cx.b_tile_bytes;
     const uint32_t fb = cx.full_bar(w_slot);
     const uint32_t dst = cx.smem_base + (uint32_t)w_slot * cx.slot_bytes;
@@ -295,7 +313,10 @@ __device__ __forceinline__ void producer_phase(const GemmParams& p, const CUtens
         if (k == ((it0 + w) & 7)) info[k] = inf;
     }
     src += wb;
-    if (++c.j == c.ns + c.nd) next_tile<MODE>(p, c);
+    if (++c.j == c.ns + c.nd) {
+      next_tile<MODE>(p, c);
+      if (p.nb > 1) src = p.section + stage_byte_offset<MODE>(p, c.tile, 0);   // same tile again for the next token block
+    }
     ++w;
     if (++w_slot == S) { w_slot = 0; ++w_round; }
     return true;
@@ -428,6 +449,20 @@ __device__ __forceinline__ void mma_phase(const GemmParams& p, const Ctx& cx, in
   trace(p, span, 4);
 }
 
+// scale tables of the token block that starts at token m_base (Mb tokens)
+__device__ __forceinline__ void epilogue_tables(const GemmParams& p, const Ctx& cx, int et, int m_base, int Mb) {
+  if (et < p.n_pad) {
+    const int m = m_base + (et < Mb ? et : Mb - 1);
+    if (p.mode == 0) {
+      const float sx = __ldg(p.s_act + m);
+      const float sh = p.amax_part ? 1.0f : __ldg(p.s_h + (size_t)m * p.sh_stride);
+      cx.sc0()[et] = make_float4(sx * p.w_scale0, sx * p.w_scale1, p.amax_part ? 0.0f : sh, __frcp_rn(sh));   // dynamic: .z = running max|h| bits
+    } else {
+      cx.sc1(p.n_pad)[et] = __ldg(p.s_act + (size_t)m * p.sh_stride) * p.w_scale0;
+    }
+  }
+}
+
 // ===================== epilogue (16 warps) =====================
 // warp & 3 selects the TMEM lane quadrant, (warp - 4) >> 2 the quarter of the token columns.
 // ring_free: this is the last phase of the kernel, so once the CTA's last accumulator is complete the stage
@@ -441,10 +476,8 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
   const int q = warp & 3;
   const int row = q * 32 + lane;                           // accumulator lane = weight row inside the tile
   const int et = threadIdx.x - 128;                        // 0..511
-  const int cols_used = min(p.n_pad, (p.M + 7) & ~7);      // token columns holding real tokens, rounded to the TMEM load width
   const int cols_per = (((p.n_pad + 3) >> 2) + 7) & ~7;    // columns per warp: a quarter, rounded to the TMEM load width
   const int c_begin = ((warp - 4) >> 2) * cols_per;
-  const int c_end = min(c_begin + cols_per, cols_used);
   const float* stg = reinterpret_cast<const float*>(cx.smem_gen);   // the stage ring doubles as partial staging
   const size_t part_floats = (size_t)2 * p.n_pad * 128;    // one partial: [mat][col][row]
   const int sb = p.span_begin[span], se = p.span_begin[span + 1];
@@ -460,6 +493,16 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
     const int seg_end = min(se, tile_end);
     const int buf = seg % p.num_acc_bufs;
     const uint32_t use = (uint32_t)(seg / p.num_acc_bufs);
+    // the token block of this (virtual) tile
+    const int m_base = cur.blk * 128;
+    const int Mb = p.nb == 1 ? p.M : min(128, p.M - m_base);
+    const int cols_used = min(p.n_pad, (Mb + 7) & ~7);     // token columns holding real tokens, rounded to the TMEM load width
+    const int c_end = min(c_begin + cols_per, cols_used);
+    if (p.nb > 1) {                                        // this block's scales (the table holds one block)
+      epi_sync();
+      epilogue_tables(p, cx, et, m_base, Mb);
+      epi_sync();
+    }
     // spans [a, b] that hold stages of this tile
     int a = span, b = span;
     while (p.span_begin[a] > cur.first) --a;
@@ -540,7 +583,7 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
         }
 #pragma unroll
         for (int i = 0; i < 8; ++i)
-          if (c + i < p.M) finish<MODE, DYN>(p, sc, cur.tile, row, c + i, f0[i], f1[i]);
+          if (c + i < Mb) finish<MODE, DYN>(p, sc, cur.tile, row, c + i, m_base + c + i, f0[i], f1[i]);
       }
       tc_fence_before();
       mbar_arrive(cx.acce_bar(buf));
@@ -570,6 +613,7 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
       if (et == 0) st_release(p.flags + span * 2 + which, epoch);   // ... one gpu-scope release publishes them (cumulativity)
       if (b > a + 1) {
         groups[n_groups].a = a; groups[n_groups].b = b; groups[n_groups].tile = cur.tile; groups[n_groups].first = cur.first;
+        groups[n_groups].blk = cur.blk;
         ++n_groups;
       }
     }
@@ -585,8 +629,15 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
     const Group g = groups[gi];
     const int n = g.b - g.a + 1;
     const int j = span - g.a;
-    const int m0 = (int)(((long long)j * p.M) / n), m1 = (int)(((long long)(j + 1) * p.M) / n);
+    const int m_base = g.blk * 128;
+    const int Mb = p.nb == 1 ? p.M : min(128, p.M - m_base);
+    const int m0 = (int)(((long long)j * Mb) / n), m1 = (int)(((long long)(j + 1) * Mb) / n);
     const int rrow = et & 127;
+    if (p.nb > 1) {                                        // the scale table holds one block: this group's
+      epi_sync();
+      epilogue_tables(p, cx, et, m_base, Mb);
+      epi_sync();
+    }
     if (m1 > m0 && ring_free) {
       // all MMAs of this CTA are complete: the stage ring stages the partial slices
       int cc_max = (int)(cx.ring_bytes / ((uint32_t)n * 1024u));
@@ -621,7 +672,7 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
             f0 += stg[((size_t)(2 * qi) * cc + c) * 128 + rrow];
             f1 += stg[((size_t)(2 * qi + 1) * cc + c) * 128 + rrow];
           }
-          finish<MODE, DYN>(p, sc, g.tile, rrow, mc + c, f0, f1);
+          finish<MODE, DYN>(p, sc, g.tile, rrow, mc + c, m_base + mc + c, f0, f1);
         }
       }
     } else if (m1 > m0) {
@@ -650,7 +701,7 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
           for (int k = 0; k < 4; ++k)
             if (q0 + k < n) { f0 += v0[k]; f1 += v1[k]; }
         }
-        finish<MODE, DYN>(p, sc, g.tile, rrow, c, f0, f1);
+        finish<MODE, DYN>(p, sc, g.tile, rrow, c, m_base + c, f0, f1);
       }
     }
     if (FUSED0) {                                          // the last of the n reducers publishes the tile
@@ -695,19 +746,6 @@ __device__ __forceinline__ Ctx prologue(const GemmParams& p, uint8_t* smem_raw) 
   // let the next kernel of the stream start its own prologue (it waits for us in pdl_wait)
   pdl_launch_dependents();
   return cx;
-}
-
-__device__ __forceinline__ void epilogue_tables(const GemmParams& p, const Ctx& cx, int et) {
-  if (et < p.n_pad) {
-    const int m = et < p.M ? et : p.M - 1;
-    if (p.mode == 0) {
-      const float sx = __ldg(p.s_act + m);
-      const float sh = p.amax_part ? 1.0f : __ldg(p.s_h + (size_t)m * p.sh_stride);
-      cx.sc0()[et] = make_float4(sx * p.w_scale0, sx * p.w_scale1, p.amax_part ? 0.0f : sh, __frcp_rn(sh));   // dynamic: .z = running max|h| bits
-    } else {
-      cx.sc1(p.n_pad)[et] = __ldg(p.s_act + (size_t)m * p.sh_stride) * p.w_scale0;
-    }
-  }
 }
 
 // Epoch of a launch = epoch word + 1.  Every CTA reads the word BEFORE it counts itself; the CTA that counts
@@ -760,7 +798,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
     const int et = threadIdx.x - 128;
     // scales, the workspace and the epoch word may be produced / still in use by the previous kernel
     pdl_wait();
-    epilogue_tables(p, cx, et);
+    epilogue_tables(p, cx, et, 0, p.nb == 1 ? p.M : min(128, p.M));
     if (et == kEpiThreads - 1) take_epoch(p.ws_ctrl, nullptr, p.n_spans, cx.epoch_ptr());
     epi_sync();
     const int epoch = cx.epoch_ptr()[0];                   // flag value of THIS launch (never equals a stale flag)
@@ -825,8 +863,8 @@ spense_mlp_kernel(const __grid_constant__ GemmParams pg, const __grid_constant__
   } else if (warp >= 4) {
     const int et = threadIdx.x - 128;
     pdl_wait();
-    epilogue_tables(pg, cx, et);
-    epilogue_tables(pd, cx, et);
+    epilogue_tables(pg, cx, et, 0, pg.M);
+    epilogue_tables(pd, cx, et, 0, pd.M);
     if (et == kEpiThreads - 1) take_epoch(pg.ws_ctrl, pd.ws_ctrl, (int)gridDim.x, cx.epoch_ptr());
     epi_sync();
     const int epoch_g = cx.epoch_ptr()[0], epoch_d = cx.epoch_ptr()[1];

@@ -99,7 +99,10 @@ struct GemmParams {
   int ns, nd;               // mode 0: stages of a sparse tile / of a dense tile; mode 1: per tile both
   int dense_k0;             // K byte offset of the first dense stage in the B operand (mode 1: I_s)
   int n_spans;
-  int M, n_pad;             // tokens in this launch, padded to 16
+  int M, n_pad;             // tokens in this launch; token columns of one MMA (M padded to 16, at most 128)
+  int nb;                   // token blocks of 128 (1 for M <= 128).  nb > 1: every pair tile is visited nb times in a
+                            // row ("virtual tile" = tile * nb + block), so a weight tile is streamed from HBM once
+                            // and re-read from L2 for the following blocks
   int num_stages, slot_bytes, acc_stride, num_acc_bufs;
   // epilogue
   const float* s_act;       // mode 0: s_x [M]; mode 1: s_h (stride sh_stride)

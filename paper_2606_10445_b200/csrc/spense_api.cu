@@ -48,7 +48,6 @@ int check_shape(const spense_shape_t* s) {
 
 bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
-int n_pad_of(int M) { int n = (M + 15) / 16 * 16; return n > 128 ? 128 : n; }
 
 size_t part_bytes_for(int n_pad, int spans) { return (size_t)spans * 2 * 2 * n_pad * 128 * sizeof(float); }
 // control words, flags, max|h| table, tile flags | partials of gate_up | partials of down (they may run concurrently)
@@ -58,6 +57,13 @@ double env_double(const char* name, double dflt) {
   const char* v = std::getenv(name);
   return v ? std::atof(v) : dflt;
 }
+
+// Token columns of one MMA.  Up to 128 tokens: M padded to 16.  More: blocks of block_tokens() inside one launch
+// (virtual tiles).  128 by default; 96 would allow two accumulator buffers (2 x 2 x 96 columns + 32 of metadata
+// fit the 512 TMEM columns) but needs more passes over the weights: measured 141.6 vs 115.4 us/layer at M=256.
+int block_tokens() { static const int b = (int)env_double("SPENSE_BLOCK_TOKENS", 128.0); return b == 96 ? 96 : 128; }
+int n_pad_of(int M) { return M > 128 ? block_tokens() : (M + 15) / 16 * 16; }
+int nb_of(int M) { return M > 128 ? (M + block_tokens() - 1) / block_tokens() : 1; }
 
 // ---- stream-K schedule: cut the stage sequence into n_spans spans of (nearly) equal bytes.
 struct Schedule {
@@ -257,8 +263,8 @@ void fill_common(GemmParams& p, const Schedule& sc, int M, int n_pad, void* d_ws
   p.n_pad = n_pad;
   p.slot_bytes = slot_bytes_of(n_pad);
   p.num_stages = ring_stages_of(n_pad);
-  p.acc_stride = n_pad <= 32 ? 32 : (n_pad <= 64 ? 64 : 128);
-  p.num_acc_bufs = n_pad <= 64 ? 2 : 1;
+  p.acc_stride = n_pad <= 32 ? 32 : (n_pad <= 64 ? 64 : (n_pad <= 96 ? 96 : 128));
+  p.num_acc_bufs = n_pad <= 96 ? 2 : 1;                     // 2 buffers x 2 accumulators x 96 columns + metadata at 480
   // separate launches run one after the other and share the control words, flags and partial slots (the
   // partials then stay hot in L2); the fused kernel gives its down phase the second set (use_second_ws_half)
   uint8_t* ws = reinterpret_cast<uint8_t*>(d_ws);
@@ -293,7 +299,7 @@ int gate_up_params(const Geometry& g, const BlobHeader& hdr, const void* d_blob,
                    int m0, int Mb, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32, void* d_ws,
                    bool dynamic, GemmParams& p, CUtensorMap& tm, bool fused = false) {
   const int n_pad = n_pad_of(Mb);                            // > 128 tokens: blocks of 128 inside one launch
-  const Schedule& sc = get_schedule(0, g, n_pad, g_num_sms, fused, (Mb + 127) / 128);
+  const Schedule& sc = get_schedule(0, g, n_pad, g_num_sms, fused, nb_of(Mb));
   p = GemmParams{};
   fill_common(p, sc, Mb, n_pad, d_ws);
   p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.gate_up_off;
@@ -315,7 +321,7 @@ int down_params(const Geometry& g, const BlobHeader& hdr, const void* d_blob, co
                 bool fused = false) {
   const size_t esz = y_dtype == SPENSE_F32 ? 4 : 2;
   const int n_pad = n_pad_of(Mb);
-  const Schedule& sc = get_schedule(1, g, n_pad, g_num_sms, fused, (Mb + 127) / 128);
+  const Schedule& sc = get_schedule(1, g, n_pad, g_num_sms, fused, nb_of(Mb));
   p = GemmParams{};
   fill_common(p, sc, Mb, n_pad, d_ws);
   p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off;
@@ -469,7 +475,7 @@ int spense_workspace_size(const spense_shape_t* shape, int32_t M, size_t* bytes)
   int st = check_shape(shape);
   if (st) return st;
   if (M < 1 || !bytes) return SPENSE_ERR_ARG;
-  *bytes = ws_bytes_for(n_pad_of(M), kMaxSpans);
+  *bytes = ws_bytes_for(M > 128 ? 128 : n_pad_of(M), kMaxSpans);
   return SPENSE_OK;
 }
 

@@ -278,7 +278,7 @@ __device__ __forceinline__ void producer_phase(const GemmParams& p, const CUtens
   auto load_b = [&](int slot, uint32_t inf) {
     const uint32_t b_dst = cx.smem_base + (uint32_t)slot * cx.slot_bytes + kSparseStageBytes;
     const int k0 = (int)(inf & 0x1FFFFFu);                  // K coordinate | token block << 21 | sparse << 31
-    const int row0 = (int)((inf >> 21) & 0x3FFu) * 128;
+    const int row0 = (int)((inf >> 21) & 0x3FFu) * p.n_pad;  // token blocks hold n_pad tokens
     tma_load_2d(b_dst, tmap, k0, row0, cx.full_bar(slot), pol_a);
     if (inf >> 31) tma_load_2d(b_dst + cx.b_tile_bytes, tmap, k0 + 128, row0, cx.full_bar(slot), pol_a);
   };
@@ -494,8 +494,8 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
     const int buf = seg % p.num_acc_bufs;
     const uint32_t use = (uint32_t)(seg / p.num_acc_bufs);
     // the token block of this (virtual) tile
-    const int m_base = cur.blk * 128;
-    const int Mb = p.nb == 1 ? p.M : min(128, p.M - m_base);
+    const int m_base = cur.blk * p.n_pad;
+    const int Mb = p.nb == 1 ? p.M : min(p.n_pad, p.M - m_base);
     const int cols_used = min(p.n_pad, (Mb + 7) & ~7);     // token columns holding real tokens, rounded to the TMEM load width
     const int c_end = min(c_begin + cols_per, cols_used);
     if (p.nb > 1) {                                        // this block's scales (the table holds one block)
@@ -629,8 +629,8 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
     const Group g = groups[gi];
     const int n = g.b - g.a + 1;
     const int j = span - g.a;
-    const int m_base = g.blk * 128;
-    const int Mb = p.nb == 1 ? p.M : min(128, p.M - m_base);
+    const int m_base = g.blk * p.n_pad;
+    const int Mb = p.nb == 1 ? p.M : min(p.n_pad, p.M - m_base);
     const int m0 = (int)(((long long)j * Mb) / n), m1 = (int)(((long long)(j + 1) * Mb) / n);
     const int rrow = et & 127;
     if (p.nb > 1) {                                        // the scale table holds one block: this group's
@@ -798,7 +798,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
     const int et = threadIdx.x - 128;
     // scales, the workspace and the epoch word may be produced / still in use by the previous kernel
     pdl_wait();
-    epilogue_tables(p, cx, et, 0, p.nb == 1 ? p.M : min(128, p.M));
+    epilogue_tables(p, cx, et, 0, p.nb == 1 ? p.M : min(p.n_pad, p.M));
     if (et == kEpiThreads - 1) take_epoch(p.ws_ctrl, nullptr, p.n_spans, cx.epoch_ptr());
     epi_sync();
     const int epoch = cx.epoch_ptr()[0];                   // flag value of THIS launch (never equals a stale flag)

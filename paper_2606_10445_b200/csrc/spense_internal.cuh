@@ -100,7 +100,7 @@ struct GemmParams {
   int dense_k0;             // K byte offset of the first dense stage in the B operand (mode 1: I_s)
   int n_spans;
   int M, n_pad;             // tokens in this launch; token columns of one MMA (M padded to 16, at most 128)
-  int nb;                   // token blocks of 128 (1 for M <= 128).  nb > 1: every pair tile is visited nb times in a
+  int nb;                   // token blocks of n_pad tokens (1 for M <= 128).  nb > 1: every pair tile is visited nb times in a
                             // row ("virtual tile" = tile * nb + block), so a weight tile is streamed from HBM once
                             // and re-read from L2 for the following blocks
   int num_stages, slot_bytes, acc_stride, num_acc_bufs;

@@ -409,6 +409,28 @@ int spense_version(void) { return 100 * 0 + 1; }
 // PDL-chained launches (0, the default: measured 55.5 vs 57.4 us/layer at M=64)
 void spense_debug_set_fused(int on) { g_fused = on ? 1 : 0; }
 
+// debug hook (undeclared in spense.h; host only, no device needed): the stream-K schedule the library would use
+// for (shape, M, mode 0 gate_up / 1 down, fused, sms).  Writes n_spans + 1 span boundaries (linear stage indices)
+// into out_span_begin (room for 161 ints) and returns n_spans, or a negative status.  out_info[0..3] = total
+// stages, token blocks, token columns per MMA, ring slots.
+int spense_debug_schedule(const spense_shape_t* shape, int32_t M, int32_t mode, int32_t fused, int32_t sms,
+                          int32_t* out_span_begin, int32_t* out_info) {
+  int st = check_shape(shape);
+  if (st) return st;
+  if (M < 1 || (mode != 0 && mode != 1) || sms < 1 || !out_span_begin) return SPENSE_ERR_ARG;
+  const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
+  const int n_pad = n_pad_of(M), nb = nb_of(M);
+  const Schedule& sc = get_schedule(mode, g, n_pad, sms, fused != 0 && nb == 1, nb);
+  for (int i = 0; i <= sc.n_spans; ++i) out_span_begin[i] = sc.span_begin[i];
+  if (out_info) {
+    out_info[0] = sc.span_begin[sc.n_spans];
+    out_info[1] = nb;
+    out_info[2] = n_pad;
+    out_info[3] = ring_stages_of(n_pad);
+  }
+  return sc.n_spans;
+}
+
 // debug hook (undeclared in spense.h): per-CTA globaltimer timeline, 16 int64 per span, of the next launches
 void spense_debug_set_trace(void* d_buf) { g_trace = reinterpret_cast<long long*>(d_buf); }
 

@@ -28,7 +28,7 @@ H, I, P_DENSE = 5120, 25600, 0.25
 LAYERS = 8
 # dram__bytes_read.sum + dram__bytes_write.sum of the two spense_gemm_kernel launches of one layer at
 # M=64, from the committed ncu capture (profiles/); per layer, like `achieved`.
-NCU_TRAFFIC_BYTES_PER_LAYER = 285426304   # r01_traffic_app_replay_M64.csv: 16 launches = 8 layers, read + write
+NCU_TRAFFIC_BYTES_PER_LAYER = 286584960   # r01_traffic_app_replay_M64.csv: 16 launches = 8 layers, read + write
 
 
 def algorithmic_bytes(M: int, I_d: int) -> int:

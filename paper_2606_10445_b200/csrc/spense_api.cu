@@ -417,7 +417,7 @@ int spense_debug_schedule(const spense_shape_t* shape, int32_t M, int32_t mode, 
                           int32_t* out_span_begin, int32_t* out_info) {
   int st = check_shape(shape);
   if (st) return st;
-  if (M < 1 || (mode != 0 && mode != 1) || sms < 1 || !out_span_begin) return SPENSE_ERR_ARG;
+  if (M < 1 || M > kMaxTokens || (mode != 0 && mode != 1) || sms < 1 || !out_span_begin) return SPENSE_ERR_ARG;
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
   const int n_pad = n_pad_of(M), nb = nb_of(M);
   const Schedule& sc = get_schedule(mode, g, n_pad, sms, fused != 0 && nb == 1, nb);
@@ -496,7 +496,7 @@ int spense_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8
 int spense_workspace_size(const spense_shape_t* shape, int32_t M, size_t* bytes) {
   int st = check_shape(shape);
   if (st) return st;
-  if (M < 1 || !bytes) return SPENSE_ERR_ARG;
+  if (M < 1 || M > kMaxTokens || !bytes) return SPENSE_ERR_ARG;
   *bytes = ws_bytes_for(M > 128 ? 128 : n_pad_of(M), kMaxSpans);
   return SPENSE_OK;
 }
@@ -512,7 +512,7 @@ int spense_gate_up(const spense_shape_t* shape, const void* d_blob, const uint8_
                    spense_stream_t stream) {
   int st = check_shape(shape);
   if (st) return st;
-  if (!d_blob || !d_x || !d_sx || !d_sh || !d_hq || M < 1 || (sh_stride != 0 && sh_stride != 1)) return SPENSE_ERR_ARG;
+  if (!d_blob || !d_x || !d_sx || !d_sh || !d_hq || M < 1 || M > kMaxTokens || (sh_stride != 0 && sh_stride != 1)) return SPENSE_ERR_ARG;
   if (!aligned(d_blob, 128) || !aligned(d_x, 128) || !aligned(d_hq, 16) || !aligned(d_sx, 4) || !aligned(d_sh, 4) ||
       (d_h_f32 && !aligned(d_h_f32, 16)))
     return SPENSE_ERR_ALIGN;
@@ -532,7 +532,7 @@ int spense_down(const spense_shape_t* shape, const void* d_blob, const uint8_t* 
                 spense_stream_t stream) {
   int st = check_shape(shape);
   if (st) return st;
-  if (!d_blob || !d_hq || !d_sh || !d_y || M < 1 || (sh_stride != 0 && sh_stride != 1) ||
+  if (!d_blob || !d_hq || !d_sh || !d_y || M < 1 || M > kMaxTokens || (sh_stride != 0 && sh_stride != 1) ||
       (y_dtype != SPENSE_F32 && y_dtype != SPENSE_BF16))
     return SPENSE_ERR_ARG;
   if (!aligned(d_blob, 128) || !aligned(d_hq, 128) || !aligned(d_y, 16) || !aligned(d_sh, 4) || !aligned(d_next_blob, 128))
@@ -553,7 +553,7 @@ int spense_mlp(const spense_shape_t* shape, const void* d_blob, const uint8_t* d
                void* d_ws, size_t ws_bytes, const void* d_next_blob, spense_stream_t stream) {
   int st = check_shape(shape);
   if (st) return st;
-  if (!d_blob || !d_x || !d_sx || !d_sh || !d_hq_scratch || !d_y || M < 1 || (sh_stride != 0 && sh_stride != 1) ||
+  if (!d_blob || !d_x || !d_sx || !d_sh || !d_hq_scratch || !d_y || M < 1 || M > kMaxTokens || (sh_stride != 0 && sh_stride != 1) ||
       (y_dtype != SPENSE_F32 && y_dtype != SPENSE_BF16))
     return SPENSE_ERR_ARG;
   if (!aligned(d_blob, 128) || !aligned(d_x, 128) || !aligned(d_hq_scratch, 128) || !aligned(d_y, 16) ||
@@ -581,7 +581,7 @@ int spense_mlp_dyn(const spense_shape_t* shape, const void* d_blob, const uint8_
                    size_t ws_bytes, const void* d_next_blob, spense_stream_t stream) {
   int st = check_shape(shape);
   if (st) return st;
-  if (!d_blob || !d_x || !d_sx || !d_sh_out || !d_hq_scratch || !d_h_scratch || !d_y || M < 1 ||
+  if (!d_blob || !d_x || !d_sx || !d_sh_out || !d_hq_scratch || !d_h_scratch || !d_y || M < 1 || M > kMaxTokens ||
       (y_dtype != SPENSE_F32 && y_dtype != SPENSE_BF16))
     return SPENSE_ERR_ARG;
   if (!aligned(d_blob, 128) || !aligned(d_x, 128) || !aligned(d_hq_scratch, 128) || !aligned(d_y, 16) ||
@@ -617,7 +617,7 @@ int spense_mlp_host(const spense_shape_t* shape, const void* d_blob, const uint8
                     spense_stream_t stream) {
   int st = check_shape(shape);
   if (st) return st;
-  if (!h_x || !h_sx || !h_sh || !h_y || !d_x || !d_scales || M < 1 || (sh_stride != 0 && sh_stride != 1) ||
+  if (!h_x || !h_sx || !h_sh || !h_y || !d_x || !d_scales || M < 1 || M > kMaxTokens || (sh_stride != 0 && sh_stride != 1) ||
       (y_dtype != SPENSE_F32 && y_dtype != SPENSE_BF16))
     return SPENSE_ERR_ARG;
   cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);

@@ -36,6 +36,7 @@ constexpr int kBlobHeaderBytes = 1024;
 constexpr uint32_t kBlobMagic = 0x53504E53u;  // "SNPS"
 constexpr int kBlobVersion = 1;
 constexpr int kMaxSpans = 160;
+constexpr int kMaxTokens = 96 * 1023;        // token blocks are numbered in 10 bits of a stage descriptor
 constexpr int kSmemMax = 232448;             // opt-in dynamic shared memory per CTA
 constexpr int kFlagBytes = 4096;             // control words (128 B) + 2 flags per span
 constexpr int kAmaxBytes = 160 * 128 * 4;    // dynamic requant: max|h| per span and token (follows the flags)

@@ -89,3 +89,35 @@ def test_full_size_mlp_parity_in_bench_launch_configuration(sp, layer, M):
         torch.cuda.synchronize()
         assert torch.equal(hq2, hq), "graph replay: Hq differs from the eager launch"
         assert torch.equal(y16, y32.to(torch.bfloat16)), "graph replay: bf16 y is not the RNE rounding of the fp32 y"
+
+
+@pytest.mark.parametrize("M", [256, 2048])
+def test_full_size_many_tokens_sampled_rows(sp, layer, M):
+    """BASELINE.json configs[1] at M=256 and configs[4] (prefill-shaped, M=2048): ONE launch per GEMM over
+    128-token blocks.  Token rows are independent, so the oracle computes a sample of them one by one (first and
+    last row of blocks, a ragged spread in between) and every column of those rows is compared."""
+    L, pk = layer["L"], layer["pk"]
+    x, s_x = si.make_activations(M, H, 3000 + M)
+    rows = np.unique(np.concatenate([[0, 1, 127, 128, 129, 255, M - 129, M - 128, M - 1],
+                                     np.random.default_rng(M).integers(0, M, 23)])).astype(np.int64)
+    xs, sxs = x.numpy()[rows], s_x.numpy()[rows]
+    r1 = o.gate_up(xs, sxs, layer["wg"], layer["wu"], L.w_scale[0], L.w_scale[1], 1.0)
+    s_h = np.full(M, 0.05, np.float32)
+    s_h[rows] = o.requant_scale_from_h(r1["h"])
+    r = o.gate_up(xs, sxs, layer["wg"], layer["wu"], L.w_scale[0], L.w_scale[1], s_h[rows])
+    ws = sp.spense_workspace(pk, M)
+    xd, sxd, shd = cuda(x), cuda(s_x), cuda(torch.from_numpy(s_h))
+    h = torch.full((M, I), float("nan"), dtype=torch.float32, device="cuda")
+    hq = sp.spense_gate_up(pk, xd, sxd, shd, ws, h_f32=h)
+    y = sp.spense_down(pk, hq, shd, ws)
+    y2 = sp.spense_mlp(pk, xd, sxd, shd, ws)
+    torch.cuda.synchronize()
+    assert not torch.isnan(h).any()
+    h_s, hq_s, y_s = h.cpu().numpy()[rows], hq.cpu().numpy()[rows], y.cpu().numpy()[rows]
+    frac = assert_gate_up_parity(r, h_s, hq_s, s_h[rows], f"gate_up M={M} sampled rows")
+    assert frac < 5e-3
+    assert_down_parity(y_s, hq_s, s_h[rows], layer["wd"], L.w_scale[2], f"down M={M} sampled rows")
+    assert torch.equal(y, y2)
+    # every row: Hq is the E4M3 cast of the kernel's own h (the decision is taken in fp32 on both sides)
+    own = o.e4m3_encode((h.cpu().numpy() / s_h[:, None]).astype(np.float32))
+    assert np.array_equal(own, hq.cpu().numpy())

@@ -6,8 +6,9 @@
 //                     (tcgen05.mma).  Epilogue: scales -> SiLU(g)*u (Eq. 4) -> E4M3.
 //   MODE 1  down    : input-split.  Pair tile = 2 x 128 rows of W_down; the K loop runs
 //                     the sparse stages and then the dense stages INTO THE SAME TMEM ACCUMULATOR.
-// and three kernels built from them: spense_gemm_kernel<0>, spense_gemm_kernel<1> (one phase each) and
-// spense_mlp_kernel (gate_up then down in ONE persistent launch, see below).
+// and the kernels built from them: spense_gemm_kernel<MODE, DYN> (one phase; DYN = gate_up that keeps h in fp32
+// and tracks max|h| per token for the dynamic requant) and spense_mlp_kernel (gate_up then down in ONE persistent
+// launch, see below).
 //
 // Swap-AB: only the A operand of tcgen05.mma.sp can be sparse, so weights are A (MMA-M = 128 weight
 // rows) and tokens are B (MMA-N = padded token count); the accumulator holds Y^T [128 rows x tokens].
@@ -21,6 +22,9 @@
 //                epilogue -- nothing but the flag check sits on the owner's critical path;
 //   * > 2 spans: every span finishes late, so all dump, and the n spans reduce M/n token columns each
 //                (reduce-scatter) instead of one owner reducing n partials serially.
+// More than 128 tokens: token blocks of 128 inside the same launch.  The stage sequence then visits "virtual
+// tiles" (pair tile x token block, block index fastest): a weight tile is streamed from HBM for the first block
+// and re-read from L2 for the others; spans, fix-ups and flags work unchanged on the longer sequence.
 // Flags hold the epoch of the launch (a device-side counter in the workspace), so nothing has to be
 // reset between launches and CUDA-graph replays see fresh values.
 // Span i runs on CTA n_spans-1-i.  CTAs of one launch wait for each other, so all n_spans <= #SM CTAs

@@ -48,41 +48,60 @@ def read_peaks():
 
 
 class ClockSampler:
+    """nvidia-smi polled every 20 ms in the background; every line is stamped with the host time it arrived, so
+    the samples that fall inside the timed region can be picked out afterwards."""
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+
     def __init__(self, idx: int):
         self.p = None
         self.idx = idx
+        self.lines = []
 
     def start(self):
+        import threading
         try:
             self.p = subprocess.Popen(
                 ["nvidia-smi", f"--id={self.idx}",
                  "--query-gpu=clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
                  "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-                 "clocks_event_reasons.sw_power_cap", "--format=csv,noheader,nounits", "-lms", "50"],
-                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                 "clocks_event_reasons.sw_power_cap", "--format=csv,noheader,nounits", "-lms", "20"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True, bufsize=1)
         except Exception:
             self.p = None
+            return
 
-    def stop(self):
+        def pump():
+            for line in self.p.stdout:
+                self.lines.append((time.time(), line))
+        self.t = threading.Thread(target=pump, daemon=True)
+        self.t.start()
+
+    def n_samples(self):
+        return len(self.lines)
+
+    def stop(self, t0=None, t1=None):
         if self.p is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.06)
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"], "samples": 0}
         self.p.terminate()
-        out = self.p.communicate()[0]
+        self.t.join(timeout=2)
+        inside = [l for (t, l) in self.lines if t0 is None or (t0 <= t <= t1 + 0.02)]
+        where = "timed region"
+        if not inside:                                   # region shorter than the polling period: the load around it
+            inside = [l for (t, l) in self.lines]
+            where = "warm-up + timed region (timed region shorter than the 20 ms polling period)"
         sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for line in out.strip().splitlines():
+        for line in inside:
             t = [x.strip() for x in line.split(",")]
             try:
                 sm.append(float(t[0])); mx.append(float(t[1]))
             except Exception:
                 continue
-            for n, v in zip(names, t[2:6]):
+            for n, v in zip(self.NAMES, t[2:6]):
                 if v.lower().startswith("active"):
                     reasons.add(n)
         sm.sort()
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                "reasons": sorted(reasons), "samples": len(sm), "sampled_over": where}
 
 
 def cpu_oracle_sample(M: int, seconds_hint: float = 20.0):
@@ -263,7 +282,7 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--report", action="store_true")
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=400)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="spense")
     ap.add_argument("--M", type=int, default=64)
@@ -328,18 +347,21 @@ def main():
         torch.cuda.current_stream().wait_stream(s)
         return g
 
-    def time_steps(replay, steps, warmup):
+    def time_steps(replay, steps, warmup, host_window=None):
         for _ in range(warmup):
             replay()
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t_host0 = time.time()
         e0.record()
         for _ in range(steps):
             replay()
         e1.record()
         torch.cuda.synchronize()
+        if host_window is not None:
+            host_window[:] = [t_host0, time.time()]
         ms = e0.elapsed_time(e1)
         if dist is not None:
             ms = replicas.max_over_ranks(ms, dist, dev)
@@ -349,8 +371,13 @@ def main():
     g_main = graph_of(lambda: step_eager(blobs, x, sx, sh, hq, y))
     sampler = ClockSampler(local)
     sampler.start()
-    ms_step = time_steps(g_main.replay, args.steps, max(args.warmup, 3))
-    clocks = sampler.stop()
+    t_pre = time.time()
+    while sampler.p is not None and sampler.n_samples() == 0 and time.time() - t_pre < 2.0:
+        g_main.replay()                                  # untimed pre-roll under load until nvidia-smi is polling
+        torch.cuda.synchronize()
+    window = [None, None]
+    ms_step = time_steps(g_main.replay, args.steps, max(args.warmup, 3), window)
+    clocks = sampler.stop(window[0], window[1])
     us_layer = ms_step * 1e3 / LAYERS
 
     # ---- per-kernel view and the all-dense baseline kernel (same library, I_dense = I), rank 0 extras

@@ -207,3 +207,20 @@ def test_fused_single_launch_mlp_equals_two_launches(sp, H, I, p, M):
     y_after = sp.spense_mlp(pk, cuda(c.x), cuda(c.s_x), sh_dev, ws)      # the two-launch path still works on this workspace
     torch.cuda.synchronize()
     assert torch.equal(y_after, y_ref)
+
+
+def test_mlp_host_buffers_equal_device_call(sp):
+    """spense_mlp_host (HOST pinned x, scales and y; copies inside the call) == spense_mlp on device buffers."""
+    H, I, p, M = 640, 896, 0.43, 48
+    c = Case(H, I, p, M, seed=123)
+    pk = c.pack_gpu(sp)
+    s_h = c.default_s_h()
+    ws = sp.spense_workspace(pk, M)
+    for dtype in (torch.float32, torch.bfloat16):
+        y_dev = sp.spense_mlp(pk, cuda(c.x), cuda(c.s_x), cuda(torch.from_numpy(s_h)), ws, dtype=dtype)
+        hx, hsx, hsh = c.x.pin_memory(), c.s_x.pin_memory(), torch.from_numpy(s_h).pin_memory()
+        hy = torch.empty(M, H, dtype=dtype).pin_memory()
+        staging = dict(d_x=torch.empty(M, H, dtype=torch.uint8, device="cuda"), d_scales=torch.empty(2 * M, device="cuda"),
+                       d_hq=torch.empty(M, I, dtype=torch.uint8, device="cuda"), d_y=torch.empty(M, H, dtype=dtype, device="cuda"))
+        sp.spense_mlp_host(pk, hx, hsx, hsh, hy, staging, ws)
+        assert torch.equal(hy, y_dev.cpu())

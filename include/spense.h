@@ -40,7 +40,7 @@ typedef struct CUstream_st* spense_stream_t; /* == cudaStream_t */
 
 enum {
   SPENSE_OK = 0,
-  SPENSE_ERR_ARG = -1,              /* null pointer, M < 1 or M > 98208, bad enum */
+  SPENSE_ERR_ARG = -1,              /* null pointer, M < 1 or M > 2^20, bad enum */
   SPENSE_ERR_ALIGN = -2,            /* pointer not aligned as required */
   SPENSE_ERR_SHAPE = -3,            /* H, I, I_dense not multiples of 128, I_dense > I, too large */
   SPENSE_ERR_BUFFER_TOO_SMALL = -4, /* blob_bytes / ws_bytes below the size query */

@@ -58,16 +58,26 @@ double env_double(const char* name, double dflt) {
   return v ? std::atof(v) : dflt;
 }
 
-// Token columns of one MMA.  Up to 128 tokens: M padded to 16.  More: blocks of block_tokens() inside one launch
-// (virtual tiles).  128 by default; 96 would allow two accumulator buffers (2 x 2 x 96 columns + 32 of metadata
-// fit the 512 TMEM columns) but needs more passes over the weights: measured 141.6 vs 115.4 us/layer at M=256.
-int block_tokens() { static const int b = (int)env_double("SPENSE_BLOCK_TOKENS", 128.0); return b == 96 ? 96 : 128; }
-int n_pad_of(int M) { return M > 128 ? block_tokens() : (M + 15) / 16 * 16; }
-int nb_of(int M) { return M > 128 ? (M + block_tokens() - 1) / block_tokens() : 1; }
+// Token columns of one MMA.  Up to 128 tokens: M padded to 16.  More: blocks of 128 tokens; a launch covers nb_par of
+// them side by side (grid = nb_par * k_par CTAs, k_par stream-K spans per block), so the CTAs of different blocks read
+// the same weight stage at about the same time: one HBM read, the other blocks hit L2.
+int n_pad_of(int M) { return M > 128 ? 128 : (M + 15) / 16 * 16; }
+int nb_of(int M) { return M > 128 ? (M + 127) / 128 : 1; }
+// how many of `nb` blocks one launch takes: the split that keeps most SMs busy over all rounds (ties: more blocks)
+int nb_par_of(int nb, int sms) {
+  int best = 1;
+  double best_eff = 0;
+  for (int c = 1; c <= nb && c <= 32 && c <= sms; ++c) {
+    const int rounds = (nb + c - 1) / c, k = sms / c;
+    const double eff = (double)nb / (rounds * c) * ((double)(c * k) / sms);
+    if (eff >= best_eff - 1e-9) { best_eff = eff > best_eff ? eff : best_eff; best = c; }
+  }
+  return best;
+}
 
 // ---- stream-K schedule: cut the stage sequence into n_spans spans of (nearly) equal bytes.
 struct Schedule {
-  int mode, H, I, I_d, n_pad, sms, fused, nb;
+  int mode, H, I, I_d, n_pad, sms, fused;
   int n_spans;
   int span_begin[kMaxSpans + 1];
   uint32_t span_off[kMaxSpans];   // byte offset of the span's first stage image inside its section
@@ -88,25 +98,24 @@ std::deque<Schedule> g_sched;   // deque: references handed out stay valid
 //   gate_up: span boundaries are nudged so that no tile is shared by more than two spans where a tile is not
 //            much longer than a span (a 3-way tile finishes last and every down span that reads it waits);
 //   down   : spans are sized so that gate_up cost + down cost is the same for every CTA.
-const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms, bool fused = false, int nb = 1) {
+const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms, bool fused = false) {
   const Schedule* gate = (fused && mode == 1) ? &get_schedule(0, g, n_pad, sms, true) : nullptr;
   std::lock_guard<std::mutex> lk(g_sched_mu);
   for (const Schedule& s : g_sched)
-    if (s.mode == mode && s.H == g.H && s.I == g.I && s.I_d == g.I_d && s.n_pad == n_pad && s.sms == sms && s.fused == (int)fused && s.nb == nb) return s;
+    if (s.mode == mode && s.H == g.H && s.I == g.I && s.I_d == g.I_d && s.n_pad == n_pad && s.sms == sms && s.fused == (int)fused) return s;
   Schedule sc = {};
-  sc.mode = mode; sc.H = g.H; sc.I = g.I; sc.I_d = g.I_d; sc.n_pad = n_pad; sc.sms = sms; sc.fused = fused; sc.nb = nb;
+  sc.mode = mode; sc.H = g.H; sc.I = g.I; sc.I_d = g.I_d; sc.n_pad = n_pad; sc.sms = sms; sc.fused = fused;
   // cost of a stage.  Every CTA keeps the same number of ring slots in flight, so under HBM contention a
   // stage costs one slot latency plus its bytes: measured on B200 (profiles/) a 40 KB sparse stage takes
   // ~1.12x a 32 KB dense one => fixed part ~36 KB-equivalents; activation bytes come from L2 and weigh less.
   static const double fixed = env_double("SPENSE_SCHED_FIXED", 36864.0), gamma = env_double("SPENSE_SCHED_GAMMA", 0.25);
   const double cs = fixed + kSparseStageBytes + gamma * 2.0 * n_pad * 128, cd = fixed + kDenseStageBytes + gamma * 1.0 * n_pad * 128;
-  // nb token blocks: every tile appears nb times in a row (virtual tiles), the stage sequence is nb times longer
   std::vector<double> cost;
   if (mode == 0) {
-    cost.insert(cost.end(), (size_t)g.gu_tiles_sparse * nb * g.gu_ns, cs);
-    cost.insert(cost.end(), (size_t)(g.gu_tiles - g.gu_tiles_sparse) * nb * g.gu_nd, cd);
+    cost.insert(cost.end(), (size_t)g.gu_tiles_sparse * g.gu_ns, cs);
+    cost.insert(cost.end(), (size_t)(g.gu_tiles - g.gu_tiles_sparse) * g.gu_nd, cd);
   } else {
-    for (int t = 0; t < g.dn_tiles * nb; ++t) {
+    for (int t = 0; t < g.dn_tiles; ++t) {
       cost.insert(cost.end(), (size_t)g.dn_ns, cs);
       cost.insert(cost.end(), (size_t)g.dn_nd, cd);
     }
@@ -171,7 +180,7 @@ const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms, bo
   // byte offsets: the blob stores the stage images in exactly this linear order
   std::vector<uint32_t> bytes(total);
   if (mode == 0) {
-    for (int i = 0; i < total; ++i) bytes[i] = i < g.gu_tiles_sparse * nb * g.gu_ns ? kSparseStageBytes : kDenseStageBytes;
+    for (int i = 0; i < total; ++i) bytes[i] = i < g.gu_tiles_sparse * g.gu_ns ? kSparseStageBytes : kDenseStageBytes;
   } else {
     const int per = g.dn_ns + g.dn_nd;
     for (int i = 0; i < total; ++i) bytes[i] = (i % per) < g.dn_ns ? kSparseStageBytes : kDenseStageBytes;
@@ -256,9 +265,10 @@ void fill_common(GemmParams& p, const Schedule& sc, int M, int n_pad, void* d_ws
     const uint32_t from = next_prefetch_bytes(sc, i);
     const uint32_t left = sc.span_len[i] - from;
     p.self_off[i] = from - sc.span_pre[i];
-    p.self_len[i] = sc.nb > 1 ? 0 : (self_want < left ? self_want : left);   // virtual tiles: a span is not one byte range
+    p.self_len[i] = self_want < left ? self_want : left;
   }
-  p.nb = sc.nb;
+  p.nb = 1;
+  p.blk0 = 0;
   p.M = M;
   p.n_pad = n_pad;
   p.slot_bytes = slot_bytes_of(n_pad);
@@ -297,11 +307,13 @@ void fill_next(GemmParams& p, const uint8_t* next_section, const Schedule& next)
 // parameter block + tensor map of one gate_up launch over tokens [m0, m0 + Mb)
 int gate_up_params(const Geometry& g, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_x, const float* d_sx,
                    int m0, int Mb, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32, void* d_ws,
-                   bool dynamic, GemmParams& p, CUtensorMap& tm, bool fused = false) {
-  const int n_pad = n_pad_of(Mb);                            // > 128 tokens: blocks of 128 inside one launch
-  const Schedule& sc = get_schedule(0, g, n_pad, g_num_sms, fused, nb_of(Mb));
+                   bool dynamic, GemmParams& p, CUtensorMap& tm, bool fused = false, int k_par = 0, int nb_launch = 1,
+                   int blk0 = 0) {
+  const int n_pad = n_pad_of(Mb);
+  const Schedule& sc = get_schedule(0, g, n_pad, k_par > 0 ? k_par : g_num_sms, fused);
   p = GemmParams{};
   fill_common(p, sc, Mb, n_pad, d_ws);
+  p.nb = nb_launch; p.blk0 = blk0;
   p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.gate_up_off;
   p.mode = 0;
   p.num_tiles = g.gu_tiles; p.tiles_sparse = g.gu_tiles_sparse;
@@ -318,12 +330,13 @@ int gate_up_params(const Geometry& g, const BlobHeader& hdr, const void* d_blob,
 
 int down_params(const Geometry& g, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_hq, const float* d_sh,
                 int32_t sh_stride, int m0, int Mb, void* d_y, int32_t y_dtype, void* d_ws, GemmParams& p, CUtensorMap& tm,
-                bool fused = false) {
+                bool fused = false, int k_par = 0, int nb_launch = 1, int blk0 = 0) {
   const size_t esz = y_dtype == SPENSE_F32 ? 4 : 2;
   const int n_pad = n_pad_of(Mb);
-  const Schedule& sc = get_schedule(1, g, n_pad, g_num_sms, fused, nb_of(Mb));
+  const Schedule& sc = get_schedule(1, g, n_pad, k_par > 0 ? k_par : g_num_sms, fused);
   p = GemmParams{};
   fill_common(p, sc, Mb, n_pad, d_ws);
+  p.nb = nb_launch; p.blk0 = blk0;
   p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off;
   p.mode = 1;
   p.num_tiles = g.dn_tiles; p.tiles_sparse = 0;
@@ -340,26 +353,39 @@ int gate_up_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void*
                  const float* d_sx, int32_t M, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32,
                  void* d_ws, bool pdl, bool down_follows, cudaStream_t stream, bool dynamic = false) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  GemmParams p;
-  CUtensorMap tm;
-  int st = gate_up_params(g, hdr, d_blob, d_x, d_sx, 0, M, d_sh, sh_stride, d_hq, d_h_f32, d_ws, dynamic, p, tm);
-  if (st) return st;
-  if (down_follows && M <= 128)                              // the same layer's down projection streams next
-    fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off, get_schedule(1, g, n_pad_of(M), g_num_sms));
-  return launch_gemm(p, tm, pdl, stream);
+  const int nb = nb_of(M), par = nb_par_of(nb, g_num_sms);
+  for (int blk0 = 0; blk0 < nb; blk0 += par) {               // M <= 128: one launch of one block
+    const int nb_l = nb - blk0 < par ? nb - blk0 : par;
+    GemmParams p;
+    CUtensorMap tm;
+    int st = gate_up_params(g, hdr, d_blob, d_x, d_sx, 0, M, d_sh, sh_stride, d_hq, d_h_f32, d_ws, dynamic, p, tm, false,
+                            g_num_sms / nb_l, nb_l, blk0);
+    if (st) return st;
+    if (down_follows && nb == 1)                             // the same layer's down projection streams next
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off, get_schedule(1, g, n_pad_of(M), g_num_sms));
+    st = launch_gemm(p, tm, pdl, stream);
+    if (st) return st;
+  }
+  return SPENSE_OK;
 }
 
 int down_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_hq,
               const float* d_sh, int32_t sh_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, bool pdl,
               const void* d_next_blob, cudaStream_t stream) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  GemmParams p;
-  CUtensorMap tm;
-  int st = down_params(g, hdr, d_blob, d_hq, d_sh, sh_stride, 0, M, d_y, y_dtype, d_ws, p, tm);
-  if (st) return st;
-  if (d_next_blob && M <= 128)                               // the next layer's gate/up weights stream next
-    fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + hdr.gate_up_off, get_schedule(0, g, n_pad_of(M), g_num_sms));
-  return launch_gemm(p, tm, pdl, stream);
+  const int nb = nb_of(M), par = nb_par_of(nb, g_num_sms);
+  for (int blk0 = 0; blk0 < nb; blk0 += par) {
+    const int nb_l = nb - blk0 < par ? nb - blk0 : par;
+    GemmParams p;
+    CUtensorMap tm;
+    int st = down_params(g, hdr, d_blob, d_hq, d_sh, sh_stride, 0, M, d_y, y_dtype, d_ws, p, tm, false, g_num_sms / nb_l, nb_l, blk0);
+    if (st) return st;
+    if (d_next_blob && nb == 1)                              // the next layer's gate/up weights stream next
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + hdr.gate_up_off, get_schedule(0, g, n_pad_of(M), g_num_sms));
+    st = launch_gemm(p, tm, pdl, stream);
+    if (st) return st;
+  }
+  return SPENSE_OK;
 }
 
 // One token block: gate_up and down as ONE persistent launch (spense_mlp_kernel); down's Hq loads are gated per
@@ -412,19 +438,19 @@ void spense_debug_set_fused(int on) { g_fused = on ? 1 : 0; }
 // debug hook (undeclared in spense.h; host only, no device needed): the stream-K schedule the library would use
 // for (shape, M, mode 0 gate_up / 1 down, fused, sms).  Writes n_spans + 1 span boundaries (linear stage indices)
 // into out_span_begin (room for 161 ints) and returns n_spans, or a negative status.  out_info[0..3] = total
-// stages, token blocks, token columns per MMA, ring slots.
+// stages, token blocks per launch, token columns per MMA, ring slots.
 int spense_debug_schedule(const spense_shape_t* shape, int32_t M, int32_t mode, int32_t fused, int32_t sms,
                           int32_t* out_span_begin, int32_t* out_info) {
   int st = check_shape(shape);
   if (st) return st;
   if (M < 1 || M > kMaxTokens || (mode != 0 && mode != 1) || sms < 1 || !out_span_begin) return SPENSE_ERR_ARG;
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const int n_pad = n_pad_of(M), nb = nb_of(M);
-  const Schedule& sc = get_schedule(mode, g, n_pad, sms, fused != 0 && nb == 1, nb);
+  const int n_pad = n_pad_of(M), nb = nb_of(M), par = nb_par_of(nb, sms);
+  const Schedule& sc = get_schedule(mode, g, n_pad, sms / par, fused != 0 && nb == 1);
   for (int i = 0; i <= sc.n_spans; ++i) out_span_begin[i] = sc.span_begin[i];
   if (out_info) {
     out_info[0] = sc.span_begin[sc.n_spans];
-    out_info[1] = nb;
+    out_info[1] = par;                                       // token blocks side by side in one launch
     out_info[2] = n_pad;
     out_info[3] = ring_stages_of(n_pad);
   }

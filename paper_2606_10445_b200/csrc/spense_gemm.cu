@@ -22,9 +22,11 @@
 //                epilogue -- nothing but the flag check sits on the owner's critical path;
 //   * > 2 spans: every span finishes late, so all dump, and the n spans reduce M/n token columns each
 //                (reduce-scatter) instead of one owner reducing n partials serially.
-// More than 128 tokens: token blocks of 128 inside the same launch.  The stage sequence then visits "virtual
-// tiles" (pair tile x token block, block index fastest): a weight tile is streamed from HBM for the first block
-// and re-read from L2 for the others; spans, fix-ups and flags work unchanged on the longer sequence.
+// More than 128 tokens: blocks of 128 tokens SIDE BY SIDE in one launch.  The grid is nb * n_spans CTAs; CTA b works
+// on token block b / n_spans and span n_spans-1 - b % n_spans of the same schedule, so the CTAs of different blocks
+// read the same weight stage at about the same time: one HBM read, the other blocks hit L2 (measured at M=2048:
+// 210 MB of DRAM reads per launch of 4 blocks).  Every block has its own fix-up slots; more blocks than fit run
+// as further launches.
 // Flags hold the epoch of the launch (a device-side counter in the workspace), so nothing has to be
 // reset between launches and CUDA-graph replays see fresh values.
 // Span i runs on CTA n_spans-1-i.  CTAs of one launch wait for each other, so all n_spans <= #SM CTAs
@@ -51,10 +53,9 @@ namespace spense {
 
 namespace {
 
-// Position in the linear stage sequence: pair tile, token block, stage inside the tile, stages of the tile.
-// With nb token blocks the sequence visits "virtual tiles" v = tile * nb + blk.
+// Position in the linear stage sequence: pair tile, stage inside the tile, stages of the tile.
 struct Cursor {
-  int tile, blk, j, ns, nd, first;   // first = linear index of the (virtual) tile's first stage
+  int tile, j, ns, nd, first;   // first = linear index of the tile's first stage
 };
 
 // byte offset of stage j of pair tile `tile` inside the section (the blob stores every tile once)
@@ -73,27 +74,24 @@ __device__ __forceinline__ size_t stage_byte_offset(const GemmParams& p, int til
 template <int MODE>
 __device__ __noinline__ Cursor cursor_at(const GemmParams& p, int s, unsigned long long* byte_off) {
   Cursor c;
-  int v;                                                   // virtual tile
   if (MODE == 0) {
-    const int sparse_total = p.tiles_sparse * p.nb * p.ns;
+    const int sparse_total = p.tiles_sparse * p.ns;
     if (s < sparse_total) {
-      v = s / p.ns;
-      c.first = v * p.ns;
+      c.tile = s / p.ns;
+      c.first = c.tile * p.ns;
       c.ns = p.ns; c.nd = 0;
     } else {
       const int td = (s - sparse_total) / p.nd;
-      v = p.tiles_sparse * p.nb + td;
+      c.tile = p.tiles_sparse + td;
       c.first = sparse_total + td * p.nd;
       c.ns = 0; c.nd = p.nd;
     }
   } else {
     const int per = p.ns + p.nd;
-    v = s / per;
-    c.first = v * per;
+    c.tile = s / per;
+    c.first = c.tile * per;
     c.ns = p.ns; c.nd = p.nd;
   }
-  c.tile = p.nb == 1 ? v : v / p.nb;
-  c.blk = p.nb == 1 ? 0 : v - c.tile * p.nb;
   c.j = s - c.first;
   *byte_off = stage_byte_offset<MODE>(p, c.tile, c.j);
   return c;
@@ -102,13 +100,10 @@ __device__ __noinline__ Cursor cursor_at(const GemmParams& p, int s, unsigned lo
 template <int MODE>
 __device__ __forceinline__ void next_tile(const GemmParams& p, Cursor& c) {
   c.first += c.ns + c.nd;
+  ++c.tile;
   c.j = 0;
-  if (++c.blk == p.nb) {
-    c.blk = 0;
-    ++c.tile;
-    if (MODE == 0) {
-      if (c.tile < p.tiles_sparse) { c.ns = p.ns; c.nd = 0; } else { c.ns = 0; c.nd = p.nd; }
-    }
+  if (MODE == 0) {
+    if (c.tile < p.tiles_sparse) { c.ns = p.ns; c.nd = 0; } else { c.ns = 0; c.nd = p.nd; }
   }
 }
 
@@ -175,6 +170,8 @@ struct Ctx {
   uint8_t* smem_gen;           // the same, generic
   int S;                       // ring slots
   uint32_t slot_bytes, ring_bytes, bar_base, b_tile_bytes, tmem_base;
+  int blk;                     // token block of this CTA (0 unless the launch covers several blocks)
+  int gbase;                   // first fix-up slot (flags, partials) of this block: block-in-launch * n_spans
   __device__ __forceinline__ uint32_t full_bar(int s) const { return bar_base + 8u * s; }
   __device__ __forceinline__ uint32_t empty_bar(int s) const { return bar_base + 8u * (8 + s); }
   __device__ __forceinline__ uint32_t accf_bar(int b) const { return bar_base + 8u * (16 + b); }
@@ -230,7 +227,7 @@ __device__ __forceinline__ void finish(const GemmParams& p, const void* sc, int 
 }
 
 // A tile shared by more than two spans [a, b]: reduced at the end of the phase (reduce-scatter).
-struct Group { int a, b, tile, first, blk; };
+struct Group { int a, b, tile, first; };
 
 // ===================== producer (one thread) =====================
 // Streams the stages of span `span` of one phase through the ring.  `it` counts the stages of the whole
@@ -244,7 +241,8 @@ __device__ __forceinline__ void producer_phase(const GemmParams& p, const CUtens
   const int S = cx.S;
   const int sb = p.span_begin[span];
   const int n = p.span_begin[span + 1] - sb;
-  // one token block: a weight byte is used once (evict first); several: the next block re-reads the tile from L2
+  // one token block: a weight byte is used once (evict first); several: the CTAs of the other blocks read the same
+  // stage at about the same time and should find it in L2
   const uint64_t pol_w = p.nb == 1 ? policy_evict_first() : policy_evict_normal();
   const uint64_t pol_a = policy_evict_last();
   unsigned long long off;
@@ -255,7 +253,7 @@ __device__ __forceinline__ void producer_phase(const GemmParams& p, const CUtens
   int dep_lo = 0, dep_hi = 0;                              // Hq tiles [dep_lo, dep_hi) are known to be stored
 
   auto tiles_ready = [&](uint32_t inf) -> bool {           // at most one poll (16 flags) per call
-    const int k0 = (int)(inf & 0x1FFFFFu);
+    const int k0 = (int)(inf & 0x7FFFFFFFu);
     const int t_first = k0 >> 7;
     int t_last = (k0 + ((inf >> 31) ? 255 : 127)) >> 7;
     if (t_last >= p.dep_tiles) t_last = p.dep_tiles - 1;   // a padded K stage reads no further than the last tile
@@ -281,8 +279,8 @@ __device__ __forceinline__ void producer_phase(const GemmParams& p, const CUtens
   };
   auto load_b = [&](int slot, uint32_t inf) {
     const uint32_t b_dst = cx.smem_base + (uint32_t)slot * cx.slot_bytes + kSparseStageBytes;
-    const int k0 = (int)(inf & 0x1FFFFFu);                  // K coordinate | token block << 21 | sparse << 31
-    const int row0 = (int)((inf >> 21) & 0x3FFu) * p.n_pad;  // token blocks hold n_pad tokens
+    const int k0 = (int)(inf & 0x7FFFFFFFu);                // K coordinate | sparse << 31
+    const int row0 = cx.blk * p.n_pad;                      // this CTA's token block
     tma_load_2d(b_dst, tmap, k0, row0, cx.full_bar(slot), pol_a);
     if (inf >> 31) tma_load_2d(b_dst + cx.b_tile_bytes, tmap, k0 + 128, row0, cx.full_bar(slot), pol_a);
   };
@@ -298,8 +296,7 @@ __device__ __forceinline__ void producer_phase(const GemmParams& p, const CUtens
     // everything that does not need the slot is computed before the wait: a freed slot is refilled at once
     const bool sp = c.j < c.ns;
     const uint32_t wb = sp ? (uint32_t)kSparseStageBytes : (uint32_t)kDenseStageBytes;
-    const uint32_t inf = (uint32_t)(sp ? c.j * kSparseStageK : p.dense_k0 + (c.j - c.ns) * kDenseStageK) | ((uint32_t)c.blk << 21) |
-                         (sp ? 0x80000000u : 0u);
+    const uint32_t inf = (uint32_t)(sp ? c.j * kSparseStageK : p.dense_k0 + (c.j - c.ns) * kDenseStageK) | (sp ? 0x80000000u : 0u);
     const uint32_t tx = wb + (sp ? 2u : 1u) * cx.b_tile_bytes;
     const uint32_t fb = cx.full_bar(w_slot);
     const uint32_t dst = cx.smem_base + (uint32_t)w_slot * cx.slot_bytes;
@@ -317,10 +314,7 @@ __device__ __forceinline__ void producer_phase(const GemmParams& p, const CUtens
         if (k == ((it0 + w) & 7)) info[k] = inf;
     }
     src += wb;
-    if (++c.j == c.ns + c.nd) {
-      next_tile<MODE>(p, c);
-      if (p.nb > 1) src = p.section + stage_byte_offset<MODE>(p, c.tile, 0);   // same tile again for the next token block
-    }
+    if (++c.j == c.ns + c.nd) next_tile<MODE>(p, c);
     ++w;
     if (++w_slot == S) { w_slot = 0; ++w_round; }
     return true;
@@ -480,10 +474,16 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
   const int q = warp & 3;
   const int row = q * 32 + lane;                           // accumulator lane = weight row inside the tile
   const int et = threadIdx.x - 128;                        // 0..511
+  const int m_base = cx.blk * p.n_pad;                     // this CTA's token block
+  const int Mb = min(p.n_pad, p.M - m_base);
+  const int cols_used = min(p.n_pad, (Mb + 7) & ~7);       // token columns holding real tokens, rounded to the TMEM load width
   const int cols_per = (((p.n_pad + 3) >> 2) + 7) & ~7;    // columns per warp: a quarter, rounded to the TMEM load width
   const int c_begin = ((warp - 4) >> 2) * cols_per;
+  const int c_end = min(c_begin + cols_per, cols_used);
   const float* stg = reinterpret_cast<const float*>(cx.smem_gen);   // the stage ring doubles as partial staging
   const size_t part_floats = (size_t)2 * p.n_pad * 128;    // one partial: [mat][col][row]
+  int* const flags = p.flags + cx.gbase * 2;               // fix-up slots of this token block
+  float* const partials = p.partials + (size_t)cx.gbase * 2 * part_floats;
   const int sb = p.span_begin[span], se = p.span_begin[span + 1];
 
   Group groups[2];
@@ -497,16 +497,6 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
     const int seg_end = min(se, tile_end);
     const int buf = seg % p.num_acc_bufs;
     const uint32_t use = (uint32_t)(seg / p.num_acc_bufs);
-    // the token block of this (virtual) tile
-    const int m_base = cur.blk * p.n_pad;
-    const int Mb = p.nb == 1 ? p.M : min(p.n_pad, p.M - m_base);
-    const int cols_used = min(p.n_pad, (Mb + 7) & ~7);     // token columns holding real tokens, rounded to the TMEM load width
-    const int c_end = min(c_begin + cols_per, cols_used);
-    if (p.nb > 1) {                                        // this block's scales (the table holds one block)
-      epi_sync();
-      epilogue_tables(p, cx, et, m_base, Mb);
-      epi_sync();
-    }
     // spans [a, b] that hold stages of this tile
     int a = span, b = span;
     while (p.span_begin[a] > cur.first) --a;
@@ -527,10 +517,10 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
       // the whole tile is ours, or we own a tile whose tail the next span has (usually long ago) dumped
       const bool add = a != b;
       const bool staged = add && ring_free;                // owner = last segment of the span: every MMA is complete
-      const float* part = p.partials + (size_t)b * 2 * part_floats;   // span b starts inside the tile: its first segment
+      const float* part = partials + (size_t)b * 2 * part_floats;   // span b starts inside the tile: its first segment
       float a0[8], a1[8];                                  // direct owner-add: the partner's partial, one chunk ahead
       if (add) {
-        const int* f = p.flags + b * 2;
+        const int* f = flags + b * 2;
         if (staged) {
           if (et == 0) {
             while (ld_acquire(f) != epoch) {}
@@ -598,7 +588,7 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
     } else {
       // split tile, not (solely) ours to finish: dump the raw fp32 partial [mat][col][row] and publish it
       const int which = (sb >= cur.first) ? 0 : 1;         // our first segment, or our last one
-      float* slot = p.partials + ((size_t)span * 2 + which) * part_floats;
+      float* slot = partials + ((size_t)span * 2 + which) * part_floats;
 #pragma unroll 1
       for (int c = c_begin; c < c_end; c += 8) {
         uint32_t v0[8], v1[8];
@@ -614,10 +604,9 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
       tc_fence_before();
       mbar_arrive(cx.acce_bar(buf));
       epi_sync();                                          // all partial stores issued (CTA scope) ...
-      if (et == 0) st_release(p.flags + span * 2 + which, epoch);   // ... one gpu-scope release publishes them (cumulativity)
+      if (et == 0) st_release(flags + span * 2 + which, epoch);   // ... one gpu-scope release publishes them (cumulativity)
       if (b > a + 1) {
         groups[n_groups].a = a; groups[n_groups].b = b; groups[n_groups].tile = cur.tile; groups[n_groups].first = cur.first;
-        groups[n_groups].blk = cur.blk;
         ++n_groups;
       }
     }
@@ -633,15 +622,8 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
     const Group g = groups[gi];
     const int n = g.b - g.a + 1;
     const int j = span - g.a;
-    const int m_base = g.blk * p.n_pad;
-    const int Mb = p.nb == 1 ? p.M : min(p.n_pad, p.M - m_base);
     const int m0 = (int)(((long long)j * Mb) / n), m1 = (int)(((long long)(j + 1) * Mb) / n);
     const int rrow = et & 127;
-    if (p.nb > 1) {                                        // the scale table holds one block: this group's
-      epi_sync();
-      epilogue_tables(p, cx, et, m_base, Mb);
-      epi_sync();
-    }
     if (m1 > m0 && ring_free) {
       // all MMAs of this CTA are complete: the stage ring stages the partial slices
       int cc_max = (int)(cx.ring_bytes / ((uint32_t)n * 1024u));
@@ -659,9 +641,9 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
         for (int i = et; i < 2 * n; i += kEpiThreads) {
           const int qs = g.a + (i >> 1), mat = i & 1;
           const int which = (p.span_begin[qs] >= g.first) ? 0 : 1;
-          while (ld_acquire(p.flags + qs * 2 + which) != epoch) {}
+          while (ld_acquire(flags + qs * 2 + which) != epoch) {}
           asm volatile("fence.proxy.async.global;" ::: "memory");   // partner's generic-proxy stores -> our async-proxy read
-          const float* src = p.partials + ((size_t)qs * 2 + which) * part_floats + ((size_t)mat * p.n_pad + mc) * 128;
+          const float* src = partials + ((size_t)qs * 2 + which) * part_floats + ((size_t)mat * p.n_pad + mc) * 128;
           bulk_g2s(cx.smem_base + (uint32_t)(i * cc) * 512u, src, (uint32_t)cc * 512u, cx.red_bar(), policy_evict_first());
         }
         mbar_wait(cx.red_bar(), red_round & 1u);
@@ -684,7 +666,7 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
       if (et < n) {
         const int qs = g.a + et;
         const int which = (p.span_begin[qs] >= g.first) ? 0 : 1;
-        while (ld_acquire(p.flags + qs * 2 + which) != epoch) {}
+        while (ld_acquire(flags + qs * 2 + which) != epoch) {}
       }
       epi_sync();
 #pragma unroll 1
@@ -697,7 +679,7 @@ __device__ __forceinline__ void epilogue_phase(const GemmParams& p, const Ctx& c
           for (int k = 0; k < 4; ++k) {
             const int qs = g.a + min(q0 + k, n - 1);
             const int which = (p.span_begin[qs] >= g.first) ? 0 : 1;
-            const float* src = p.partials + ((size_t)qs * 2 + which) * part_floats;
+            const float* src = partials + ((size_t)qs * 2 + which) * part_floats;
             v0[k] = __ldcg(src + (size_t)c * 128 + rrow);
             v1[k] = __ldcg(src + (size_t)(p.n_pad + c) * 128 + rrow);
           }
@@ -777,15 +759,28 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
   if (warp == 0 && lane == 0) prefetch_tmap(&tmap_b);
-  const Ctx cx = prologue(p, smem_raw);
-  const int span = p.n_spans - 1 - (int)blockIdx.x;
-  if (p.trace && threadIdx.x == 0) {
+  Ctx cx = prologue(p, smem_raw);
+  // a launch covers p.nb token blocks: CTA b works on block blk0 + b / n_spans, span n_spans - 1 - b % n_spans of
+  // the SAME stream-K schedule, so the CTAs of different blocks read the same weight stage at about the same time
+  // (one HBM read, the rest L2 hits); each block has its own fix-up slots.  A block past the last token idles.
+  const int bp = (int)blockIdx.x / p.n_spans;
+  const int span = p.n_spans - 1 - ((int)blockIdx.x - bp * p.n_spans);
+  cx.blk = p.blk0 + bp;
+  cx.gbase = bp * p.n_spans;
+  const bool idle = cx.blk * p.n_pad >= p.M;
+  if (p.trace && threadIdx.x == 0 && bp == 0) {
     uint32_t smid;
     asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
     p.trace[(size_t)span * 16 + 0] = globaltimer(); p.trace[(size_t)span * 16 + 14] = smid;
   }
 
-  if (warp == 0) {
+  if (idle) {
+    // nothing to compute, but the launch counts its CTAs for the epoch
+    if (threadIdx.x == 128 + kEpiThreads - 1) {
+      pdl_wait();
+      take_epoch(p.ws_ctrl, nullptr, (int)gridDim.x, cx.epoch_ptr());
+    }
+  } else if (warp == 0) {
     if (lane == 0) {
       int it = 0;
       bool pdl_done = false;
@@ -802,8 +797,8 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
     const int et = threadIdx.x - 128;
     // scales, the workspace and the epoch word may be produced / still in use by the previous kernel
     pdl_wait();
-    epilogue_tables(p, cx, et, 0, p.nb == 1 ? p.M : min(p.n_pad, p.M));
-    if (et == kEpiThreads - 1) take_epoch(p.ws_ctrl, nullptr, p.n_spans, cx.epoch_ptr());
+    epilogue_tables(p, cx, et, cx.blk * p.n_pad, min(p.n_pad, p.M - cx.blk * p.n_pad));
+    if (et == kEpiThreads - 1) take_epoch(p.ws_ctrl, nullptr, (int)gridDim.x, cx.epoch_ptr());
     epi_sync();
     const int epoch = cx.epoch_ptr()[0];                   // flag value of THIS launch (never equals a stale flag)
     int seg = 0;
@@ -815,7 +810,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
       if (et < p.n_pad) p.amax_part[(size_t)span * p.n_pad + et] = et < p.M ? cx.sc0()[et].z : 0.0f;
     }
     if (et == 0) *cx.epi_done_ptr() = 1;
-    if (p.trace && et == 0) p.trace[(size_t)span * 16 + 10] = globaltimer();
+    if (p.trace && et == 0 && bp == 0) p.trace[(size_t)span * 16 + 10] = globaltimer();
   }
 
   tc_fence_before();
@@ -833,7 +828,9 @@ spense_mlp_kernel(const __grid_constant__ GemmParams pg, const __grid_constant__
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
   if (warp == 0 && lane == 0) { prefetch_tmap(&tmap_x); prefetch_tmap(&tmap_hq); }
-  const Ctx cx = prologue(pg, smem_raw);
+  Ctx cx = prologue(pg, smem_raw);
+  cx.blk = 0;
+  cx.gbase = 0;
   const int span_g = pg.n_spans - 1 - (int)blockIdx.x;
   const int span_d = pd.n_spans - 1 - (int)blockIdx.x;
   if (threadIdx.x == 0) {
@@ -915,7 +912,7 @@ cudaError_t set_attrs() {
 int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, bool pdl, cudaStream_t stream) {
   if (set_attrs() != cudaSuccess) return SPENSE_ERR_CUDA;
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)p.n_spans);
+  cfg.gridDim = dim3((unsigned)(p.n_spans * p.nb));
   cfg.blockDim = dim3(kThreads);
   cfg.dynamicSmemBytes = smem_bytes_of(p);
   cfg.stream = stream;

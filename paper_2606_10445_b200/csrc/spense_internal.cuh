@@ -36,7 +36,7 @@ constexpr int kBlobHeaderBytes = 1024;
 constexpr uint32_t kBlobMagic = 0x53504E53u;  // "SNPS"
 constexpr int kBlobVersion = 1;
 constexpr int kMaxSpans = 160;
-constexpr int kMaxTokens = 96 * 1023;        // token blocks are numbered in 10 bits of a stage descriptor
+constexpr int kMaxTokens = 1 << 20;           // tokens per call (the activation tensor map is built over all of them)
 constexpr int kSmemMax = 232448;             // opt-in dynamic shared memory per CTA
 constexpr int kFlagBytes = 4096;             // control words (128 B) + 2 flags per span
 constexpr int kAmaxBytes = 160 * 128 * 4;    // dynamic requant: max|h| per span and token (follows the flags)
@@ -101,9 +101,9 @@ struct GemmParams {
   int dense_k0;             // K byte offset of the first dense stage in the B operand (mode 1: I_s)
   int n_spans;
   int M, n_pad;             // tokens in this launch; token columns of one MMA (M padded to 16, at most 128)
-  int nb;                   // token blocks of n_pad tokens (1 for M <= 128).  nb > 1: every pair tile is visited nb times in a
-                            // row ("virtual tile" = tile * nb + block), so a weight tile is streamed from HBM once
-                            // and re-read from L2 for the following blocks
+  int nb, blk0;             // token blocks of n_pad tokens covered by this launch (grid = nb * n_spans CTAs) and the first
+                            // of them: the CTAs of the nb blocks walk the same schedule side by side, so a weight stage is
+                            // read from HBM once and found in L2 by the other blocks
   int num_stages, slot_bytes, acc_stride, num_acc_bufs;
   // epilogue
   const float* s_act;       // mode 0: s_x [M]; mode 1: s_h (stride sh_stride)

@@ -27,7 +27,7 @@ def schedule(lib, H, I, I_d, M, mode, fused=0, sms=148):
 
 
 def stage_layout(H, I, I_d, mode, nb):
-    """stage counts per (virtual) tile and bytes per stage, written out from the blob layout"""
+    """stage counts per tile and bytes per stage, written out from the blob layout"""
     I_s = I - I_d
     if mode == 0:
         tiles = [("s", -(-H // 256))] * ((I_s // 128) * nb) + [("d", H // 128)] * ((I_d // 128) * nb)
@@ -44,12 +44,16 @@ SEED0 = (5120, 27648, 0)
 @pytest.mark.parametrize("M", [1, 64, 128, 200, 1000])
 @pytest.mark.parametrize("mode", [0, 1])
 def test_spans_partition_the_stage_sequence(lib, shape, M, mode):
-    sb, (total, nb, n_pad, ring) = schedule(lib, *shape, M, mode)
-    tiles = stage_layout(*shape, mode, nb)
+    sb, (total, par, n_pad, ring) = schedule(lib, *shape, M, mode)
+    tiles = stage_layout(*shape, mode, 1)
     assert total == sum(len(t) for t in tiles)
-    assert nb == (1 if M <= 128 else -(-M // 128)) and n_pad == (min(128, -(-M // 16) * 16))
+    nb = 1 if M <= 128 else -(-M // 128)
+    # more than 128 tokens: `par` blocks of 128 side by side in one launch, each with 148 // par spans of the same schedule
+    assert 1 <= par <= min(nb, 32) and (par == 1) == (nb == 1) and n_pad == (min(128, -(-M // 16) * 16))
     assert sb[0] == 0 and sb[-1] == total and (np.diff(sb) >= 1).all()          # every CTA owns at least one stage
-    assert len(sb) - 1 <= 148 and 2 <= ring <= 8
+    assert len(sb) - 1 <= 148 // par and 2 <= ring <= 8
+    rounds = -(-nb // par)
+    assert nb / (rounds * par) * (par * (148 // par) / 148) >= 0.8              # the split keeps most SMs busy
     assert ring * (40960 + 2 * n_pad * 128) + 1024 + 256 + 20 * n_pad <= 232448   # the ring fits the opt-in smem
 
 

@@ -61,8 +61,9 @@ double env_double(const char* name, double dflt) {
 // Token columns of one MMA.  Up to 128 tokens: M padded to 16.  More: blocks of 128 tokens; a launch covers nb_par of
 // them side by side (grid = nb_par * k_par CTAs, k_par stream-K spans per block), so the CTAs of different blocks read
 // the same weight stage at about the same time: one HBM read, the other blocks hit L2.
-int n_pad_of(int M) { return M > 128 ? 128 : (M + 15) / 16 * 16; }
-int nb_of(int M) { return M > 128 ? (M + 127) / 128 : 1; }
+int block_tokens() { static const int b = (int)env_double("SPENSE_BLOCK_TOKENS", 128.0); return b == 96 ? 96 : 128; }
+int n_pad_of(int M) { return M > 128 ? block_tokens() : (M + 15) / 16 * 16; }
+int nb_of(int M) { return M > 128 ? (M + block_tokens() - 1) / block_tokens() : 1; }
 // how many of `nb` blocks one launch takes: the split that keeps most SMs busy over all rounds (ties: more blocks)
 int nb_par_of(int nb, int sms) {
   int best = 1;

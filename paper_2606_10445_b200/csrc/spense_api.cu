@@ -64,16 +64,20 @@ double env_double(const char* name, double dflt) {
 int block_tokens() { static const int b = (int)env_double("SPENSE_BLOCK_TOKENS", 128.0); return b == 96 ? 96 : 128; }
 int n_pad_of(int M) { return M > 128 ? block_tokens() : (M + 15) / 16 * 16; }
 int nb_of(int M) { return M > 128 ? (M + block_tokens() - 1) / block_tokens() : 1; }
-// how many of `nb` blocks one launch takes: the split that keeps most SMs busy over all rounds (ties: more blocks)
+// how many of `nb` blocks one launch takes: the largest split within 5 % of the best SM occupancy over all rounds
+// (every round is a launch with its own start-up and fix-up tail, so fewer rounds win a near tie)
 int nb_par_of(int nb, int sms) {
-  int best = 1;
-  double best_eff = 0;
-  for (int c = 1; c <= nb && c <= 32 && c <= sms; ++c) {
+  auto eff = [&](int c) {
     const int rounds = (nb + c - 1) / c, k = sms / c;
-    const double eff = (double)nb / (rounds * c) * ((double)(c * k) / sms);
-    if (eff >= best_eff - 1e-9) { best_eff = eff > best_eff ? eff : best_eff; best = c; }
-  }
-  return best;
+    return (double)nb / (rounds * c) * ((double)(c * k) / sms);
+  };
+  const int cmax = nb < 32 ? (nb < sms ? nb : sms) : (32 < sms ? 32 : sms);
+  double best = 0;
+  for (int c = 1; c <= cmax; ++c) best = eff(c) > best ? eff(c) : best;
+  int pick = 1;
+  for (int c = 1; c <= cmax; ++c)
+    if (eff(c) >= 0.95 * best) pick = c;
+  return pick;
 }
 
 // ---- stream-K schedule: cut the stage sequence into n_spans spans of (nearly) equal bytes.

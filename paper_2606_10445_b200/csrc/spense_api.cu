@@ -278,8 +278,8 @@ void fill_common(GemmParams& p, const Schedule& sc, int M, int n_pad, void* d_ws
   p.n_pad = n_pad;
   p.slot_bytes = slot_bytes_of(n_pad);
   p.num_stages = ring_stages_of(n_pad);
-  p.acc_stride = n_pad <= 32 ? 32 : (n_pad <= 64 ? 64 : (n_pad <= 96 ? 96 : 128));
-  p.num_acc_bufs = n_pad <= 96 ? 2 : 1;                     // 2 buffers x 2 accumulators x 96 columns + metadata at 480
+  p.acc_stride = n_pad <= 32 ? 32 : (n_pad <= 64 ? 64 : (n_pad <= 96 ? 96 : (n_pad <= 112 ? 112 : 128)));
+  p.num_acc_bufs = n_pad <= 112 ? 2 : 1;                    // 2 buffers x 2 accumulators x 112 columns = 448, metadata at 480
   // separate launches run one after the other and share the control words, flags and partial slots (the
   // partials then stay hot in L2); the fused kernel gives its down phase the second set (use_second_ws_half)
   uint8_t* ws = reinterpret_cast<uint8_t*>(d_ws);

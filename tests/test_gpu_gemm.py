@@ -47,6 +47,7 @@ GEMM_CASES = [
     (1024, 4096, 0.25, None, 64),   # enough stages for many spans / split-K partials
     (256, 1024, 0.25, None, 80),    # 64 < M <= 96: two accumulator buffers at a 96-column stride
     (1024, 4096, 0.25, None, 96),
+    (1024, 4096, 0.25, None, 112),  # 96 < M <= 112: two buffers at a 112-column stride (448 of the 480 columns below the metadata)
     (256, 1024, 0.25, None, 256),   # two full token blocks in one launch (weights re-read from L2 for the second)
     (1024, 4096, 0.25, None, 300),  # three token blocks, ragged last one, spans crossing block boundaries
     (640, 896, None, 384, 513),     # five blocks, last one holds a single token

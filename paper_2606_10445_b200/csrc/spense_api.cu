@@ -25,6 +25,7 @@ int check_device() {
   cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
   cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev);
   cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
+  if (g_num_sms > kMaxSpans) g_num_sms = kMaxSpans;   // persistent CTAs (all token blocks of a launch together) own fix-up slots 0..kMaxSpans-1
   g_arch_ok = (major == 10 && minor == 0) ? 1 : 0;
   if (g_arch_ok) {
     void* fn = nullptr;

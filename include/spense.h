@@ -22,8 +22,14 @@
  *     Device pointers must be 128-byte aligned.
  *   - Every call returns a status (0 = SPENSE_OK, negative = error).  Nothing throws, aborts or
  *     prints.  Argument errors are detected on the host before any launch.
- *   - All GPU work is enqueued on the caller's stream.  GEMM calls never synchronise.
+ *   - All GPU work is enqueued on the caller's stream.  GEMM calls never synchronise and never read device
+ *     memory on the host: the first call on a fresh blob may be issued inside a CUDA stream capture.
  *     spense_pack synchronises the stream once to read back its validation word.
+ *   - What only the device can see is reported through a pinned host status word (spense_device_status):
+ *     the blob header (magic, version, shape) is checked by the kernels that read the weight scales from it
+ *     (SPENSE_ERR_BAD_BLOB), and a CTA that waits more than 2 s for the other CTAs of its launch records
+ *     SPENSE_ERR_TIMEOUT and traps instead of hanging.  A recorded error is returned by every later GEMM call
+ *     until it is cleared.
  *   - There is NO CPU fallback: on a device that is not sm_100 the calls return SPENSE_ERR_ARCH.
  */
 #ifndef SPENSE_H_
@@ -49,7 +55,8 @@ enum {
   SPENSE_ERR_BAD_PERM = -7,         /* perm is not a bijection of [0, I) */
   SPENSE_ERR_ARCH = -8,             /* current device is not sm_100 */
   SPENSE_ERR_CUDA = -9,             /* a CUDA call failed; cudaGetLastError is preserved */
-  SPENSE_ERR_BAD_BLOB = -10         /* blob header does not match the shape / version */
+  SPENSE_ERR_BAD_BLOB = -10,        /* blob header does not match the shape / version (detected on the device) */
+  SPENSE_ERR_TIMEOUT = -11          /* a CTA gave up waiting for the other CTAs of its launch (detected on the device) */
 };
 
 enum { SPENSE_F32 = 0, SPENSE_BF16 = 1 };          /* y_dtype */
@@ -81,6 +88,11 @@ typedef struct {
 int spense_version(void);
 const char* spense_strerror(int status);
 
+/* The first error a kernel of an earlier launch recorded (SPENSE_OK if none): SPENSE_ERR_BAD_BLOB or
+ * SPENSE_ERR_TIMEOUT.  Host only; meaningful once the launches in question have completed (synchronise the
+ * stream first).  clear != 0 resets the word.                                                            */
+int spense_device_status(int clear);
+
 /* Host helper (Sec. 3.3.1; reading Q9): the permutation that moves the chosen dense
  * indices to the back, keeping ascending original order inside both regions.  h_perm[new] = old. */
 int spense_perm_from_dense_idx(int32_t I, const int32_t* h_dense_idx, int32_t n_dense, int32_t* h_perm);
@@ -108,9 +120,19 @@ int spense_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8
  * The workspace must be initialised ONCE with spense_workspace_init before its first use; every
  * launch advances the epoch word, so nothing needs resetting between calls or CUDA-graph replays.
  * One workspace must not be used by two streams concurrently.  The CTAs of one GEMM launch wait
- * for each other (split-K fix-up): the device must not be shared with other work that pins SMs.  */
+ * for each other (split-K fix-up): the calls refuse (SPENSE_ERR_CUDA) a grid the device cannot hold resident at
+ * once, and a launch starved of SMs by other work ends with SPENSE_ERR_TIMEOUT instead of hanging.          */
 int spense_workspace_size(const spense_shape_t* shape, int32_t M, size_t* bytes);
 int spense_workspace_init(void* d_ws, size_t ws_bytes, spense_stream_t stream);
+
+/* Launch geometry the library uses for (shape, M tokens, mode 0 = gate_up / 1 = down) on a device with `sms` SMs
+ * (host only, no device needed): the stream-K schedule cuts the linear sequence of weight stages (the byte order of
+ * the blob) into spans of equal cost, one persistent CTA (M <= 112) or CTA pair (M > 112) per span.  Writes
+ * n_spans + 1 span boundaries (linear stage indices) into span_begin (room for 161 ints) and returns n_spans, or a
+ * negative status.  info (nullable, 6 ints) = {stages, token blocks per launch, token columns per block, ring
+ * slots, token blocks, CTAs per span}.  Every CTA of a launch must be resident at the same time: the grid is
+ * info[1] * n_spans * info[5] CTAs at one CTA per SM.                                                       */
+int spense_schedule(const spense_shape_t* shape, int32_t M, int32_t mode, int32_t sms, int32_t* span_begin, int32_t* info);
 
 /* spense_gate_up -- output-split Spense GEMM for W_gate and W_up fused with the GLU
  * (Eq. 4, sigma = SiLU) and FP8 re-quantisation for the down projection:

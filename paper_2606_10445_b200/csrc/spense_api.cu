@@ -1,8 +1,7 @@
 // C-ABI entry points of libspense (include/spense.h): argument checking, stream-K schedule,
-// tensor-map creation and launches.  No device allocation, no synchronisation in the GEMM calls.
+// tensor-map creation and launches.  No device allocation, no synchronisation and no device reads in the GEMM calls.
 #include <cudaTypedefs.h>
 
-#include <cstdlib>
 #include <cstring>
 #include <deque>
 #include <mutex>
@@ -13,30 +12,51 @@
 namespace spense {
 namespace {
 
-int g_num_sms = 0;
-int g_arch_ok = -1;
+// ---- per-process / per-device state.  One entry per device ordinal; nothing assumes a single device.
+struct Device { int probed = 0, arch_ok = 0, sms = 0; };
+std::mutex g_dev_mu;
+Device g_dev[64];
 PFN_cuTensorMapEncodeTiled_v12000 g_encode = nullptr;
+int* g_status = nullptr;        // mapped pinned host word: the first device-side error (see spense_device_status)
+#ifdef SPENSE_DEBUG_HOOKS
+long long* g_trace = nullptr;   // debug: set by spense_debug_set_trace
+#endif
 
-int check_device() {
-  if (g_arch_ok >= 0) return g_arch_ok ? SPENSE_OK : SPENSE_ERR_ARCH;
+int check_device(int* dev_out, int* sms_out) {
   int dev = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess) return SPENSE_ERR_CUDA;
-  int major = 0, minor = 0;
-  cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
-  cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev);
-  cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
-  if (g_num_sms > kMaxSpans) g_num_sms = kMaxSpans;   // persistent CTAs (all token blocks of a launch together) own fix-up slots 0..kMaxSpans-1
-  g_arch_ok = (major == 10 && minor == 0) ? 1 : 0;
-  if (g_arch_ok) {
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return SPENSE_ERR_CUDA;
+  std::lock_guard<std::mutex> lk(g_dev_mu);
+  Device& d = g_dev[dev];
+  if (!d.probed) {
+    int major = 0, minor = 0;
+    cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev);
+    cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev);
+    if (d.sms > kMaxSpans) d.sms = kMaxSpans;   // the persistent CTAs of a launch own fix-up slots 0..kMaxSpans-1
+    d.arch_ok = (major == 10 && minor == 0) ? 1 : 0;
+    d.probed = 1;
+  }
+  if (!d.arch_ok) return SPENSE_ERR_ARCH;
+  if (!g_encode) {
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) {
-      g_arch_ok = -1;
-      return SPENSE_ERR_CUDA;
-    }
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) return SPENSE_ERR_CUDA;
     g_encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(fn);
   }
-  return g_arch_ok ? SPENSE_OK : SPENSE_ERR_ARCH;
+  if (!g_status) {
+    void* h = nullptr;
+    if (cudaHostAlloc(&h, 64, cudaHostAllocMapped | cudaHostAllocPortable) != cudaSuccess) return SPENSE_ERR_CUDA;
+    std::memset(h, 0, 64);
+    g_status = reinterpret_cast<int*>(h);
+  }
+  if (dev_out) *dev_out = dev;
+  if (sms_out) *sms_out = d.sms;
+  return SPENSE_OK;
+}
+
+// a device-side error recorded by an earlier launch (bad blob header, a CTA that gave up waiting for its peers)
+int pending_device_error() {
+  return g_status ? *reinterpret_cast<volatile int*>(g_status) : SPENSE_OK;
 }
 
 int check_shape(const spense_shape_t* s) {
@@ -49,30 +69,36 @@ int check_shape(const spense_shape_t* s) {
 
 bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
+// ---- launch geometry.
+// Up to kDecodeMaxTokens tokens: the decode kernel, one CTA per stream-K span, token columns = M padded to 16.
+// More: the wide kernel on CTA pairs; token blocks of at most kWideMaxTokens tokens, `par` blocks side by side in one
+// launch with pairs / par spans each (the CTAs of different blocks walk the same schedule, so a weight stage is read from
+// HBM once and found in L2 by the other blocks); more blocks than fit run as further launches.
+struct Plan {
+  bool wide;
+  int n_pad;      // token columns of one block
+  int nb;         // token blocks
+  int par;        // blocks per launch
+  int spans;      // stream-K spans per block (CTAs, or CTA pairs)
+  int ring;       // stage-ring slots
+  int slot_bytes;
+};
 
-size_t part_bytes_for(int n_pad, int spans) { return (size_t)spans * 2 * 2 * n_pad * 128 * sizeof(float); }
-// control words, flags, max|h| table, tile flags | partials of gate_up | partials of down (they may run concurrently)
-size_t ws_bytes_for(int n_pad, int spans) { return kWsFixedBytes + 2 * part_bytes_for(n_pad, spans); }
-
-double env_double(const char* name, double dflt) {
-  const char* v = std::getenv(name);
-  return v ? std::atof(v) : dflt;
+int ring_of(bool wide, int n_pad, int* slot_bytes) {
+  const int slot = wide ? kSparseOperandBytes + (n_pad / 2) * 256 : kSparseStageBytes + 2 * n_pad * 128;
+  const int stages = (kSmemMax - 1024 - 256 - 20 * n_pad) / slot;   // barriers + the scale tables
+  if (slot_bytes) *slot_bytes = slot;
+  return stages > 8 ? 8 : stages;
 }
 
-// Token columns of one MMA.  Up to 128 tokens: M padded to 16.  More: blocks of 128 tokens; a launch covers nb_par of
-// them side by side (grid = nb_par * k_par CTAs, k_par stream-K spans per block), so the CTAs of different blocks read
-// the same weight stage at about the same time: one HBM read, the other blocks hit L2.
-int block_tokens() { static const int b = (int)env_double("SPENSE_BLOCK_TOKENS", 128.0); return b == 96 ? 96 : 128; }
-int n_pad_of(int M) { return M > 128 ? block_tokens() : (M + 15) / 16 * 16; }
-int nb_of(int M) { return M > 128 ? (M + block_tokens() - 1) / block_tokens() : 1; }
-// how many of `nb` blocks one launch takes: the largest split within 5 % of the best SM occupancy over all rounds
+// how many of `nb` blocks one launch takes: the largest split within 5 % of the best occupancy over all rounds
 // (every round is a launch with its own start-up and fix-up tail, so fewer rounds win a near tie)
-int nb_par_of(int nb, int sms) {
+int par_of(int nb, int units) {
   auto eff = [&](int c) {
-    const int rounds = (nb + c - 1) / c, k = sms / c;
-    return (double)nb / (rounds * c) * ((double)(c * k) / sms);
+    const int rounds = (nb + c - 1) / c, k = units / c;
+    return (double)nb / (rounds * c) * ((double)(c * k) / units);
   };
-  const int cmax = nb < 32 ? (nb < sms ? nb : sms) : (32 < sms ? 32 : sms);
+  const int cmax = nb < 37 ? (nb < units ? nb : units) : (37 < units ? 37 : units);
   double best = 0;
   for (int c = 1; c <= cmax; ++c) best = eff(c) > best ? eff(c) : best;
   int pick = 1;
@@ -81,41 +107,60 @@ int nb_par_of(int nb, int sms) {
   return pick;
 }
 
-// ---- stream-K schedule: cut the stage sequence into n_spans spans of (nearly) equal bytes.
+Plan plan_of(int M, int sms) {
+  Plan pl = {};
+  if (M <= kDecodeMaxTokens) {
+    pl.wide = false;
+    pl.n_pad = (M + 15) / 16 * 16;
+    pl.nb = 1; pl.par = 1; pl.spans = sms;
+  } else {
+    pl.wide = true;
+    pl.nb = (M + kWideMaxTokens - 1) / kWideMaxTokens;
+    pl.n_pad = ((M + pl.nb - 1) / pl.nb + 15) / 16 * 16;
+    const int pairs = sms / 2;
+    pl.par = par_of(pl.nb, pairs);
+    pl.spans = pairs / pl.par;
+  }
+  pl.ring = ring_of(pl.wide, pl.n_pad, &pl.slot_bytes);
+  return pl;
+}
+
+// one partial tile: decode = both operands of the pair tile, wide = the CTA's operand; 2 per slot
+size_t part_floats_of(const Plan& pl) { return (size_t)(pl.wide ? 1 : 2) * pl.n_pad * 128; }
+size_t ws_bytes_for(int M) {
+  const size_t cols = M <= kDecodeMaxTokens ? 2 * (size_t)((M + 15) / 16 * 16) : (size_t)kWideMaxTokens;
+  return kWsFixedBytes + (size_t)kMaxSpans * 2 * cols * 128 * sizeof(float);
+}
+
+// ---- stream-K schedule: cut the stage sequence into n_spans spans of (nearly) equal cost.
 struct Schedule {
-  int mode, H, I, I_d, n_pad, sms, fused;
+  int mode, H, I, I_d, n_pad, spans_req, ring, wide;
   int n_spans;
   int span_begin[kMaxSpans + 1];
   uint32_t span_off[kMaxSpans];   // byte offset of the span's first stage image inside its section
   uint32_t span_pre[kMaxSpans];   // bytes of the stages the producer issues before anything else (one ring)
   uint32_t span_len[kMaxSpans];   // bytes of the whole span
-  double span_cost[kMaxSpans];    // modelled cost of the span (fused: down spans are sized to equalise gate_up + down)
 };
 
-int slot_bytes_of(int n_pad) { return kSparseStageBytes + 2 * n_pad * 128; }
-int ring_stages_of(int n_pad) {
-  const int stages = (kSmemMax - 1024 - 256 - 20 * n_pad) / slot_bytes_of(n_pad);   // barriers + the two scale tables
-  return stages > 8 ? 8 : stages;
-}
 std::mutex g_sched_mu;
 std::deque<Schedule> g_sched;   // deque: references handed out stay valid
 
-// fused = schedules of the single-launch MLP kernel (CTA b runs span n-1-b of gate_up AND of down):
-//   gate_up: span boundaries are nudged so that no tile is shared by more than two spans where a tile is not
-//            much longer than a span (a 3-way tile finishes last and every down span that reads it waits);
-//   down   : spans are sized so that gate_up cost + down cost is the same for every CTA.
-const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms, bool fused = false) {
-  const Schedule* gate = (fused && mode == 1) ? &get_schedule(0, g, n_pad, sms, true) : nullptr;
+const Schedule& get_schedule(int mode, const Geometry& g, const Plan& pl) {
   std::lock_guard<std::mutex> lk(g_sched_mu);
   for (const Schedule& s : g_sched)
-    if (s.mode == mode && s.H == g.H && s.I == g.I && s.I_d == g.I_d && s.n_pad == n_pad && s.sms == sms && s.fused == (int)fused) return s;
+    if (s.mode == mode && s.H == g.H && s.I == g.I && s.I_d == g.I_d && s.n_pad == pl.n_pad && s.spans_req == pl.spans &&
+        s.ring == pl.ring && s.wide == (int)pl.wide)
+      return s;
   Schedule sc = {};
-  sc.mode = mode; sc.H = g.H; sc.I = g.I; sc.I_d = g.I_d; sc.n_pad = n_pad; sc.sms = sms; sc.fused = fused;
+  sc.mode = mode; sc.H = g.H; sc.I = g.I; sc.I_d = g.I_d; sc.n_pad = pl.n_pad; sc.spans_req = pl.spans; sc.ring = pl.ring; sc.wide = pl.wide;
   // cost of a stage.  Every CTA keeps the same number of ring slots in flight, so under HBM contention a
   // stage costs one slot latency plus its bytes: measured on B200 (profiles/) a 40 KB sparse stage takes
   // ~1.12x a 32 KB dense one => fixed part ~36 KB-equivalents; activation bytes come from L2 and weigh less.
-  static const double fixed = env_double("SPENSE_SCHED_FIXED", 36864.0), gamma = env_double("SPENSE_SCHED_GAMMA", 0.25);
-  const double cs = fixed + kSparseStageBytes + gamma * 2.0 * n_pad * 128, cd = fixed + kDenseStageBytes + gamma * 1.0 * n_pad * 128;
+  // Wide token tiles are paced by the tensor pipe instead: a sparse stage (K 256) and a dense one (K 128) issue the
+  // same four MMAs.
+  const double fixed = 36864.0, gamma = 0.25;
+  const double cs = pl.wide ? 1.0 : fixed + kSparseStageBytes + gamma * 2.0 * pl.n_pad * 128;
+  const double cd = pl.wide ? 1.0 : fixed + kDenseStageBytes + gamma * 1.0 * pl.n_pad * 128;
   std::vector<double> cost;
   if (mode == 0) {
     cost.insert(cost.end(), (size_t)g.gu_tiles_sparse * g.gu_ns, cs);
@@ -127,30 +172,16 @@ const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms, bo
     }
   }
   const int total = (int)cost.size();
-  int spans = sms < kMaxSpans ? sms : kMaxSpans;
+  int spans = pl.spans < kMaxSpans ? pl.spans : kMaxSpans;
   if (spans > total) spans = total;
   double sum = 0;
   for (double c : cost) sum += c;
   sc.n_spans = spans;
-  // cumulative share of the cost each span should end at: equal, or (fused down) what is left of an equal
-  // share of gate_up + down after the CTA's gate_up span
-  std::vector<double> cum(spans + 1, 0.0);
-  for (int i = 1; i <= spans; ++i) cum[i] = (double)i / spans;
-  if (gate && gate->n_spans == spans) {
-    double gsum = 0;
-    for (int i = 0; i < spans; ++i) gsum += gate->span_cost[i];
-    const double share = (gsum + sum) / spans;
-    double tot = 0;
-    std::vector<double> w(spans);
-    for (int i = 0; i < spans; ++i) { w[i] = share - gate->span_cost[i]; if (w[i] < 0.25 * sum / spans) w[i] = 0.25 * sum / spans; tot += w[i]; }
-    double run = 0;
-    for (int i = 0; i < spans; ++i) { run += w[i]; cum[i + 1] = run / tot; }
-  }
   double acc = 0;
   int s = 0;
   sc.span_begin[0] = 0;
   for (int i = 1; i < spans; ++i) {
-    const double target = sum * cum[i];
+    const double target = sum * (double)i / spans;
     while (s < total && acc + 0.5 * cost[s] < target) acc += cost[s++];
     int b = s;
     if (b <= sc.span_begin[i - 1]) b = sc.span_begin[i - 1] + 1;     // every span owns >= 1 stage
@@ -159,30 +190,6 @@ const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms, bo
     sc.span_begin[i] = b;
   }
   sc.span_begin[spans] = total;
-  if (fused && mode == 0) {
-    // a span lying strictly inside a tile makes the tile 3-way: stretch it to the nearer tile boundary
-    int tf = 0;
-    for (int t = 0; t < g.gu_tiles; ++t) {
-      const int per = t < g.gu_tiles_sparse ? g.gu_ns : g.gu_nd;
-      const int te = tf + per;
-      if (per < 2 * total / spans) {
-        for (int m = 1; m + 1 < spans; ++m) {
-          if (sc.span_begin[m] > tf && sc.span_begin[m + 1] < te) {
-            const int head = sc.span_begin[m] - tf, tail = te - sc.span_begin[m + 1];
-            if (head <= tail && sc.span_begin[m - 1] < tf) sc.span_begin[m] = tf;
-            else if (sc.span_begin[m + 2] > te) sc.span_begin[m + 1] = te;
-            else if (sc.span_begin[m - 1] < tf) sc.span_begin[m] = tf;
-          }
-        }
-      }
-      tf = te;
-    }
-  }
-  for (int i = 0; i < spans; ++i) {
-    double c = 0;
-    for (int k = sc.span_begin[i]; k < sc.span_begin[i + 1]; ++k) c += cost[k];
-    sc.span_cost[i] = c;
-  }
   // byte offsets: the blob stores the stage images in exactly this linear order
   std::vector<uint32_t> bytes(total);
   if (mode == 0) {
@@ -191,14 +198,13 @@ const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms, bo
     const int per = g.dn_ns + g.dn_nd;
     for (int i = 0; i < total; ++i) bytes[i] = (i % per) < g.dn_ns ? kSparseStageBytes : kDenseStageBytes;
   }
-  const int ring = ring_stages_of(n_pad);
   uint64_t off = 0;
   int st = 0;
   for (int i = 0; i < spans; ++i) {
     while (st < sc.span_begin[i]) off += bytes[st++];
     sc.span_off[i] = (uint32_t)off;
     uint32_t pre = 0;
-    for (int k = sc.span_begin[i]; k < sc.span_begin[i + 1] && k < sc.span_begin[i] + ring; ++k) pre += bytes[k];
+    for (int k = sc.span_begin[i]; k < sc.span_begin[i + 1] && k < sc.span_begin[i] + pl.ring; ++k) pre += bytes[k];
     sc.span_pre[i] = pre;
     uint32_t len = 0;
     for (int k = sc.span_begin[i]; k < sc.span_begin[i + 1]; ++k) len += bytes[k];
@@ -208,6 +214,7 @@ const Schedule& get_schedule(int mode, const Geometry& g, int n_pad, int sms, bo
   return g_sched.back();
 }
 
+// uint8 tensor [rows, K] row-major; box = 128 bytes of K x box_rows rows, 128-byte swizzle (activation tiles)
 int make_tmap(CUtensorMap* map, const uint8_t* base, int K, int rows, int box_rows) {
   cuuint64_t dims[2] = {(cuuint64_t)K, (cuuint64_t)rows};
   cuuint64_t strides[1] = {(cuuint64_t)K};
@@ -219,90 +226,69 @@ int make_tmap(CUtensorMap* map, const uint8_t* base, int K, int rows, int box_ro
   return r == CUDA_SUCCESS ? SPENSE_OK : SPENSE_ERR_CUDA;
 }
 
-// header cache: one D2H copy per (blob pointer), so the GEMM calls stay asynchronous afterwards
-struct HeaderEntry { const void* p; BlobHeader h; };
-std::mutex g_hdr_mu;
-std::vector<HeaderEntry> g_hdr_cache;
-
-void forget_header(const void* d_blob) {
-  std::lock_guard<std::mutex> lk(g_hdr_mu);
-  for (size_t i = 0; i < g_hdr_cache.size(); ++i)
-    if (g_hdr_cache[i].p == d_blob) { g_hdr_cache.erase(g_hdr_cache.begin() + i); break; }
-}
-
-int read_header(const void* d_blob, const spense_shape_t* shape, BlobHeader* out) {
-  std::mutex& mu = g_hdr_mu;
-  std::vector<HeaderEntry>& cache = g_hdr_cache;
-  using Entry = HeaderEntry;
-  {
-    std::lock_guard<std::mutex> lk(mu);
-    for (const Entry& e : cache)
-      if (e.p == d_blob && e.h.H == shape->H && e.h.I == shape->I && e.h.I_dense == shape->I_dense) { *out = e.h; return SPENSE_OK; }
-  }
-  BlobHeader h;
-  if (cudaMemcpy(&h, d_blob, sizeof(h), cudaMemcpyDeviceToHost) != cudaSuccess) return SPENSE_ERR_CUDA;
-  if (h.magic != kBlobMagic || h.version != kBlobVersion || h.H != shape->H || h.I != shape->I || h.I_dense != shape->I_dense)
-    return SPENSE_ERR_BAD_BLOB;
-  std::lock_guard<std::mutex> lk(mu);
-  for (Entry& e : cache)
-    if (e.p == d_blob) { e.h = h; *out = h; return SPENSE_OK; }
-  cache.push_back({d_blob, h});
-  *out = h;
-  return SPENSE_OK;
+// a blob section seen as rows of 128 bytes; box = one operand of a stage image (already swizzled: plain copy).  Lets a
+// CTA of a pair fetch its operand with a tensor copy whose completion counts on the LEADER CTA's barrier.
+int make_tmap_section(CUtensorMap* map, const uint8_t* base, size_t bytes, int box_rows) {
+  cuuint64_t dims[2] = {128u, (cuuint64_t)(bytes / 128)};
+  cuuint64_t strides[1] = {128u};
+  cuuint32_t box[2] = {128u, (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1u, 1u};
+  CUresult r = g_encode(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<uint8_t*>(base), dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? SPENSE_OK : SPENSE_ERR_CUDA;
 }
 
 // bytes of span k that the PREVIOUS launch pulls into L2 during its tail: at least one ring
+constexpr uint32_t kPfNextBytes = 640u * 1024u, kPfSelfBytes = 160u * 1024u;
+constexpr int kPfPaceNs = 750;
 uint32_t next_prefetch_bytes(const Schedule& sc, int k) {
-  static const uint32_t want = (uint32_t)(env_double("SPENSE_PF_NEXT_KB", 640.0) * 1024.0);
-  uint32_t n = sc.span_pre[k] > want ? sc.span_pre[k] : want;
+  uint32_t n = sc.span_pre[k] > kPfNextBytes ? sc.span_pre[k] : kPfNextBytes;
   return n < sc.span_len[k] ? n : sc.span_len[k];
 }
 
-int g_fused = -1;               // spense_mlp as ONE persistent launch (SPENSE_FUSED / spense_debug_set_fused); -1 = read the environment
-long long* g_trace = nullptr;   // debug: set by spense_debug_set_trace (not part of the public ABI)
-
-void fill_common(GemmParams& p, const Schedule& sc, int M, int n_pad, void* d_ws) {
+void fill_common(GemmParams& p, const Schedule& sc, const Plan& pl, const spense_shape_t* shape, const void* d_blob, int M, void* d_ws) {
+#ifdef SPENSE_DEBUG_HOOKS
   p.trace = g_trace;
   if (g_trace) g_trace += (size_t)kMaxSpans * 16;   // debug: consecutive launches fill consecutive timelines
+#endif
+  p.hdr = reinterpret_cast<const BlobHeader*>(d_blob);
+  p.H = shape->H; p.I = shape->I; p.I_d = shape->I_dense;
+  p.status = g_status;
   p.n_spans = sc.n_spans;
   std::memcpy(p.span_begin, sc.span_begin, sizeof(int) * (sc.n_spans + 1));
-  static const uint32_t self_want = (uint32_t)(env_double("SPENSE_PF_SELF_KB", 160.0) * 1024.0);
-  for (int i = 0; i < sc.n_spans; ++i) {                    // own stages pulled into L2 while waiting for the previous kernel
-    const uint32_t from = next_prefetch_bytes(sc, i);
-    const uint32_t left = sc.span_len[i] - from;
-    p.self_off[i] = from - sc.span_pre[i];
-    p.self_len[i] = self_want < left ? self_want : left;
+  if (!pl.wide) {
+    for (int i = 0; i < sc.n_spans; ++i) {                    // own stages pulled into L2 while waiting for the previous kernel
+      const uint32_t from = next_prefetch_bytes(sc, i);
+      const uint32_t left = sc.span_len[i] - from;
+      p.self_off[i] = from - sc.span_pre[i];
+      p.self_len[i] = kPfSelfBytes < left ? kPfSelfBytes : left;
+    }
   }
   p.nb = 1;
   p.blk0 = 0;
   p.M = M;
-  p.n_pad = n_pad;
-  p.slot_bytes = slot_bytes_of(n_pad);
-  p.num_stages = ring_stages_of(n_pad);
-  p.acc_stride = n_pad <= 32 ? 32 : (n_pad <= 64 ? 64 : (n_pad <= 96 ? 96 : (n_pad <= 112 ? 112 : 128)));
-  p.num_acc_bufs = n_pad <= 112 ? 2 : 1;                    // 2 buffers x 2 accumulators x 112 columns = 448, metadata at 480
-  // separate launches run one after the other and share the control words, flags and partial slots (the
-  // partials then stay hot in L2); the fused kernel gives its down phase the second set (use_second_ws_half)
+  p.n_pad = pl.n_pad;
+  p.slot_bytes = pl.slot_bytes;
+  p.num_stages = pl.ring;
+  if (pl.wide) {
+    p.acc_stride = kWideMaxTokens;                            // 2 buffers x 240 columns, metadata at 480
+    p.num_acc_bufs = 2;
+  } else {
+    p.acc_stride = pl.n_pad <= 32 ? 32 : (pl.n_pad <= 64 ? 64 : (pl.n_pad <= 96 ? 96 : 112));
+    p.num_acc_bufs = 2;                                       // 2 buffers x 2 accumulators x 112 columns = 448, metadata at 480
+  }
   uint8_t* ws = reinterpret_cast<uint8_t*>(d_ws);
   p.ws_ctrl = reinterpret_cast<int*>(ws);
   p.flags = reinterpret_cast<int*>(ws + 128);
   p.partials = reinterpret_cast<float*>(ws + kWsFixedBytes);
 }
 
-void use_second_ws_half(GemmParams& p, void* d_ws) {
-  uint8_t* ws = reinterpret_cast<uint8_t*>(d_ws);
-  p.ws_ctrl = reinterpret_cast<int*>(ws) + 2;
-  p.flags = reinterpret_cast<int*>(ws + 128 + kMaxSpans * 2 * sizeof(int));
-  p.partials = reinterpret_cast<float*>(ws + kWsFixedBytes + part_bytes_for(p.n_pad, kMaxSpans));
-}
-
 // L2 prefetch hint: while this launch runs its fix-up tail, pull what the next launch streams first.
 void fill_next(GemmParams& p, const uint8_t* next_section, const Schedule& next) {
-  static const bool enabled = env_double("SPENSE_L2_PREFETCH", 1.0) != 0.0;
-  if (!enabled || !next_section) return;
+  if (!next_section) return;
   p.next_base = next_section;
-  static const int pace = (int)env_double("SPENSE_PF_PACE_NS", 750.0);
-  p.pf_pace_ns = pace;
+  p.pf_pace_ns = kPfPaceNs;
   for (int i = 0; i < p.n_spans; ++i) {
     const int k = i < next.n_spans ? i : next.n_spans - 1;
     p.next_off[i] = next.span_off[k];
@@ -310,113 +296,100 @@ void fill_next(GemmParams& p, const uint8_t* next_section, const Schedule& next)
   }
 }
 
-// parameter block + tensor map of one gate_up launch over tokens [m0, m0 + Mb)
-int gate_up_params(const Geometry& g, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_x, const float* d_sx,
-                   int m0, int Mb, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32, void* d_ws,
-                   bool dynamic, GemmParams& p, CUtensorMap& tm, bool fused = false, int k_par = 0, int nb_launch = 1,
-                   int blk0 = 0) {
-  const int n_pad = n_pad_of(Mb);
-  const Schedule& sc = get_schedule(0, g, n_pad, k_par > 0 ? k_par : g_num_sms, fused);
-  p = GemmParams{};
-  fill_common(p, sc, Mb, n_pad, d_ws);
-  p.nb = nb_launch; p.blk0 = blk0;
-  p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.gate_up_off;
-  p.mode = 0;
-  p.num_tiles = g.gu_tiles; p.tiles_sparse = g.gu_tiles_sparse;
-  p.ns = g.gu_ns; p.nd = g.gu_nd; p.dense_k0 = 0;
-  p.s_act = d_sx + m0;
-  p.s_h = d_sh + (size_t)m0 * sh_stride; p.sh_stride = sh_stride;
-  p.w_scale0 = hdr.w_scale[0]; p.w_scale1 = hdr.w_scale[1];
-  p.hq = d_hq + (size_t)m0 * g.I;
-  p.h_f32 = d_h_f32 ? d_h_f32 + (size_t)m0 * g.I : nullptr;
-  p.amax_part = dynamic ? reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes) : nullptr;
-  p.ld_out = g.I; p.out_rows = g.I;
-  return make_tmap(&tm, d_x + (size_t)m0 * g.H, g.H, Mb, n_pad);
-}
+struct Launch { int dev, sms; };
 
-int down_params(const Geometry& g, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_hq, const float* d_sh,
-                int32_t sh_stride, int m0, int Mb, void* d_y, int32_t y_dtype, void* d_ws, GemmParams& p, CUtensorMap& tm,
-                bool fused = false, int k_par = 0, int nb_launch = 1, int blk0 = 0) {
-  const size_t esz = y_dtype == SPENSE_F32 ? 4 : 2;
-  const int n_pad = n_pad_of(Mb);
-  const Schedule& sc = get_schedule(1, g, n_pad, k_par > 0 ? k_par : g_num_sms, fused);
-  p = GemmParams{};
-  fill_common(p, sc, Mb, n_pad, d_ws);
-  p.nb = nb_launch; p.blk0 = blk0;
-  p.section = reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off;
-  p.mode = 1;
-  p.num_tiles = g.dn_tiles; p.tiles_sparse = 0;
-  p.ns = g.dn_ns; p.nd = g.dn_nd; p.dense_k0 = g.I_s;
-  p.s_act = d_sh + (size_t)m0 * sh_stride; p.sh_stride = sh_stride;
-  p.w_scale0 = hdr.w_scale[2]; p.w_scale1 = hdr.w_scale[2];
-  p.y = reinterpret_cast<uint8_t*>(d_y) + (size_t)m0 * g.H * esz;
-  p.y_dtype = y_dtype;
-  p.ld_out = g.H; p.out_rows = g.H;
-  return make_tmap(&tm, d_hq + (size_t)m0 * g.I, g.I, Mb, n_pad);
-}
-
-int gate_up_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_x,
-                 const float* d_sx, int32_t M, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32,
-                 void* d_ws, bool pdl, bool down_follows, cudaStream_t stream, bool dynamic = false) {
+// gate_up over all M tokens (one or several launches); dynamic: h stays in fp32, max|h| per slot goes to the workspace
+int gate_up_impl(const Launch& L, const spense_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx, int32_t M,
+                 const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32, void* d_ws, bool pdl, bool down_follows,
+                 cudaStream_t stream, bool dynamic = false, float* d_sh_out = nullptr) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const int nb = nb_of(M), par = nb_par_of(nb, g_num_sms);
-  for (int blk0 = 0; blk0 < nb; blk0 += par) {               // M <= 128: one launch of one block
-    const int nb_l = nb - blk0 < par ? nb - blk0 : par;
-    GemmParams p;
-    CUtensorMap tm;
-    int st = gate_up_params(g, hdr, d_blob, d_x, d_sx, 0, M, d_sh, sh_stride, d_hq, d_h_f32, d_ws, dynamic, p, tm, false,
-                            g_num_sms / nb_l, nb_l, blk0);
+  const Plan pl = plan_of(M, L.sms);
+  const Schedule& sc = get_schedule(0, g, pl);
+  const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + g.gate_up_off;
+  CUtensorMap tm, tws, twd;
+  int st = make_tmap(&tm, d_x, g.H, M, pl.wide ? pl.n_pad / 2 : pl.n_pad);
+  if (st) return st;
+  if (pl.wide) {
+    st = make_tmap_section(&tws, section, g.down_off - g.gate_up_off, kSparseOperandBytes / 128);
+    if (!st) st = make_tmap_section(&twd, section, g.down_off - g.gate_up_off, kOperandBytes / 128);
     if (st) return st;
-    if (down_follows && nb == 1)                             // the same layer's down projection streams next
-      fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + hdr.down_off, get_schedule(1, g, n_pad_of(M), g_num_sms));
-    st = launch_gemm(p, tm, pdl, stream);
+  }
+  for (int blk0 = 0; blk0 < pl.nb; blk0 += pl.par) {
+    GemmParams p = {};
+    fill_common(p, sc, pl, shape, d_blob, M, d_ws);
+    p.nb = pl.nb - blk0 < pl.par ? pl.nb - blk0 : pl.par;
+    p.blk0 = blk0;
+    p.section = section;
+    p.mode = 0;
+    p.num_tiles = g.gu_tiles; p.tiles_sparse = g.gu_tiles_sparse;
+    p.ns = g.gu_ns; p.nd = g.gu_nd; p.dense_k0 = 0;
+    p.s_act = d_sx;
+    p.s_h = d_sh; p.sh_stride = sh_stride;
+    p.scale0 = 0; p.scale1 = 1;
+    p.hq = d_hq;
+    p.h_f32 = d_h_f32;
+    p.amax_part = dynamic ? reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes) : nullptr;
+    p.ld_out = g.I; p.out_rows = g.I;
+    if (!pl.wide) {
+      if (down_follows)                                        // the same layer's down projection streams next
+        fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + g.down_off, get_schedule(1, g, pl));
+      st = launch_gemm(p, tm, pdl, L.dev, L.sms, stream);
+    } else {
+      st = launch_gemm_wide(p, tm, tws, twd, pdl, L.dev, L.sms, stream);
+    }
     if (st) return st;
+    if (dynamic) {
+      // rows of this launch: s_h = max over the block's slots / 448, Hq = E4M3(h / s_h)
+      const int m0 = blk0 * pl.n_pad;
+      const int rows = (M - m0) < p.nb * pl.n_pad ? (M - m0) : p.nb * pl.n_pad;
+      const int slots_per_block = pl.wide ? 2 * sc.n_spans : sc.n_spans;
+      st = launch_requant_rows(d_h_f32 + (size_t)m0 * g.I, rows, g.I, p.amax_part, slots_per_block, pl.n_pad, pl.n_pad,
+                               d_hq + (size_t)m0 * g.I, d_sh_out + m0, stream);
+      if (st) return st;
+    }
   }
   return SPENSE_OK;
 }
 
-int down_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_hq,
-              const float* d_sh, int32_t sh_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, bool pdl,
-              const void* d_next_blob, cudaStream_t stream) {
+int down_impl(const Launch& L, const spense_shape_t* shape, const void* d_blob, const uint8_t* d_hq, const float* d_sh,
+              int32_t sh_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, bool pdl, const void* d_next_blob,
+              cudaStream_t stream) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const int nb = nb_of(M), par = nb_par_of(nb, g_num_sms);
-  for (int blk0 = 0; blk0 < nb; blk0 += par) {
-    const int nb_l = nb - blk0 < par ? nb - blk0 : par;
-    GemmParams p;
-    CUtensorMap tm;
-    int st = down_params(g, hdr, d_blob, d_hq, d_sh, sh_stride, 0, M, d_y, y_dtype, d_ws, p, tm, false, g_num_sms / nb_l, nb_l, blk0);
+  const Plan pl = plan_of(M, L.sms);
+  const Schedule& sc = get_schedule(1, g, pl);
+  const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + g.down_off;
+  CUtensorMap tm, tws, twd;
+  int st = make_tmap(&tm, d_hq, g.I, M, pl.wide ? pl.n_pad / 2 : pl.n_pad);
+  if (st) return st;
+  if (pl.wide) {
+    st = make_tmap_section(&tws, section, g.total_bytes - g.down_off, kSparseOperandBytes / 128);
+    if (!st) st = make_tmap_section(&twd, section, g.total_bytes - g.down_off, kOperandBytes / 128);
     if (st) return st;
-    if (d_next_blob && nb == 1)                              // the next layer's gate/up weights stream next
-      fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + hdr.gate_up_off, get_schedule(0, g, n_pad_of(M), g_num_sms));
-    st = launch_gemm(p, tm, pdl, stream);
+  }
+  for (int blk0 = 0; blk0 < pl.nb; blk0 += pl.par) {
+    GemmParams p = {};
+    fill_common(p, sc, pl, shape, d_blob, M, d_ws);
+    p.nb = pl.nb - blk0 < pl.par ? pl.nb - blk0 : pl.par;
+    p.blk0 = blk0;
+    p.section = section;
+    p.mode = 1;
+    p.num_tiles = g.dn_tiles; p.tiles_sparse = 0;
+    p.ns = g.dn_ns; p.nd = g.dn_nd; p.dense_k0 = g.I_s;
+    p.s_act = d_sh; p.sh_stride = sh_stride;
+    p.scale0 = 2; p.scale1 = 2;
+    p.y = d_y;
+    p.y_dtype = y_dtype;
+    p.ld_out = g.H; p.out_rows = g.H;
+    if (!pl.wide) {
+      if (d_next_blob)                                         // the next layer's gate/up weights stream next
+        fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + g.gate_up_off, get_schedule(0, g, pl));
+      st = launch_gemm(p, tm, pdl, L.dev, L.sms, stream);
+    } else {
+      st = launch_gemm_wide(p, tm, tws, twd, pdl, L.dev, L.sms, stream);
+    }
     if (st) return st;
   }
   return SPENSE_OK;
-}
-
-// One token block: gate_up and down as ONE persistent launch (spense_mlp_kernel); down's Hq loads are gated per
-// 128-column tile by flags gate_up publishes, no grid-wide barrier in between.
-int mlp_fused_impl(const spense_shape_t* shape, const BlobHeader& hdr, const void* d_blob, const uint8_t* d_x,
-                   const float* d_sx, int32_t M, const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32,
-                   void* d_y, int32_t y_dtype, void* d_ws, const void* d_next_blob, cudaStream_t stream) {
-  const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  GemmParams pg, pd;
-  CUtensorMap tx, th;
-  int st = gate_up_params(g, hdr, d_blob, d_x, d_sx, 0, M, d_sh, sh_stride, d_hq, d_h_f32, d_ws, false, pg, tx, true);
-  if (st) return st;
-  st = down_params(g, hdr, d_blob, d_hq, d_sh, sh_stride, 0, M, d_y, y_dtype, d_ws, pd, th, true);
-  if (st) return st;
-  use_second_ws_half(pd, d_ws);
-  int* dep = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes + kAmaxBytes);
-  pg.tile_flags = dep;
-  pg.tile_cnt = dep + kDepInts;
-  pd.dep_flags = dep;
-  pd.dep_done = reinterpret_cast<int*>(d_ws) + kCtrlDepDone;
-  pd.dep_tiles = g.gu_tiles;
-  { static const uint32_t pfb = (uint32_t)(env_double("SPENSE_PF_GATED_KB", 256.0) * 1024.0); pd.gated_pf_bytes = pfb; }
-  if (d_next_blob)                                           // the next layer's gate/up weights stream next
-    fill_next(pd, reinterpret_cast<const uint8_t*>(d_next_blob) + hdr.gate_up_off, get_schedule(0, g, n_pad_of(M), g_num_sms, true));
-  return launch_mlp(pg, tx, pd, th, stream);
 }
 
 int check_ws(const spense_shape_t* shape, int M, const void* d_ws, size_t ws_bytes) {
@@ -428,6 +401,15 @@ int check_ws(const spense_shape_t* shape, int M, const void* d_ws, size_t ws_byt
   return ws_bytes < need ? SPENSE_ERR_BUFFER_TOO_SMALL : SPENSE_OK;
 }
 
+// what every GEMM entry point does before it launches
+int enter(const spense_shape_t* shape, int M, const void* d_ws, size_t ws_bytes, Launch* L) {
+  int st = check_ws(shape, M, d_ws, ws_bytes);
+  if (st) return st;
+  st = check_device(&L->dev, &L->sms);
+  if (st) return st;
+  return pending_device_error();
+}
+
 }  // namespace
 }  // namespace spense
 
@@ -435,36 +417,12 @@ using namespace spense;
 
 extern "C" {
 
-int spense_version(void) { return 100 * 0 + 1; }
+int spense_version(void) { return 2; }
 
-// debug hook (undeclared in spense.h): run spense_mlp (M <= 128) as the fused single-launch kernel (1) or as two
-// PDL-chained launches (0, the default: measured 55.5 vs 57.4 us/layer at M=64)
-void spense_debug_set_fused(int on) { g_fused = on ? 1 : 0; }
-
-// debug hook (undeclared in spense.h; host only, no device needed): the stream-K schedule the library would use
-// for (shape, M, mode 0 gate_up / 1 down, fused, sms).  Writes n_spans + 1 span boundaries (linear stage indices)
-// into out_span_begin (room for 161 ints) and returns n_spans, or a negative status.  out_info[0..3] = total
-// stages, token blocks per launch, token columns per MMA, ring slots.
-int spense_debug_schedule(const spense_shape_t* shape, int32_t M, int32_t mode, int32_t fused, int32_t sms,
-                          int32_t* out_span_begin, int32_t* out_info) {
-  int st = check_shape(shape);
-  if (st) return st;
-  if (M < 1 || M > kMaxTokens || (mode != 0 && mode != 1) || sms < 1 || !out_span_begin) return SPENSE_ERR_ARG;
-  const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const int n_pad = n_pad_of(M), nb = nb_of(M), par = nb_par_of(nb, sms);
-  const Schedule& sc = get_schedule(mode, g, n_pad, sms / par, fused != 0 && nb == 1);
-  for (int i = 0; i <= sc.n_spans; ++i) out_span_begin[i] = sc.span_begin[i];
-  if (out_info) {
-    out_info[0] = sc.span_begin[sc.n_spans];
-    out_info[1] = par;                                       // token blocks side by side in one launch
-    out_info[2] = n_pad;
-    out_info[3] = ring_stages_of(n_pad);
-  }
-  return sc.n_spans;
-}
-
-// debug hook (undeclared in spense.h): per-CTA globaltimer timeline, 16 int64 per span, of the next launches
+#ifdef SPENSE_DEBUG_HOOKS
+// debug hook (SPENSE_DEBUG_HOOKS builds only): per-CTA globaltimer timeline, 16 int64 per span, of the next launches
 void spense_debug_set_trace(void* d_buf) { g_trace = reinterpret_cast<long long*>(d_buf); }
+#endif
 
 const char* spense_strerror(int status) {
   switch (status) {
@@ -479,8 +437,34 @@ const char* spense_strerror(int status) {
     case SPENSE_ERR_ARCH: return "device is not sm_100 (no fallback path exists)";
     case SPENSE_ERR_CUDA: return "CUDA error";
     case SPENSE_ERR_BAD_BLOB: return "blob header does not match";
+    case SPENSE_ERR_TIMEOUT: return "a CTA gave up waiting for the other CTAs of its launch (device shared with other work?)";
     default: return "unknown status";
   }
+}
+
+int spense_device_status(int clear) {
+  const int st = pending_device_error();
+  if (clear && g_status) *reinterpret_cast<volatile int*>(g_status) = 0;
+  return st;
+}
+
+int spense_schedule(const spense_shape_t* shape, int32_t M, int32_t mode, int32_t sms, int32_t* out_span_begin, int32_t* out_info) {
+  int st = check_shape(shape);
+  if (st) return st;
+  if (M < 1 || M > kMaxTokens || (mode != 0 && mode != 1) || sms < 2 || sms > kMaxSpans || !out_span_begin) return SPENSE_ERR_ARG;
+  const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
+  const Plan pl = plan_of(M, sms);
+  const Schedule& sc = get_schedule(mode, g, pl);
+  for (int i = 0; i <= sc.n_spans; ++i) out_span_begin[i] = sc.span_begin[i];
+  if (out_info) {
+    out_info[0] = sc.span_begin[sc.n_spans];
+    out_info[1] = pl.par;
+    out_info[2] = pl.n_pad;
+    out_info[3] = pl.ring;
+    out_info[4] = pl.nb;
+    out_info[5] = pl.wide ? 2 : 1;
+  }
+  return sc.n_spans;
 }
 
 int spense_perm_from_dense_idx(int32_t I, const int32_t* h_dense_idx, int32_t n_dense, int32_t* h_perm) {
@@ -518,9 +502,8 @@ int spense_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8
   size_t need_blob = 0, need_ws = 0;
   spense_pack_sizes(shape, &need_blob, &need_ws);
   if (blob_bytes < need_blob || ws_bytes < need_ws) return SPENSE_ERR_BUFFER_TOO_SMALL;
-  st = check_device();
+  st = check_device(nullptr, nullptr);
   if (st) return st;
-  forget_header(d_blob);
   return launch_pack(shape, d_wgate, d_wup, d_wdown, h_w_scale, d_perm, d_blob, canon, d_ws, h_err_where,
                      reinterpret_cast<cudaStream_t>(stream));
 }
@@ -529,7 +512,7 @@ int spense_workspace_size(const spense_shape_t* shape, int32_t M, size_t* bytes)
   int st = check_shape(shape);
   if (st) return st;
   if (M < 1 || M > kMaxTokens || !bytes) return SPENSE_ERR_ARG;
-  *bytes = ws_bytes_for(M > 128 ? 128 : n_pad_of(M), kMaxSpans);
+  *bytes = ws_bytes_for(M);
   return SPENSE_OK;
 }
 
@@ -548,14 +531,10 @@ int spense_gate_up(const spense_shape_t* shape, const void* d_blob, const uint8_
   if (!aligned(d_blob, 128) || !aligned(d_x, 128) || !aligned(d_hq, 16) || !aligned(d_sx, 4) || !aligned(d_sh, 4) ||
       (d_h_f32 && !aligned(d_h_f32, 16)))
     return SPENSE_ERR_ALIGN;
-  st = check_ws(shape, M, d_ws, ws_bytes);
+  Launch L;
+  st = enter(shape, M, d_ws, ws_bytes, &L);
   if (st) return st;
-  st = check_device();
-  if (st) return st;
-  BlobHeader hdr;
-  st = read_header(d_blob, shape, &hdr);
-  if (st) return st;
-  return gate_up_impl(shape, hdr, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq, d_h_f32, d_ws, false, false,
+  return gate_up_impl(L, shape, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq, d_h_f32, d_ws, false, false,
                       reinterpret_cast<cudaStream_t>(stream));
 }
 
@@ -569,14 +548,10 @@ int spense_down(const spense_shape_t* shape, const void* d_blob, const uint8_t* 
     return SPENSE_ERR_ARG;
   if (!aligned(d_blob, 128) || !aligned(d_hq, 128) || !aligned(d_y, 16) || !aligned(d_sh, 4) || !aligned(d_next_blob, 128))
     return SPENSE_ERR_ALIGN;
-  st = check_ws(shape, M, d_ws, ws_bytes);
+  Launch L;
+  st = enter(shape, M, d_ws, ws_bytes, &L);
   if (st) return st;
-  st = check_device();
-  if (st) return st;
-  BlobHeader hdr;
-  st = read_header(d_blob, shape, &hdr);
-  if (st) return st;
-  return down_impl(shape, hdr, d_blob, d_hq, d_sh, sh_stride, M, d_y, y_dtype, d_ws, false, d_next_blob,
+  return down_impl(L, shape, d_blob, d_hq, d_sh, sh_stride, M, d_y, y_dtype, d_ws, false, d_next_blob,
                    reinterpret_cast<cudaStream_t>(stream));
 }
 
@@ -591,21 +566,13 @@ int spense_mlp(const spense_shape_t* shape, const void* d_blob, const uint8_t* d
   if (!aligned(d_blob, 128) || !aligned(d_x, 128) || !aligned(d_hq_scratch, 128) || !aligned(d_y, 16) ||
       !aligned(d_sx, 4) || !aligned(d_sh, 4) || (d_h_f32 && !aligned(d_h_f32, 16)) || !aligned(d_next_blob, 128))
     return SPENSE_ERR_ALIGN;
-  st = check_ws(shape, M, d_ws, ws_bytes);
-  if (st) return st;
-  st = check_device();
-  if (st) return st;
-  BlobHeader hdr;
-  st = read_header(d_blob, shape, &hdr);
+  Launch L;
+  st = enter(shape, M, d_ws, ws_bytes, &L);
   if (st) return st;
   cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
-  if (g_fused < 0) g_fused = env_double("SPENSE_FUSED", 0.0) != 0.0 ? 1 : 0;
-  if (g_fused && M <= 128)
-    return mlp_fused_impl(shape, hdr, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq_scratch, d_h_f32, d_y, y_dtype, d_ws,
-                          d_next_blob, s);
-  st = gate_up_impl(shape, hdr, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq_scratch, d_h_f32, d_ws, true, true, s);
+  st = gate_up_impl(L, shape, d_blob, d_x, d_sx, M, d_sh, sh_stride, d_hq_scratch, d_h_f32, d_ws, true, true, s);
   if (st) return st;
-  return down_impl(shape, hdr, d_blob, d_hq_scratch, d_sh, sh_stride, M, d_y, y_dtype, d_ws, true, d_next_blob, s);
+  return down_impl(L, shape, d_blob, d_hq_scratch, d_sh, sh_stride, M, d_y, y_dtype, d_ws, true, d_next_blob, s);
 }
 
 int spense_mlp_dyn(const spense_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx, int32_t M,
@@ -619,28 +586,14 @@ int spense_mlp_dyn(const spense_shape_t* shape, const void* d_blob, const uint8_
   if (!aligned(d_blob, 128) || !aligned(d_x, 128) || !aligned(d_hq_scratch, 128) || !aligned(d_y, 16) ||
       !aligned(d_sx, 4) || !aligned(d_sh_out, 4) || !aligned(d_h_scratch, 16) || !aligned(d_next_blob, 128))
     return SPENSE_ERR_ALIGN;
-  st = check_ws(shape, M, d_ws, ws_bytes);
-  if (st) return st;
-  st = check_device();
-  if (st) return st;
-  BlobHeader hdr;
-  st = read_header(d_blob, shape, &hdr);
+  Launch L;
+  st = enter(shape, M, d_ws, ws_bytes, &L);
   if (st) return st;
   cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
-  const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const float* amax = reinterpret_cast<const float*>(reinterpret_cast<const uint8_t*>(d_ws) + kFlagBytes);
-  for (int m0 = 0; m0 < M; m0 += 128) {                      // gate_up (h in fp32, max|h| per CTA) -> requant, per token block
-    const int Mb = (M - m0) < 128 ? (M - m0) : 128;
-    const int n_pad = n_pad_of(Mb);
-    st = gate_up_impl(shape, hdr, d_blob, d_x + (size_t)m0 * g.H, d_sx + m0, Mb, d_sx, 0, d_hq_scratch + (size_t)m0 * g.I,
-                      d_h_scratch + (size_t)m0 * g.I, d_ws, true, m0 + 128 >= M, s, true);
-    if (st) return st;
-    const Schedule& sc = get_schedule(0, g, n_pad, g_num_sms);
-    st = launch_requant_rows(d_h_scratch + (size_t)m0 * g.I, Mb, g.I, amax, sc.n_spans, n_pad, d_hq_scratch + (size_t)m0 * g.I,
-                             d_sh_out + m0, s);
-    if (st) return st;
-  }
-  return down_impl(shape, hdr, d_blob, d_hq_scratch, d_sh_out, 1, M, d_y, y_dtype, d_ws, true, d_next_blob, s);
+  // gate_up (h in fp32, max|h| per CTA) -> row requant (s_h, Hq), per launch of token blocks; then down
+  st = gate_up_impl(L, shape, d_blob, d_x, d_sx, M, d_sx, 0, d_hq_scratch, d_h_scratch, d_ws, true, true, s, true, d_sh_out);
+  if (st) return st;
+  return down_impl(L, shape, d_blob, d_hq_scratch, d_sh_out, 1, M, d_y, y_dtype, d_ws, true, d_next_blob, s);
 }
 
 int spense_mlp_host(const spense_shape_t* shape, const void* d_blob, const uint8_t* h_x, const float* h_sx, int32_t M,
@@ -662,7 +615,8 @@ int spense_mlp_host(const spense_shape_t* shape, const void* d_blob, const uint8
   if (st) return st;
   const size_t esz = y_dtype == SPENSE_F32 ? 4 : 2;
   if (cudaMemcpyAsync(h_y, d_y, (size_t)M * shape->H * esz, cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPENSE_ERR_CUDA;
-  return cudaStreamSynchronize(s) == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;
+  if (cudaStreamSynchronize(s) != cudaSuccess) return SPENSE_ERR_CUDA;
+  return pending_device_error();
 }
 
 int spense_select_workspace_size(const spense_shape_t* shape, size_t* bytes) {
@@ -687,7 +641,7 @@ int spense_select_dense(const spense_shape_t* shape, const float* d_wgate, const
   size_t need = 0;
   spense_select_workspace_size(shape, &need);
   if (ws_bytes < need) return SPENSE_ERR_BUFFER_TOO_SMALL;
-  st = check_device();
+  st = check_device(nullptr, nullptr);
   if (st) return st;
   return launch_select(shape, d_wgate, d_wup, d_wdown, d_hdiag_x, d_hdiag_h, eps, d_score, d_dense_idx, d_perm, d_ws,
                        reinterpret_cast<cudaStream_t>(stream));
@@ -699,7 +653,7 @@ int spense_quantize_e4m3(const float* d_in, int64_t rows, int64_t cols, int32_t 
     return SPENSE_ERR_ARG;
   if (rows > 0x7FFFFFFF) return SPENSE_ERR_SHAPE;
   if (ws_bytes < (size_t)(rows + 1) * 4) return SPENSE_ERR_BUFFER_TOO_SMALL;
-  int st = check_device();
+  int st = check_device(nullptr, nullptr);
   if (st) return st;
   return launch_quantize(d_in, rows, cols, mode, d_out, d_scales, d_ws, reinterpret_cast<cudaStream_t>(stream));
 }

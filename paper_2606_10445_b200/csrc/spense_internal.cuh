@@ -19,32 +19,38 @@ namespace spense {
 //   "pair tile" = two 128-row A operands (MMA-M = 128 each) that share one B (activation) tile:
 //       gate_up : rows [128t, 128t+128) of W_gate and of W_up       (tile t < I_s/128 sparse, else dense)
 //       down    : rows [256t, 256t+128) and [256t+128, 256t+256) of W_down (sparse K range, then dense)
-//   sparse stage (K = 256 logical): A0 vals 16 KB | A1 vals 16 KB | A0 meta 4 KB | A1 meta 4 KB
+//   sparse stage (K = 256 logical): A0 vals 16 KB | A0 meta 4 KB | A1 vals 16 KB | A1 meta 4 KB
 //   dense  stage (K = 128)        : A0 16 KB | A1 16 KB
+//   (operand-major, so that the CTA pair of the wide-token kernel loads one operand each: 20 KB / 16 KB contiguous)
 //   vals / dense images: 128 rows x 128 B, canonical K-major SWIZZLE_128B (8-row x 128 B atoms,
 //       16-byte chunk index XOR (row & 7)).  meta image: 2 atoms of 128 rows x 16 B, row-major
 //       (one atom = K 128 logical = what one tcgen05.cp.128x128b moves to TMEM).
+//   gate_up operand rows: operand a of pair tile t holds the gate AND the up rows of the 64 intermediate indices
+//       128 t + 64 a + [0, 64): operand row 32 q + i = gate row of index 16 q + i, operand row 32 q + 16 + i = up row of
+//       the same index (q < 4, i < 16).  g and u of one index then sit in the two 16-lane halves of ONE TMEM lane
+//       quadrant of ONE accumulator, so a warp reads both with two tcgen05.ld.16x256b and every operand is a
+//       self-contained GLU tile (what lets the wide-token kernel give each CTA of a pair one operand).
 // ------------------------------------------------------------------------------------------
 constexpr int kTileRows = 128;
 constexpr int kSparseStageK = 256;           // logical K per sparse stage
 constexpr int kDenseStageK = 128;            // K per dense stage
 constexpr int kOperandBytes = 128 * 128;     // one 128 x 128 B operand image
 constexpr int kMetaBytes = 128 * 32;         // one operand's metadata per sparse stage
-constexpr int kSparseStageBytes = 2 * kOperandBytes + 2 * kMetaBytes;  // 40960
+constexpr int kSparseOperandBytes = kOperandBytes + kMetaBytes;         // 20480: values + metadata of one operand
+constexpr int kSparseStageBytes = 2 * kSparseOperandBytes;              // 40960
 constexpr int kDenseStageBytes = 2 * kOperandBytes;                    // 32768
 constexpr int kBlobHeaderBytes = 1024;
 constexpr uint32_t kBlobMagic = 0x53504E53u;  // "SNPS"
-constexpr int kBlobVersion = 1;
-constexpr int kMaxSpans = 160;
+constexpr int kBlobVersion = 2;
+constexpr int kMaxSpans = 160;               // fix-up slots of a launch (one per CTA)
 constexpr int kMaxTokens = 1 << 20;           // tokens per call (the activation tensor map is built over all of them)
 constexpr int kSmemMax = 232448;             // opt-in dynamic shared memory per CTA
-constexpr int kFlagBytes = 4096;             // control words (128 B) + 2 flags per span
-constexpr int kAmaxBytes = 160 * 128 * 4;    // dynamic requant: max|h| per span and token (follows the flags)
-constexpr int kMaxGateTiles = 8192;          // I <= 2^20
-constexpr int kDepInts = kMaxGateTiles + 1024;   // padded so that kWsFixedBytes is a multiple of 4 KB // gate_up tile-done flags (down polls them 16 at a time past the end)
-constexpr int kDepBytes = 2 * kDepInts * 4;  // flags, then the arrival counters of tiles finished by several CTAs
-constexpr int kWsFixedBytes = kFlagBytes + kAmaxBytes + kDepBytes;   // zeroed by spense_workspace_init; partials follow
-constexpr int kCtrlDepDone = 4;              // int index in the control words: down CTAs that are done with the tile flags
+constexpr int kDecodeMaxTokens = 112;        // up to here: one CTA per span, pair stages, two accumulator buffers (4 x 112 TMEM columns)
+constexpr int kWideMaxTokens = 240;          // token columns of one CTA pair of the wide kernel (2 buffers x 240 + 16 metadata columns)
+constexpr int kFlagBytes = 4096;             // control words (128 B) + 2 flags per slot
+constexpr int kAmaxBytes = kMaxSpans * 256 * 4;   // dynamic requant: max|h| per slot and token column (follows the flags)
+constexpr int kWsFixedBytes = kFlagBytes + kAmaxBytes;   // zeroed by spense_workspace_init; partials follow
+constexpr long long kWaitBudgetNs = 2000000000ll;   // a CTA gives up waiting for a peer after 2 s (a launch takes < 10 ms)
 
 struct BlobHeader {
   uint32_t magic;
@@ -95,40 +101,35 @@ __host__ __device__ inline int sw128_offset(int r, int b) {
 // ------------------------------------------------------------------------------------------
 struct GemmParams {
   const uint8_t* section;   // first stage image of this matrix family
+  const BlobHeader* hdr;    // the blob header (device): weight scales are READ ON THE DEVICE from it, magic / shape are checked there
+  int H, I, I_d;            // the shape the caller states (compared with the header on the device)
   int mode;                 // 0 gate_up, 1 down
   int num_tiles, tiles_sparse;
   int ns, nd;               // mode 0: stages of a sparse tile / of a dense tile; mode 1: per tile both
   int dense_k0;             // K byte offset of the first dense stage in the B operand (mode 1: I_s)
-  int n_spans;
-  int M, n_pad;             // tokens in this launch; token columns of one MMA (M padded to 16, at most 128)
-  int nb, blk0;             // token blocks of n_pad tokens covered by this launch (grid = nb * n_spans CTAs) and the first
-                            // of them: the CTAs of the nb blocks walk the same schedule side by side, so a weight stage is
-                            // read from HBM once and found in L2 by the other blocks
+  int n_spans;              // stream-K spans of the schedule (= CTAs, or CTA pairs, per token block)
+  int M, n_pad;             // tokens in this call; token columns of one MMA (a token block, padded to 16)
+  int nb, blk0;             // token blocks covered by this launch and the first of them: the CTAs of the nb blocks walk the
+                            // same schedule side by side, so a weight stage is read from HBM once and found in L2 by the others
   int num_stages, slot_bytes, acc_stride, num_acc_bufs;
   // epilogue
   const float* s_act;       // mode 0: s_x [M]; mode 1: s_h (stride sh_stride)
   const float* s_h;         // mode 0: requant scale
   int sh_stride;
-  float w_scale0, w_scale1; // mode 0: gate, up; mode 1: down, down
+  int scale0, scale1;       // indices into hdr->w_scale: mode 0: gate, up; mode 1: down, down
   uint8_t* hq;              // mode 0 out [M, ld_out]
   float* h_f32;             // mode 0 optional out
-  float* amax_part;         // mode 0, dynamic requant: per-span per-token max|h| [n_spans][n_pad] (then hq is not written)
+  float* amax_part;         // mode 0, dynamic requant: per-slot per-token max|h| [slots][n_pad] (then hq is not written)
   void* y;                  // mode 1 out [M, ld_out]
   int y_dtype;
   int ld_out;               // I (mode 0) or H (mode 1)
   int out_rows;             // valid output columns (I or H) for masking padded tiles
-  int* ws_ctrl;             // workspace control words of this mode: [0] epoch of the last launch, [1] started-CTA count
-  int* flags;               // workspace: 2 ints per span (first / last segment), hold the epoch of the dump
-  float* partials;          // workspace: 2 slots per span of 2 * n_pad * 128 floats
-  // fine-grained gate_up -> down dependency inside spense_mlp (replaces the grid-wide wait of down's loads)
-  int* tile_flags;          // mode 0: set to 1 when all of Hq[:, 128 t .. 128 t + 128) is stored (nullptr: off)
-  int* tile_cnt;            // mode 0: arrivals at tiles that several CTAs finish (reduce-scatter)
-  const int* dep_flags;     // mode 1: the same flags, polled before the Hq tile of a stage is loaded (nullptr: PDL wait)
-  int* dep_done;            // mode 1: CTAs done; the last one clears the flags for the next layer
-  int dep_tiles;
-  uint32_t gated_pf_bytes;  // mode 1 gated: L2 prefetch budget per span while waiting for the first Hq tiles
+  int* ws_ctrl;             // workspace control words: [0] epoch of the last launch, [1] started-CTA count
+  int* flags;               // workspace: 2 ints per slot (first / last segment), hold the epoch of the dump
+  float* partials;          // workspace: 2 partial tiles per slot
+  int* status;              // mapped pinned host word: first device-side error (bad blob header, a peer CTA never showed up)
   int pf_pace_ns;           // next-kernel L2 prefetch: nanoseconds per 32 KB chunk (0 = all at once)
-  long long* trace;         // debug timeline (16 slots per span) or nullptr
+  long long* trace;         // debug timeline (16 slots per span; SPENSE_DEBUG_HOOKS builds) or nullptr
   const uint8_t* next_base; // section the NEXT kernel of the stream will stream (L2 prefetch during our tail) or nullptr
   int span_begin[kMaxSpans + 1];
   uint32_t next_off[kMaxSpans];   // byte offset of span i's first stage in next_base ...
@@ -160,6 +161,30 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "@p bra WAIT_DONE;\n\t"
       "bra WAIT_LOOP;\n\t"
       "WAIT_DONE:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+// one try (the hardware suspends the thread up to an implementation-defined time): true once the phase is complete
+__device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+               : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return ok != 0;
+}
+// arrive on a barrier of another CTA of the cluster (address from mapa)
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ uint32_t mapa_shared(uint32_t addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 __device__ __forceinline__ void fence_barrier_init() {
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -193,6 +218,14 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
       "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint "
       "[%0], [%1, {%2, %3}], [%4], %5;"
       ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar), "l"(pol) : "memory");
+}
+// the same issued by either CTA of a pair: the bytes land in the issuing CTA, the transaction count goes to `cluster_bar`
+// (the LEADER CTA's barrier, a shared::cluster address), so the leader's MMA thread sees both halves of a stage
+__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t cluster_bar, uint64_t pol) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint "
+      "[%0], [%1, {%2, %3}], [%4], %5;"
+      ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(cluster_bar), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
@@ -229,6 +262,40 @@ __device__ __forceinline__ void mma_f8_sparse(uint32_t d, uint64_t adesc, uint64
 // shared -> TMEM copy of one metadata atom: 128 lanes x 128 bit (SASS: UTCCP)
 __device__ __forceinline__ void tc_cp_128x128b(uint32_t taddr, uint64_t sdesc) {
   asm volatile("tcgen05.cp.cta_group::1.128x128b [%0], %1;" ::"r"(taddr), "l"(sdesc) : "memory");
+}
+// ---- CTA-pair (cta_group::2) forms: one thread of the leader CTA issues for both CTAs; A = 128 rows from each CTA
+// (same smem offset), B = N/2 rows from each, D = 128 lanes x N columns in each CTA's TMEM, metadata per CTA
+__device__ __forceinline__ void tmem_alloc_pair(uint32_t smem_dst, uint32_t ncols) {   // one warp of EACH CTA, same smem offset
+  asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc_pair(uint32_t taddr, uint32_t ncols) {
+  asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void tc_commit_pair(uint32_t bar, uint16_t cta_mask) {   // arrives on `bar` (same offset) in every CTA of the mask
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               ::"r"(bar), "h"(cta_mask) : "memory");
+}
+__device__ __forceinline__ void mma_f8_dense_pair(uint32_t d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::f8f6f4 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void mma_f8_sparse_pair(uint32_t d, uint64_t adesc, uint64_t bdesc, uint32_t e, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %5, 0;\n\t"
+      "tcgen05.mma.sp.cta_group::2.kind::f8f6f4 [%0], %1, %2, [%3], %4, p;\n\t}"
+      ::"r"(d), "l"(adesc), "l"(bdesc), "r"(e), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void tc_cp_128x128b_pair(uint32_t taddr, uint64_t sdesc) {
+  asm volatile("tcgen05.cp.cta_group::2.128x128b [%0], %1;" ::"r"(taddr), "l"(sdesc) : "memory");
+}
+// 16 lanes x 8 columns: thread t gets lanes t/4 (v[0], v[1]) and t/4 + 8 (v[2], v[3]) of the 16 lanes that start at the
+// address's lane (a multiple of 16 inside the warp's quadrant), columns 2 (t % 4) and 2 (t % 4) + 1
+__device__ __forceinline__ void tmem_ld_16x256b(uint32_t taddr, uint32_t (&v)[4]) {
+  asm volatile("tcgen05.ld.sync.aligned.16x256b.x1.b32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]) : "r"(taddr) : "memory");
 }
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
   asm volatile(
@@ -270,11 +337,11 @@ __device__ __forceinline__ bool elect_one() {
 int launch_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8_t* d_wup, const uint8_t* d_wdown,
                 const float* h_w_scale, const int32_t* d_perm, void* d_blob, const spense_canon_t* canon, void* d_ws,
                 int64_t* h_err_where, cudaStream_t stream);
-int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, bool pdl, cudaStream_t stream);
-int launch_mlp(const GemmParams& pg, const CUtensorMap& tmap_x, const GemmParams& pd, const CUtensorMap& tmap_hq,
-               cudaStream_t stream);
+int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, bool pdl, int dev, int sms, cudaStream_t stream);
+int launch_gemm_wide(const GemmParams& p, const CUtensorMap& tmap_b, const CUtensorMap& tmap_ws, const CUtensorMap& tmap_wd,
+                     bool pdl, int dev, int sms, cudaStream_t stream);
 int launch_requant_rows(const float* d_h, int rows, int cols, const float* d_amax_part, int n_part, int part_stride,
-                        uint8_t* d_hq, float* d_sh, cudaStream_t stream);
+                        int block_rows, uint8_t* d_hq, float* d_sh, cudaStream_t stream);
 int launch_select(const spense_shape_t* shape, const float* d_wgate, const float* d_wup, const float* d_wdown,
                   const float* d_hdiag_x, const float* d_hdiag_h, float eps, float* d_score, int32_t* d_dense_idx,
                   int32_t* d_perm, void* d_ws, cudaStream_t stream);

@@ -79,7 +79,10 @@ __global__ void pack_gate_up_kernel(Geometry g, const uint8_t* __restrict__ wgat
   const int r = blockIdx.x;
   const int src_row = perm ? perm[r] : r;
   const uint8_t* src = (matrix == 0 ? wgate : wup) + (size_t)src_row * g.H;
-  const int tile = r >> 7, rr = r & 127;
+  // pair tile r / 128; inside it operand (r % 128) / 64 holds the gate and the up row of an index in the two 16-lane
+  // halves of one lane quadrant (layout: spense_internal.cuh)
+  const int tile = r >> 7, opnd = (r >> 6) & 1;
+  const int rr = (((r >> 4) & 3) << 5) | (matrix << 4) | (r & 15);
   uint8_t* sec = blob + g.gate_up_off;
   if (matrix == 0 && canon.perm && threadIdx.x == 0) canon.perm[r] = src_row;
   if (r < g.I_s) {
@@ -104,8 +107,8 @@ __global__ void pack_gate_up_kernel(Geometry g, const uint8_t* __restrict__ wgat
       const int js = t >> 5;                                // 32 meta bytes (= 128 value bytes) per stage and row
       const int tb = t & 31;
       uint8_t* stage = tile_base + (size_t)js * kSparseStageBytes;
-      *reinterpret_cast<uint32_t*>(stage + matrix * kOperandBytes + sw128_offset(rr, 4 * tb)) = vals;
-      stage[2 * kOperandBytes + matrix * kMetaBytes + (tb >> 4) * 2048 + rr * 16 + (tb & 15)] = (uint8_t)meta;
+      *reinterpret_cast<uint32_t*>(stage + opnd * kSparseOperandBytes + sw128_offset(rr, 4 * tb)) = vals;
+      stage[opnd * kSparseOperandBytes + kOperandBytes + (tb >> 4) * 2048 + rr * 16 + (tb & 15)] = (uint8_t)meta;
     }
   } else {
     const int td = tile - g.gu_tiles_sparse;
@@ -123,7 +126,7 @@ __global__ void pack_gate_up_kernel(Geometry g, const uint8_t* __restrict__ wgat
       if (st & 4) report(err, 1, matrix, r, 2 * t + 1);
       if (cdn) *reinterpret_cast<uint2*>(cdn + (size_t)(r - g.I_s) * g.H + 8 * t) = w;
       const int jd = (8 * t) >> 7, b = (8 * t) & 127;
-      *reinterpret_cast<uint2*>(tile_base + (size_t)jd * kDenseStageBytes + matrix * kOperandBytes + sw128_offset(rr, b)) = w;
+      *reinterpret_cast<uint2*>(tile_base + (size_t)jd * kDenseStageBytes + opnd * kOperandBytes + sw128_offset(rr, b)) = w;
     }
   }
 }
@@ -160,8 +163,8 @@ __global__ void pack_down_kernel(Geometry g, const uint8_t* __restrict__ wdown, 
     }
     const int js = t >> 5, tb = t & 31;
     uint8_t* stage = tile_base + (size_t)js * kSparseStageBytes;
-    *reinterpret_cast<uint32_t*>(stage + sub * kOperandBytes + sw128_offset(rr, 4 * tb)) = vals;
-    stage[2 * kOperandBytes + sub * kMetaBytes + (tb >> 4) * 2048 + rr * 16 + (tb & 15)] = (uint8_t)meta;
+    *reinterpret_cast<uint32_t*>(stage + sub * kSparseOperandBytes + sw128_offset(rr, 4 * tb)) = vals;
+    stage[sub * kSparseOperandBytes + kOperandBytes + (tb >> 4) * 2048 + rr * 16 + (tb & 15)] = (uint8_t)meta;
   }
   // dense K range
   uint8_t* dense_base = tile_base + (size_t)g.dn_ns * kSparseStageBytes;
@@ -233,16 +236,20 @@ __global__ void quantize_kernel(const float* __restrict__ in, int64_t cols, cons
 
 // ---------------------------------------------------------------- dynamic per-token requant
 // h [rows, cols] fp32 (written by gate_up in dynamic mode) -> s_h[m] = max_j|h[m,j]| / 448 (1 if zero),
-// Hq[m,j] = E4M3_rne_sat(h[m,j] / s_h[m]).  The row maximum comes from the per-CTA maxima gate_up left in
-// amax_part [n_part][part_stride] (no atomics, nothing to reset).  grid = (column chunks of 4096, rows).
+// Hq[m,j] = E4M3_rne_sat(h[m,j] / s_h[m]).  The row maximum comes from the per-CTA maxima gate_up left in amax_part:
+// row m belongs to token block m / block_rows whose CTAs own the slots [blk * n_part, (blk + 1) * n_part), each
+// [part_stride] floats indexed by the token column m % block_rows (no atomics, nothing to reset).
+// grid = (column chunks of 4096, rows).
 __global__ void __launch_bounds__(256) requant_rows_kernel(const float* __restrict__ h, int cols, const float* __restrict__ amax_part,
-                                                           int n_part, int part_stride, uint8_t* __restrict__ hq,
+                                                           int n_part, int part_stride, int block_rows, uint8_t* __restrict__ hq,
                                                            float* __restrict__ s_h) {
   asm volatile("griddepcontrol.wait;" ::: "memory");            // h and amax_part come from the previous kernel
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const int row = blockIdx.y;
+  const int blk = row / block_rows, col = row - blk * block_rows;
+  const float* part = amax_part + (size_t)blk * n_part * part_stride + col;
   float m = 0.0f;
-  for (int i = threadIdx.x; i < n_part; i += blockDim.x) m = fmaxf(m, __ldcg(amax_part + (size_t)i * part_stride + row));
+  for (int i = threadIdx.x; i < n_part; i += blockDim.x) m = fmaxf(m, __ldcg(part + (size_t)i * part_stride));
   m = block_max(m);
   const float s = m > 0.0f ? __fdiv_rn(m, 448.0f) : 1.0f;
   if (blockIdx.x == 0 && threadIdx.x == 0) s_h[row] = s;
@@ -262,7 +269,7 @@ __global__ void __launch_bounds__(256) requant_rows_kernel(const float* __restri
 }  // namespace
 
 int launch_requant_rows(const float* d_h, int rows, int cols, const float* d_amax_part, int n_part, int part_stride,
-                        uint8_t* d_hq, float* d_sh, cudaStream_t stream) {
+                        int block_rows, uint8_t* d_hq, float* d_sh, cudaStream_t stream) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)((cols + 4095) / 4096), (unsigned)rows);
   cfg.blockDim = dim3(256);
@@ -272,7 +279,7 @@ int launch_requant_rows(const float* d_h, int rows, int cols, const float* d_ama
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  const cudaError_t e = cudaLaunchKernelEx(&cfg, requant_rows_kernel, d_h, cols, d_amax_part, n_part, part_stride, d_hq, d_sh);
+  const cudaError_t e = cudaLaunchKernelEx(&cfg, requant_rows_kernel, d_h, cols, d_amax_part, n_part, part_stride, block_rows, d_hq, d_sh);
   return e == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;
 }
 

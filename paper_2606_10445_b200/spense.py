@@ -19,9 +19,10 @@ SPENSE_PER_TENSOR, SPENSE_PER_ROW = 0, 1
 
 STATUS = {0: "SPENSE_OK", -1: "SPENSE_ERR_ARG", -2: "SPENSE_ERR_ALIGN", -3: "SPENSE_ERR_SHAPE",
           -4: "SPENSE_ERR_BUFFER_TOO_SMALL", -5: "SPENSE_ERR_NOT_2_4", -6: "SPENSE_ERR_NAN_WEIGHT",
-          -7: "SPENSE_ERR_BAD_PERM", -8: "SPENSE_ERR_ARCH", -9: "SPENSE_ERR_CUDA", -10: "SPENSE_ERR_BAD_BLOB"}
+          -7: "SPENSE_ERR_BAD_PERM", -8: "SPENSE_ERR_ARCH", -9: "SPENSE_ERR_CUDA", -10: "SPENSE_ERR_BAD_BLOB",
+          -11: "SPENSE_ERR_TIMEOUT"}
 
-EXPORTS = ["spense_version", "spense_strerror", "spense_perm_from_dense_idx", "spense_pack_sizes", "spense_pack",
+EXPORTS = ["spense_version", "spense_strerror", "spense_device_status", "spense_schedule", "spense_perm_from_dense_idx", "spense_pack_sizes", "spense_pack",
            "spense_workspace_size", "spense_workspace_init", "spense_gate_up", "spense_down", "spense_mlp",
            "spense_mlp_dyn", "spense_mlp_host", "spense_quantize_e4m3", "spense_select_workspace_size",
            "spense_select_dense"]
@@ -58,6 +59,8 @@ def lib() -> ctypes.CDLL:
         L.spense_version.restype = c_int
         L.spense_strerror.restype = c_char_p
         L.spense_strerror.argtypes = [c_int]
+        L.spense_device_status.argtypes = [c_int]
+        L.spense_schedule.argtypes = [POINTER(Shape), c_int32, c_int32, c_int32, POINTER(c_int32), POINTER(c_int32)]
         L.spense_perm_from_dense_idx.argtypes = [c_int32, POINTER(c_int32), c_int32, POINTER(c_int32)]
         L.spense_pack_sizes.argtypes = [POINTER(Shape), POINTER(c_size_t), POINTER(c_size_t)]
         L.spense_pack.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, POINTER(c_float), c_void_p, c_void_p,
@@ -110,6 +113,21 @@ def _dev(t: torch.Tensor, dtype=None):
 
 def spense_version() -> int:
     return lib().spense_version()
+
+
+def spense_device_status(clear: bool = False) -> str:
+    """The first device-side error an earlier launch recorded (synchronise first), as its status name."""
+    return STATUS[lib().spense_device_status(1 if clear else 0)]
+
+
+def spense_schedule(H: int, I: int, I_dense: int, M: int, mode: int, sms: int = 148):
+    """(span boundaries, info) of the launch geometry for M tokens; see include/spense.h."""
+    sb = (c_int32 * 161)()
+    info = (c_int32 * 6)()
+    n = lib().spense_schedule(ctypes.byref(Shape(H, I, I_dense)), M, mode, sms, sb, info)
+    if n < 0:
+        raise SpenseError(n)
+    return list(sb[:n + 1]), dict(zip(("stages", "blocks_per_launch", "n_pad", "ring", "blocks", "ctas_per_span"), info))
 
 
 def spense_perm_from_dense_idx(I: int, dense_idx) -> torch.Tensor:

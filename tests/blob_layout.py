@@ -23,15 +23,29 @@ def _put_rows_sw128(img, rows_bytes):
 
 
 def _sparse_stage(vals0, meta0, vals1, meta1):
-    """vals*: [128, 128] compressed bytes (K 256 logical), meta*: [128, 32]."""
+    """vals*: [128, 128] compressed bytes (K 256 logical), meta*: [128, 32].
+    Stage image = operand 0 (values 16 KB, metadata 4 KB as two 128 x 16 B atoms), then operand 1 likewise."""
     st = np.zeros(SPARSE_STAGE, np.uint8)
-    _put_rows_sw128(st[0:OPER], vals0)
-    _put_rows_sw128(st[OPER:2 * OPER], vals1)
-    for m, meta in enumerate((meta0, meta1)):
-        base = 2 * OPER + m * META
+    for m, (vals, meta) in enumerate(((vals0, meta0), (vals1, meta1))):
+        base = m * (OPER + META)
+        _put_rows_sw128(st[base:base + OPER], vals)
         for atom in range(2):
-            st[base + atom * 2048: base + (atom + 1) * 2048] = meta[:, atom * 16:(atom + 1) * 16].reshape(-1)
+            st[base + OPER + atom * 2048: base + OPER + (atom + 1) * 2048] = meta[:, atom * 16:(atom + 1) * 16].reshape(-1)
     return st
+
+
+def _glu_operands(gate_rows, up_rows):
+    """gate_rows, up_rows: [128, n] = the gate / up rows of the 128 intermediate indices of a pair tile.  Operand a
+    holds the indices 64 a + [0, 64): operand row 32 q + i = gate row of index 16 q + i, row 32 q + 16 + i = its up row."""
+    ops = []
+    for a in range(2):
+        op = np.zeros_like(gate_rows)
+        for q in range(4):
+            for i in range(16):
+                op[32 * q + i] = gate_rows[64 * a + 16 * q + i]
+                op[32 * q + 16 + i] = up_rows[64 * a + 16 * q + i]
+        ops.append(op)
+    return ops
 
 
 def _dense_stage(a0, a1):
@@ -62,13 +76,16 @@ def expected_blob_body(c, H, I, I_d):
     gm, um = _pad_cols(c["gate_sp_meta"], ns * 32, 0x44), _pad_cols(c["up_sp_meta"], ns * 32, 0x44)
     for t in range(I_s // 128):
         r = slice(128 * t, 128 * t + 128)
+        v0, v1 = _glu_operands(gv[r], uv[r])
+        m0, m1 = _glu_operands(gm[r], um[r])
         for j in range(ns):
-            out.append(_sparse_stage(gv[r, 128 * j:128 * j + 128], gm[r, 32 * j:32 * j + 32],
-                                     uv[r, 128 * j:128 * j + 128], um[r, 32 * j:32 * j + 32]))
+            out.append(_sparse_stage(v0[:, 128 * j:128 * j + 128], m0[:, 32 * j:32 * j + 32],
+                                     v1[:, 128 * j:128 * j + 128], m1[:, 32 * j:32 * j + 32]))
     for t in range(I_d // 128):
         r = slice(128 * t, 128 * t + 128)
+        a0, a1 = _glu_operands(c["gate_dn"][r], c["up_dn"][r])
         for j in range(H // 128):
-            out.append(_dense_stage(c["gate_dn"][r, 128 * j:128 * j + 128], c["up_dn"][r, 128 * j:128 * j + 128]))
+            out.append(_dense_stage(a0[:, 128 * j:128 * j + 128], a1[:, 128 * j:128 * j + 128]))
     # down: 256-row tiles, sparse K stages then dense K stages
     nt = (H + 255) // 256
     ns = (I_s + 255) // 256

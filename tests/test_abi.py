@@ -27,6 +27,11 @@ def test_every_declared_symbol_is_exported(sp):
     L = ctypes.CDLL(sp.LIB_PATH)
     for n in names:
         assert hasattr(L, n), n
+    # and nothing else: the default build exports exactly what the header declares (no debug hooks)
+    import subprocess
+    out = subprocess.run(["nm", "-D", "--defined-only", sp.LIB_PATH], capture_output=True, text=True, check=True).stdout
+    exported = {ln.split()[-1] for ln in out.splitlines() if ln.split()[-2] in ("T", "t") and ln.split()[-1].startswith("spense_")}
+    assert exported == names, exported ^ names
     assert sp.spense_version() >= 1
     assert sp.lib().spense_strerror(-5).decode().startswith("a group of 4")
 

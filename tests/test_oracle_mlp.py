@@ -159,3 +159,50 @@ def test_dynamic_requant_scale_pins():
     assert np.array_equal(r2["s_h"][live], 2.0 * r["s_h"][live])
     assert np.array_equal(r2["hq"], r["hq"])
     assert np.array_equal(r2["y"], 2.0 * r["y"])
+
+
+def test_down_scale_and_abs_sum_hand_computed():
+    """Pin for `down`'s scaling (PAPER.md:125 input-split; Q5/Q10: y = acc * s_h[m] * s_wd): a 3 x 4 x 8
+    case written out with a plain Python-integer triple loop over hand-listed small values and explicit
+    power-of-two scales, so every product is exact.  Dropping s_wd or s_h[m] from the oracle, applying s_h to the
+    wrong axis, or losing the |.| in absY fails here."""
+    byte_of = {0: 0x00, 1: 0x38, 2: 0x40, 3: 0x44, -1: 0xB8, -2: 0xC0, -3: 0xC4, 0.5: 0x30, -0.5: 0xB0}
+    hq_v = [[1, -2, 0, 3, 0.5, -1, 2, 0],
+            [0, 0, -3, 1, 2, -0.5, 1, 1],
+            [3, 3, -3, -3, 0, 1, -2, 0.5]]                           # [M=3][K=8]
+    wd_v = [[1, 0, -1, 2, 0, 0, 3, -2],
+            [0.5, 2, 0, 0, -3, 1, 0, 0],
+            [0, -1, 0, 2, 0, -0.5, 0, 1],
+            [2, 0, 0, -2, 1, 0, 0, 3]]                               # [N=4][K=8]
+    s_h = [0.5, 2.0, 0.25]                                           # per token
+    s_wd = 0.25
+    hq = np.array([[byte_of[v] for v in row] for row in hq_v], np.uint8)
+    wd = np.array([[byte_of[v] for v in row] for row in wd_v], np.uint8)
+    r = o.down(hq, np.array(s_h, np.float32), wd, s_wd)
+    for m in range(3):
+        for n in range(4):
+            acc = sum(hq_v[m][k] * wd_v[n][k] for k in range(8))             # Y = Hq Wd^T
+            ab = sum(abs(hq_v[m][k] * wd_v[n][k]) for k in range(8))
+            assert r["y"][m, n] == acc * s_h[m] * s_wd, (m, n)
+            assert r["absY"][m, n] == ab * s_h[m] * s_wd, (m, n)
+    assert r["y"][0, 0] == (1 + 6 + 6) * 0.5 * 0.25 and r["y"][1, 1] == (-6 - 0.5) * 2.0 * 0.25   # two entries by hand
+    # a scalar s_h applies to every token
+    r1 = o.down(hq, 2.0, wd, s_wd)
+    assert np.array_equal(r1["y"], r["y"] / np.array(s_h)[:, None] * 2.0)
+
+
+def test_gate_up_scales_hand_computed():
+    """The same for gate_up: g = accG * s_x[m] * s_gate, u = accU * s_x[m] * s_up (Eq. 4)."""
+    byte_of = {0: 0x00, 1: 0x38, 2: 0x40, -1: 0xB8, -2: 0xC0}
+    x_v = [[1, 2, 0, -1], [0, -2, 2, 1]]
+    wg_v = [[1, 0, 0, 2], [0, -1, 1, 0], [2, 2, -2, 0]]
+    wu_v = [[0, 1, -1, 0], [1, 1, 0, 0], [0, 0, 2, -2]]
+    s_x, s_g, s_u = [0.5, 4.0], 0.25, 2.0
+    enc = lambda t: np.array([[byte_of[v] for v in row] for row in t], np.uint8)
+    r = o.gate_up(enc(x_v), np.array(s_x, np.float32), enc(wg_v), enc(wu_v), s_g, s_u, 1.0)
+    for m in range(2):
+        for j in range(3):
+            g = sum(x_v[m][k] * wg_v[j][k] for k in range(4)) * s_x[m] * s_g
+            u = sum(x_v[m][k] * wu_v[j][k] for k in range(4)) * s_x[m] * s_u
+            assert r["g"][m, j] == g and r["u"][m, j] == u
+            assert abs(r["h"][m, j] - g / (1.0 + np.exp(-g)) * u) <= 1e-15 * max(1.0, abs(g * u))

@@ -125,8 +125,6 @@ Plan plan_of(int M, int sms) {
   return pl;
 }
 
-// one partial tile: decode = both operands of the pair tile, wide = the CTA's operand; 2 per slot
-size_t part_floats_of(const Plan& pl) { return (size_t)(pl.wide ? 1 : 2) * pl.n_pad * 128; }
 size_t ws_bytes_for(int M) {
   const size_t cols = M <= kDecodeMaxTokens ? 2 * (size_t)((M + 15) / 16 * 16) : (size_t)kWideMaxTokens;
   return kWsFixedBytes + (size_t)kMaxSpans * 2 * cols * 128 * sizeof(float);
@@ -134,7 +132,7 @@ size_t ws_bytes_for(int M) {
 
 // ---- stream-K schedule: cut the stage sequence into n_spans spans of (nearly) equal cost.
 struct Schedule {
-  int mode, H, I, I_d, n_pad, spans_req, ring, wide;
+  int mode, H, I, I_d, n_pad, spans_req, ring, wide, nb;
   int n_spans;
   int span_begin[kMaxSpans + 1];
   uint32_t span_off[kMaxSpans];   // byte offset of the span's first stage image inside its section
@@ -149,18 +147,19 @@ const Schedule& get_schedule(int mode, const Geometry& g, const Plan& pl) {
   std::lock_guard<std::mutex> lk(g_sched_mu);
   for (const Schedule& s : g_sched)
     if (s.mode == mode && s.H == g.H && s.I == g.I && s.I_d == g.I_d && s.n_pad == pl.n_pad && s.spans_req == pl.spans &&
-        s.ring == pl.ring && s.wide == (int)pl.wide)
+        s.ring == pl.ring && s.wide == (int)pl.wide && s.nb == pl.nb)
       return s;
   Schedule sc = {};
-  sc.mode = mode; sc.H = g.H; sc.I = g.I; sc.I_d = g.I_d; sc.n_pad = pl.n_pad; sc.spans_req = pl.spans; sc.ring = pl.ring; sc.wide = pl.wide;
+  sc.mode = mode; sc.H = g.H; sc.I = g.I; sc.I_d = g.I_d; sc.n_pad = pl.n_pad; sc.spans_req = pl.spans; sc.ring = pl.ring; sc.wide = pl.wide; sc.nb = pl.nb;
   // cost of a stage.  Every CTA keeps the same number of ring slots in flight, so under HBM contention a
   // stage costs one slot latency plus its bytes: measured on B200 (profiles/) a 40 KB sparse stage takes
   // ~1.12x a 32 KB dense one => fixed part ~36 KB-equivalents; activation bytes come from L2 and weigh less.
-  // Wide token tiles are paced by the tensor pipe instead: a sparse stage (K 256) and a dense one (K 128) issue the
-  // same four MMAs.
+  // From three token blocks on (M > 480) a launch is paced by the tensor pipe instead: a sparse stage (K 256) and a
+  // dense one (K 128) issue the same four MMAs.
   const double fixed = 36864.0, gamma = 0.25;
-  const double cs = pl.wide ? 1.0 : fixed + kSparseStageBytes + gamma * 2.0 * pl.n_pad * 128;
-  const double cd = pl.wide ? 1.0 : fixed + kDenseStageBytes + gamma * 1.0 * pl.n_pad * 128;
+  const bool tensor_paced = pl.nb > 2;
+  const double cs = tensor_paced ? 1.0 : fixed + kSparseStageBytes + gamma * 2.0 * pl.n_pad * 128;
+  const double cd = tensor_paced ? 1.0 : fixed + kDenseStageBytes + gamma * 1.0 * pl.n_pad * 128;
   std::vector<double> cost;
   if (mode == 0) {
     cost.insert(cost.end(), (size_t)g.gu_tiles_sparse * g.gu_ns, cs);

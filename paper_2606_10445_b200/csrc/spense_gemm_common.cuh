@@ -29,7 +29,7 @@ __device__ __forceinline__ size_t stage_byte_offset(const GemmParams& p, int til
 
 // The only place with integer divisions (one copy per mode, called once per role).
 template <int MODE>
-__device__ __noinline__ Cursor cursor_at(const GemmParams& p, int s, unsigned long long* byte_off) {
+static __device__ __noinline__ Cursor cursor_at(const GemmParams& p, int s, unsigned long long* byte_off) {
   Cursor c;
   if (MODE == 0) {
     const int sparse_total = p.tiles_sparse * p.ns;
@@ -114,7 +114,7 @@ __device__ __forceinline__ void st_release(int* p, int v) {
 // gives up after kWaitBudgetNs: the CTA records SPENSE_ERR_TIMEOUT in the mapped host status word and traps, so a launch
 // whose peers never show up (device shared with work that pins SMs) fails with a CUDA error instead of hanging for ever;
 // spense_device_status() then says why.  A launch that works never reads the timer: the first try succeeds.
-__device__ __noinline__ void give_up(int* status, int code) {
+static __device__ __noinline__ void give_up(int* status, int code) {
   atomicCAS_system(status, 0, code);
   __threadfence_system();
   __trap();

@@ -1,7 +1,528 @@
-// placeholder until the wide kernel lands
-#include "spense_internal.cuh"
+// Spense hybrid sparse-dense FP8 GEMM for sm_100a: the WIDE-TOKEN kernel (more than kDecodeMaxTokens tokens: the top of
+// the decode range, M = 128-256, and prefill-shaped calls).  Same blob, same stream-K walk, same epilogue arithmetic as
+// the decode kernel (spense_gemm.cu); what changes is who holds what:
+//
+//   * CTA PAIRS (cluster of 2, tcgen05 cta_group::2).  One MMA instruction spans both SMs: M = 256 weight rows = the two
+//     operands of a pair stage, ONE PER CTA (the blob stores stages operand-major and every gate_up operand is a
+//     self-contained GLU tile, spense_internal.cuh), N = up to 240 tokens, of which each CTA stages HALF (the B operand of
+//     a cta_group::2 MMA is split across the pair).  Per MMA a CTA therefore fills and reads 128 weight rows + N/2 token
+//     rows of shared memory instead of 256 + N: the decode kernel run over 128-token blocks was bound by exactly that
+//     traffic (tensor pipe 35-44 % active, round 1).
+//   * One accumulator of up to 240 columns per tile and CTA, DOUBLE BUFFERED (2 x 240 TMEM columns + 16 columns of 2:4
+//     metadata = 496 <= 512): the epilogue of a tile overlaps the MMAs of the next one.
+//   * Token blocks of up to 240 tokens side by side in one launch (grid = blocks x spans x 2 CTAs): the pairs of different
+//     blocks walk the same schedule, so a weight stage is read from HBM once and found in L2 by the other blocks.
+//   * Weights arrive by TENSOR copies (the blob section seen as rows of 128 bytes, one box = one operand image) because
+//     only cp.async.bulk.tensor has the .cta_group::2 form whose completion counts on the LEADER CTA's barrier: the
+//     leader's MMA thread waits on one barrier for both CTAs' halves of a stage.
+//
+// Roles per CTA (640 threads): warp 0 producer (its operand + its half of the token tile), warp 1 MMA issuer (leader CTA
+// only), warp 2 TMEM allocator, warps 4-19 epilogue of the CTA's own 128 accumulator lanes.  The split-K fix-up is the
+// decode kernel's, per CTA: its partners are the CTAs of the same rank in the neighbouring spans of the same token block.
+#include <mutex>
+
+#include "spense_gemm_common.cuh"
+
 namespace spense {
-int launch_gemm_wide(const GemmParams&, const CUtensorMap&, const CUtensorMap&, const CUtensorMap&, bool, int, int, cudaStream_t) {
-  return SPENSE_ERR_CUDA;
+
+namespace {
+
+using namespace dev;
+
+__device__ __forceinline__ void epi_sync() { asm volatile("bar.sync 1, 512;" ::: "memory"); }   // the 16 epilogue warps
+
+constexpr int kEpiThreads = 512;
+constexpr int kEpiWarps = kEpiThreads / 32;
+constexpr int kThreads = 128 + kEpiThreads;
+constexpr int kTmemCols = 512;
+constexpr int kMetaCol = 480;   // 2 buffers x 8 columns of 2:4 metadata (one operand, K 256)
+
+struct Ctx {
+  uint32_t smem_base;          // 1 KB aligned start of the stage ring (shared address)
+  uint8_t* smem_gen;           // the same, generic
+  int S;                       // ring slots
+  uint32_t slot_bytes, ring_bytes, bar_base, b_half_bytes, tmem_base;
+  uint32_t rank;               // CTA of the pair: 0 = leader (issues the MMAs), holds operand `rank` and token half `rank`
+  int blk;                     // token block of this pair
+  int slot0;                   // fix-up slot of span 0 of this block and rank: slot(span) = slot0 + 2 * span
+  __device__ __forceinline__ uint32_t full_bar(int s) const { return bar_base + 8u * s; }
+  __device__ __forceinline__ uint32_t empty_bar(int s) const { return bar_base + 8u * (8 + s); }
+  __device__ __forceinline__ uint32_t accf_bar(int b) const { return bar_base + 8u * (16 + b); }
+  __device__ __forceinline__ uint32_t acce_bar(int b) const { return bar_base + 8u * (18 + b); }
+  __device__ __forceinline__ uint32_t tmem_slot() const { return bar_base + 8u * 20; }
+  __device__ __forceinline__ uint32_t red_bar() const { return bar_base + 8u * 22; }
+  __device__ __forceinline__ volatile uint32_t* tmem_slot_ptr() const { return reinterpret_cast<volatile uint32_t*>(smem_gen + ring_bytes + 8 * 20); }
+  __device__ __forceinline__ volatile int* epoch_ptr() const { return reinterpret_cast<volatile int*>(smem_gen + ring_bytes + 8 * 21); }
+  __device__ __forceinline__ float4* sc0() const { return reinterpret_cast<float4*>(smem_gen + ring_bytes + 256); }
+  __device__ __forceinline__ float* sc1(int n_pad) const { return reinterpret_cast<float*>(smem_gen + ring_bytes + 256 + 16 * n_pad); }
+};
+
+struct Group { int a, b, tile, first; };
+
+// ===================== producer (one thread per CTA) =====================
+// Slot image: [operand: values 16 KB | metadata 4 KB] [token half-tile(s): n_pad/2 rows x 128 B, two for a sparse stage].
+// Every copy counts on the LEADER's full barrier; the leader's producer arms it with the bytes of both CTAs.
+template <int MODE>
+__device__ __forceinline__ void producer(const GemmParams& p, const CUtensorMap* tmap_b, const CUtensorMap* tmap_ws,
+                                         const CUtensorMap* tmap_wd, const Ctx& cx, int span) {
+  const int S = cx.S;
+  const int sb = p.span_begin[span];
+  const int n = p.span_begin[span + 1] - sb;
+  // one token block: a weight byte is used once (evict first); several: the pairs of the other blocks read the same
+  // stage at about the same time and should find it in L2
+  const uint64_t pol_w = p.nb == 1 ? policy_evict_first() : policy_evict_normal();
+  const uint64_t pol_a = policy_evict_last();
+  unsigned long long off;
+  Cursor c = cursor_at<MODE>(p, sb, &off);
+  uint32_t row = (uint32_t)(off >> 7);                     // position in the section, in rows of 128 bytes
+  uint32_t info[8];                                        // stages whose weights are in flight: K coordinate | sparse << 31
+  const int tok0 = cx.blk * p.n_pad + (int)cx.rank * (p.n_pad >> 1);   // first token row of this CTA's half
+
+  int w = 0;
+  uint32_t inf_last = 0;
+  int w_slot = 0, w_round = 0, b_slot = 0;
+  auto issue_weight = [&](bool blocking) -> bool {
+    const bool sp = c.j < c.ns;
+    const uint32_t inf = (uint32_t)(sp ? c.j * kSparseStageK : p.dense_k0 + (c.j - c.ns) * kDenseStageK) | (sp ? 0x80000000u : 0u);
+    const uint32_t opb = sp ? (uint32_t)kSparseOperandBytes : (uint32_t)kOperandBytes;
+    const uint32_t tx = 2u * (opb + (sp ? 2u : 1u) * cx.b_half_bytes);
+    const uint32_t fb = mapa_shared(cx.full_bar(w_slot), 0);
+    const uint32_t dst = cx.smem_base + (uint32_t)w_slot * cx.slot_bytes;
+    if (w_round > 0) {
+      const uint32_t par = ((uint32_t)w_round & 1u) ^ 1u;
+      if (blocking) wait_bar(p, cx.empty_bar(w_slot), par);
+      else if (!mbar_try(cx.empty_bar(w_slot), par)) return false;
+    }
+    if (cx.rank == 0) mbar_expect_tx(cx.full_bar(w_slot), tx);
+    tma_load_2d_pair(dst, sp ? tmap_ws : tmap_wd, 0, (int)(row + cx.rank * (opb >> 7)), fb, pol_w);
+    inf_last = inf;
+    if (!blocking) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k)
+        if (k == (w & 7)) info[k] = inf;
+    }
+    row += 2u * (opb >> 7);
+    if (++c.j == c.ns + c.nd) next_tile<MODE>(p, c);
+    ++w;
+    if (++w_slot == S) { w_slot = 0; ++w_round; }
+    return true;
+  };
+  auto load_b = [&](int slot, uint32_t inf) {
+    const uint32_t b_dst = cx.smem_base + (uint32_t)slot * cx.slot_bytes + kSparseOperandBytes;
+    const uint32_t fb = mapa_shared(cx.full_bar(slot), 0);
+    const int k0 = (int)(inf & 0x7FFFFFFFu);
+    tma_load_2d_pair(b_dst, tmap_b, k0, tok0, fb, pol_a);
+    if (inf >> 31) tma_load_2d_pair(b_dst + cx.b_half_bytes, tmap_b, k0 + 128, tok0, fb, pol_a);
+  };
+
+  // weights never depend on the previous kernel of the stream, activations do
+#pragma unroll 1
+  while (w < n && w < S && issue_weight(false)) {}
+  trace(p, span, 1);
+  pdl_wait();
+#pragma unroll 1
+  for (int b = 0; b < n; ++b) {
+    uint32_t inf = 0;
+    if (w <= b) {
+      issue_weight(true);
+      inf = inf_last;
+    } else {
+#pragma unroll
+      for (int k = 0; k < 8; ++k)
+        if (k == (b & 7)) inf = info[k];
+    }
+    load_b(b_slot, inf);
+    if (++b_slot == S) b_slot = 0;
+  }
 }
+
+// ===================== MMA issuer (one thread of the leader CTA) =====================
+template <int MODE>
+__device__ __forceinline__ void mma_issuer(const GemmParams& p, const Ctx& cx, int span) {
+  const int S = cx.S;
+  const uint32_t idesc_d = (1u << 4) | ((uint32_t)(p.n_pad >> 3) << 17) | ((256u >> 4) << 24);
+  const uint32_t idesc_s = idesc_d | (1u << 2);
+  const int sb = p.span_begin[span], se = p.span_begin[span + 1];
+  unsigned long long off;
+  Cursor c = cursor_at<MODE>(p, sb, &off);
+  int slot = 0, it = 0, seg = 0;
+  uint32_t ph = 0;
+#pragma unroll 1
+  for (int s = sb; s < se; ++seg) {
+    const int tile_end = c.first + c.ns + c.nd;
+    const int seg_end = min(se, tile_end);
+    const int buf = seg & 1;
+    const uint32_t use = (uint32_t)(seg >> 1);
+    wait_bar(p, cx.acce_bar(buf), (use & 1u) ^ 1u);        // both CTAs' epilogues have drained this accumulator
+    tc_fence_after();
+    const uint32_t d = cx.tmem_base + (uint32_t)(buf * p.acc_stride);
+    uint32_t acc = 0;
+#pragma unroll 1
+    for (; s < seg_end; ++s, ++it, ++c.j) {
+      wait_bar(p, cx.full_bar(slot), ph);
+      tc_fence_after();
+      if (s == sb) trace(p, span, 3);
+      const uint32_t a0 = cx.smem_base + (uint32_t)slot * cx.slot_bytes;
+      const uint32_t b0 = a0 + kSparseOperandBytes;
+      if (c.j < c.ns) {
+        const uint32_t e_base = cx.tmem_base + kMetaCol + (uint32_t)(it & 1) * 8u;
+        tc_cp_128x128b_pair(e_base, make_desc(a0 + kOperandBytes, 0, 128, kLayoutNone));
+        tc_cp_128x128b_pair(e_base + 4u, make_desc(a0 + kOperandBytes + 2048u, 0, 128, kLayoutNone));
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {                     // 4 sparse MMAs of K = 64 logical (32 B of A, 64 B of B)
+          const uint64_t bd = make_desc(b0 + (uint32_t)(k >> 1) * cx.b_half_bytes + (uint32_t)(k & 1) * 64u, 16, 1024, kLayoutSW128);
+          mma_f8_sparse_pair(d, make_desc(a0 + 32u * k, 16, 1024, kLayoutSW128), bd, e_base + 2u * k, idesc_s, acc);
+          acc = 1;
+        }
+      } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {                     // 4 dense MMAs of K = 32
+          mma_f8_dense_pair(d, make_desc(a0 + 32u * k, 16, 1024, kLayoutSW128), make_desc(b0 + 32u * k, 16, 1024, kLayoutSW128), idesc_d, acc);
+          acc = 1;
+        }
+      }
+      tc_commit_pair(cx.empty_bar(slot), 3);              // both CTAs' slots are free once these MMAs have read them
+      if (++slot == S) { slot = 0; ph ^= 1u; }
+    }
+    tc_commit_pair(cx.accf_bar(buf), 3);                  // accumulator complete in both CTAs
+    if (s == tile_end) next_tile<MODE>(p, c);
+  }
+  trace(p, span, 4);
+}
+
+// scale tables of the pair's token block (weight scales come from the blob header, on the device)
+__device__ __forceinline__ void epilogue_tables(const GemmParams& p, const Ctx& cx, int et, int m_base, int Mb) {
+  if (et < p.n_pad) {
+    const int m = m_base + (et < Mb ? et : Mb - 1);
+    const float w0 = __ldg(&p.hdr->w_scale[p.scale0]);
+    if (p.mode == 0) {
+      const float w1 = __ldg(&p.hdr->w_scale[p.scale1]);
+      const float sx = __ldg(p.s_act + m);
+      const float sh = p.amax_part ? 1.0f : __ldg(p.s_h + (size_t)m * p.sh_stride);
+      cx.sc0()[et] = make_float4(sx * w0, sx * w1, p.amax_part ? 0.0f : sh, __frcp_rn(sh));
+    } else {
+      cx.sc1(p.n_pad)[et] = __ldg(p.s_act + (size_t)m * p.sh_stride) * w0;
+    }
+  }
+}
+
+// 8 token columns of the CTA's accumulator as one thread holds them.
+//   MODE 1 (32x32b): v[i] = lane 32 q + t, column c + i.
+//   MODE 0 (16x256b of the gate half and of the up half of the quadrant): v[4 gu + k] = lane 32 q + 16 gu + t/4 + 8 (k >> 1),
+//          column c + 2 (t % 4) + (k & 1).
+template <int MODE>
+__device__ __forceinline__ void load_acc(uint32_t t0, int c, float (&v)[8]) {
+  uint32_t r[8];
+  if (MODE == 1) {
+    tmem_ld8(t0 + c, r);
+  } else {
+    tmem_ld_16x256b(t0 + c, reinterpret_cast<uint32_t(&)[4]>(r[0]));
+    tmem_ld_16x256b(t0 + (16u << 16) + c, reinterpret_cast<uint32_t(&)[4]>(r[4]));
+  }
+  tmem_ld_wait();
+#pragma unroll
+  for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
+}
+template <int MODE>
+__device__ __forceinline__ int part_index(int i, int q, int t, int c) {
+  if (MODE == 1) return (c + i) * 128 + 32 * q + t;
+  return (c + 2 * (t & 3) + (i & 1)) * 128 + 32 * q + 16 * (i >> 2) + (t >> 2) + 8 * ((i >> 1) & 1);
+}
+
+// ===================== epilogue (16 warps per CTA, the CTA's own 128 lanes) =====================
+template <int MODE, bool DYN>
+__device__ __forceinline__ void epilogue(const GemmParams& p, const Ctx& cx, int span, int epoch) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int q = warp & 3;
+  const int et = threadIdx.x - 128;
+  const int m_base = cx.blk * p.n_pad;
+  const int Mb = min(p.n_pad, p.M - m_base);
+  const int cols_used = min(p.n_pad, (Mb + 7) & ~7);
+  const int cols_per = (((p.n_pad + 3) >> 2) + 7) & ~7;
+  const int c_begin = ((warp - 4) >> 2) * cols_per;
+  const int c_end = min(c_begin + cols_per, cols_used);
+  const float* stg = reinterpret_cast<const float*>(cx.smem_gen);
+  const size_t part_floats = (size_t)p.n_pad * 128;        // one partial: [col][lane]
+  const int sb = p.span_begin[span], se = p.span_begin[span + 1];
+  float4* const sc4 = cx.sc0();
+  const float* const sc1 = cx.sc1(p.n_pad);
+  const uint32_t lead_acce0 = mapa_shared(cx.acce_bar(0), 0);
+  const int rank = (int)cx.rank;
+  uint32_t red_round = 0;
+  auto flag_of = [&](int s, int which) { return p.flags + (cx.slot0 + 2 * s) * 2 + which; };
+  auto part_of = [&](int s, int which) { return p.partials + ((size_t)(cx.slot0 + 2 * s) * 2 + which) * part_floats; };
+
+  Group groups[2];
+  int n_groups = 0;
+  unsigned long long off;
+  Cursor cur = cursor_at<MODE>(p, sb, &off);
+  int seg = 0;
+#pragma unroll 1
+  for (int s = sb; s < se; ++seg) {
+    const int tile_end = cur.first + cur.ns + cur.nd;
+    const int seg_end = min(se, tile_end);
+    const int buf = seg & 1;
+    const uint32_t use = (uint32_t)(seg >> 1);
+    int a = span, b = span;
+    while (p.span_begin[a] > cur.first) --a;
+    while (b + 1 < p.n_spans && p.span_begin[b + 1] < tile_end) ++b;
+
+    wait_bar(p, cx.accf_bar(buf), use & 1u);
+    tc_fence_after();
+    if (et == 0) trace(p, span, seg == 0 ? 5 : 7);
+    const uint32_t t0 = cx.tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * p.acc_stride);
+
+    if (a == b || (b == a + 1 && span == a)) {
+      const bool add = a != b;
+      if (add) {
+        // last segment of this span: every MMA that reads this CTA's ring is complete, the ring stages the partner's partial
+        if (et == 0) {
+          wait_flag(p, flag_of(b, 0), epoch);
+          asm volatile("fence.proxy.async.global;" ::: "memory");
+          mbar_expect_tx(cx.red_bar(), (uint32_t)cols_used * 512u);
+          bulk_g2s(cx.smem_base, part_of(b, 0), (uint32_t)cols_used * 512u, cx.red_bar(), policy_evict_first());
+        }
+        wait_bar(p, cx.red_bar(), red_round & 1u);
+        ++red_round;
+        if (et == 0) trace(p, span, 8);
+      }
+#pragma unroll 1
+      for (int c = c_begin; c < c_end; c += 8) {
+        float v[8];
+        load_acc<MODE>(t0, c, v);
+        if (add) {
+#pragma unroll
+          for (int i = 0; i < 8; ++i) v[i] += stg[part_index<MODE>(i, q, lane, c)];
+        }
+        if (MODE == 0) {
+          glu_chunk<DYN>(p, sc4, cur.tile, 64 * rank + 16 * q, c, Mb, m_base, reinterpret_cast<const float(&)[4]>(v[0]),
+                         reinterpret_cast<const float(&)[4]>(v[4]));
+        } else {
+#pragma unroll
+          for (int i = 0; i < 8; ++i)
+            if (c + i < Mb) store_y(p, cur.tile * 256 + 128 * rank + 32 * q + lane, m_base + c + i, v[i] * sc1[c + i]);
+        }
+      }
+    } else {
+      // split tile, not (solely) ours to finish: dump the raw fp32 partial [col][lane] and publish it
+      const int which = (sb >= cur.first) ? 0 : 1;
+      float* slot = part_of(span, which);
+#pragma unroll 1
+      for (int c = c_begin; c < c_end; c += 8) {
+        uint32_t v0[8];
+        tmem_ld8(t0 + c, v0);
+        tmem_ld_wait();
+#pragma unroll
+        for (int i = 0; i < 8; ++i) __stcg(slot + (size_t)(c + i) * 128 + 32 * q + lane, __uint_as_float(v0[i]));
+      }
+      epi_sync();                                          // all partial stores issued (CTA scope) ...
+      if (et == 0) st_release(flag_of(span, which), epoch);   // ... one gpu-scope release publishes them (cumulativity)
+      if (b > a + 1) {
+        groups[n_groups].a = a; groups[n_groups].b = b; groups[n_groups].tile = cur.tile; groups[n_groups].first = cur.first;
+        ++n_groups;
+      }
+    }
+    // this CTA's warps are done with the accumulator: one arrival per warp on the LEADER's barrier
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive_cluster(lead_acce0 + 8u * (uint32_t)buf);
+    if (et == 0) trace(p, span, 6);
+    s = seg_end;
+    if (s == tile_end) next_tile<MODE>(p, cur);
+  }
+
+  // ---- deferred reduce-scatter of tiles shared by > 2 spans (see spense_gemm.cu); the ring is idle by now
+#pragma unroll 1
+  for (int gi = 0; gi < n_groups; ++gi) {
+    const Group g = groups[gi];
+    const int n = g.b - g.a + 1;
+    const int j = span - g.a;
+    const int m0 = (int)(((long long)j * Mb) / n), m1 = (int)(((long long)(j + 1) * Mb) / n);
+    const int rrow = et & 127;
+    if (m1 > m0) {
+      int cc_max = (int)(cx.ring_bytes / ((uint32_t)n * 512u));
+      if (cc_max > m1 - m0) cc_max = m1 - m0;
+#pragma unroll 1
+      for (int mc = m0; mc < m1; mc += cc_max) {
+        const int cc = min(cc_max, m1 - mc);
+        if (red_round > 0) {
+          fence_proxy_async();
+          epi_sync();
+        }
+        if (et == 0) mbar_expect_tx(cx.red_bar(), (uint32_t)n * (uint32_t)cc * 512u);
+#pragma unroll 1
+        for (int i = et; i < n; i += kEpiThreads) {
+          const int qs = g.a + i;
+          const int which = (p.span_begin[qs] >= g.first) ? 0 : 1;
+          wait_flag(p, flag_of(qs, which), epoch);
+          asm volatile("fence.proxy.async.global;" ::: "memory");
+          bulk_g2s(cx.smem_base + (uint32_t)(i * cc) * 512u, part_of(qs, which) + (size_t)mc * 128, (uint32_t)cc * 512u, cx.red_bar(),
+                   policy_evict_first());
+        }
+        wait_bar(p, cx.red_bar(), red_round & 1u);
+        ++red_round;
+        if (et == 0) trace(p, span, 15);
+        if (MODE == 0) {
+          // threads 0..63 of each 128-thread column group finish one intermediate index each (gate lane, up lane)
+          const int j64 = rrow & 63;
+          const int lane_g = glu_gate_lane_of_index(j64);
+          const int first = lane_g ^ (lane & 16);
+#pragma unroll 1
+          for (int c = (et >> 6); c < cc; c += kEpiThreads >> 6) {
+            float x = 0.0f, y = 0.0f;
+#pragma unroll 4
+            for (int qi = 0; qi < n; ++qi) {               // fixed span order: deterministic
+              const float* img = stg + ((size_t)qi * cc + c) * 128;
+              x += img[first];
+              y += img[first ^ 16];
+            }
+            const float ah = finish_glu<DYN>(p, sc4, g.tile, 64 * rank + j64, mc + c, m_base + mc + c, (lane & 16) ? y : x, (lane & 16) ? x : y);
+            if (DYN) {
+              const int mx = __reduce_max_sync(0xffffffffu, __float_as_int(ah));
+              if (lane == 0) atomicMax(reinterpret_cast<int*>(sc4 + mc + c) + 2, mx);
+            }
+          }
+        } else {
+#pragma unroll 1
+          for (int c = et >> 7; c < cc; c += kEpiThreads >> 7) {
+            float f0 = 0.0f;
+#pragma unroll 4
+            for (int qi = 0; qi < n; ++qi) f0 += stg[((size_t)qi * cc + c) * 128 + rrow];
+            store_y(p, g.tile * 256 + 128 * rank + rrow, m_base + mc + c, f0 * sc1[mc + c]);
+          }
+        }
+      }
+    }
+    if (et == 0) trace(p, span, 9);
+  }
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------ the kernel
+template <int MODE, bool DYN>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+spense_gemm_wide_kernel(const __grid_constant__ GemmParams p, const __grid_constant__ CUtensorMap tmap_b,
+                        const __grid_constant__ CUtensorMap tmap_ws, const __grid_constant__ CUtensorMap tmap_wd) {
+  extern __shared__ uint8_t smem_raw[];
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  if (warp == 0 && lane == 0) { prefetch_tmap(&tmap_b); prefetch_tmap(&tmap_ws); prefetch_tmap(&tmap_wd); }
+  Ctx cx;
+  {
+    const uint32_t raw = smem_u32(smem_raw);
+    cx.smem_base = (raw + 1023u) & ~1023u;
+    cx.smem_gen = smem_raw + (cx.smem_base - raw);
+    cx.S = p.num_stages;
+    cx.slot_bytes = (uint32_t)p.slot_bytes;
+    cx.ring_bytes = (uint32_t)cx.S * cx.slot_bytes;
+    cx.bar_base = cx.smem_base + cx.ring_bytes;
+    cx.b_half_bytes = (uint32_t)(p.n_pad >> 1) * 128u;
+    cx.rank = cluster_ctarank();
+  }
+  // pair b / 2 works on token block blk0 + pair / n_spans, span n_spans - 1 - pair % n_spans of the SAME schedule
+  const int pair = (int)blockIdx.x >> 1;
+  const int bp = pair / p.n_spans;
+  const int span = p.n_spans - 1 - (pair - bp * p.n_spans);
+  cx.blk = p.blk0 + bp;
+  cx.slot0 = bp * p.n_spans * 2 + (int)cx.rank;
+  if (warp == 0 && lane == 0) {
+    for (int s = 0; s < cx.S; ++s) { mbar_init(cx.full_bar(s), 1); mbar_init(cx.empty_bar(s), 1); }
+    for (int b = 0; b < 2; ++b) { mbar_init(cx.accf_bar(b), 1); mbar_init(cx.acce_bar(b), 2 * kEpiWarps); }
+    mbar_init(cx.red_bar(), 1);
+    fence_barrier_init();
+  }
+  if (warp == 2) tmem_alloc_pair(cx.tmem_slot(), kTmemCols);
+  tc_fence_before();
+  cluster_sync_all();                                      // barriers and TMEM of BOTH CTAs exist before anyone signals or writes them
+  tc_fence_after();
+  cx.tmem_base = *cx.tmem_slot_ptr();
+  pdl_launch_dependents();
+  if (p.trace && threadIdx.x == 0 && bp == 0 && cx.rank == 0) {
+    uint32_t smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    p.trace[(size_t)span * 16 + 0] = globaltimer(); p.trace[(size_t)span * 16 + 14] = smid;
+  }
+
+  if (warp == 0) {
+    if (lane == 0) {
+      producer<MODE>(p, &tmap_b, &tmap_ws, &tmap_wd, cx, span);
+      trace(p, span, 2);
+    }
+  } else if (warp == 1) {
+    if (lane == 0 && cx.rank == 0) mma_issuer<MODE>(p, cx, span);
+  } else if (warp >= 4) {
+    const int et = threadIdx.x - 128;
+    pdl_wait();
+    epilogue_tables(p, cx, et, cx.blk * p.n_pad, min(p.n_pad, p.M - cx.blk * p.n_pad));
+    if (et == kEpiThreads - 1) {
+      check_header(p);
+      take_epoch(p.ws_ctrl, (int)gridDim.x, cx.epoch_ptr());
+    }
+    epi_sync();
+    const int epoch = cx.epoch_ptr()[0];
+    epilogue<MODE, DYN>(p, cx, span, epoch);
+    if (DYN) {                        // this CTA's max|h| per token column of its block, for the row requant kernel
+      epi_sync();
+      const int Mb = min(p.n_pad, p.M - cx.blk * p.n_pad);
+      if (et < p.n_pad) p.amax_part[(size_t)(cx.slot0 + 2 * span) * p.n_pad + et] = et < Mb ? cx.sc0()[et].z : 0.0f;
+    }
+    if (p.trace && et == 0 && bp == 0 && cx.rank == 0) p.trace[(size_t)span * 16 + 10] = globaltimer();
+  }
+
+  tc_fence_before();
+  cluster_sync_all();                                      // the peer's MMAs read our ring, its epilogue arrives on our barriers
+  if (warp == 2) { tc_fence_after(); tmem_dealloc_pair(cx.tmem_base, kTmemCols); }
+}
+
+namespace {
+size_t smem_bytes_of(const GemmParams& p) { return (size_t)p.num_stages * p.slot_bytes + 1024 + 256 + 20 * (size_t)p.n_pad; }
+
+// per device and kernel instance, once: opt in to the shared memory; how many CTA pairs can be resident at once
+template <typename K>
+int prepare(K kernel, int which, int dev, int grid) {
+  static std::mutex mu;
+  static bool ready[3][64] = {};
+  static int resident[3][64] = {};
+  std::lock_guard<std::mutex> lk(mu);
+  if (dev < 0 || dev >= 64) return SPENSE_ERR_CUDA;
+  if (!ready[which][dev]) {
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax) != cudaSuccess) return SPENSE_ERR_CUDA;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(2);
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = kSmemMax;
+    int clusters = 0;
+    if (cudaOccupancyMaxActiveClusters(&clusters, kernel, &cfg) != cudaSuccess) return SPENSE_ERR_CUDA;
+    resident[which][dev] = 2 * clusters;
+    ready[which][dev] = true;
+  }
+  return grid <= resident[which][dev] ? SPENSE_OK : SPENSE_ERR_CUDA;
+}
+}  // namespace
+
+int launch_gemm_wide(const GemmParams& p, const CUtensorMap& tmap_b, const CUtensorMap& tmap_ws, const CUtensorMap& tmap_wd,
+                     bool pdl, int dev, int sms, cudaStream_t stream) {
+  (void)sms;
+  const int grid = 2 * p.n_spans * p.nb;
+  int st = p.mode == 1     ? prepare(spense_gemm_wide_kernel<1, false>, 2, dev, grid)
+           : p.amax_part ? prepare(spense_gemm_wide_kernel<0, true>, 1, dev, grid)
+                         : prepare(spense_gemm_wide_kernel<0, false>, 0, dev, grid);
+  if (st) return st;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = smem_bytes_of(p);
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  const cudaError_t e = p.mode == 1     ? cudaLaunchKernelEx(&cfg, spense_gemm_wide_kernel<1, false>, p, tmap_b, tmap_ws, tmap_wd)
+                        : p.amax_part ? cudaLaunchKernelEx(&cfg, spense_gemm_wide_kernel<0, true>, p, tmap_b, tmap_ws, tmap_wd)
+                                      : cudaLaunchKernelEx(&cfg, spense_gemm_wide_kernel<0, false>, p, tmap_b, tmap_ws, tmap_wd);
+  return e == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;
+}
+
 }  // namespace spense

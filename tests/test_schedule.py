@@ -51,9 +51,9 @@ def test_spans_partition_the_stage_sequence(sp, shape, M, mode):
     assert par * (len(sb) - 1) * cps <= 148                                                # all CTAs of a launch are resident
 
 
-@pytest.mark.parametrize("M", [1, 64, 112])
+@pytest.mark.parametrize("M", [1, 64, 112, 128, 256])
 @pytest.mark.parametrize("mode", [0, 1])
-def test_decode_spans_are_balanced_in_bytes(sp, M, mode):
+def test_weight_streaming_spans_are_balanced_in_bytes(sp, M, mode):
     sb, info = sp.spense_schedule(*QWEN, M, mode)
     b = np.concatenate([np.array(t) for t in stage_layout(*QWEN, mode)])
     per_span = np.add.reduceat(b, np.array(sb[:-1]))
@@ -61,9 +61,10 @@ def test_decode_spans_are_balanced_in_bytes(sp, M, mode):
     assert per_span.max() - per_span.min() <= 2 * 40960 + 0.12 * per_span.mean()
 
 
-@pytest.mark.parametrize("M", [128, 256, 2048])
-def test_wide_spans_are_balanced_in_stages(sp, M):
-    # tensor-paced: a sparse stage (K 256) and a dense one (K 128) issue the same four MMAs, so spans hold equal stage counts
+@pytest.mark.parametrize("M", [2048, 8192])
+def test_prefill_spans_are_balanced_in_stages(sp, M):
+    # tensor-paced (3 or more token blocks): a sparse stage (K 256) and a dense one (K 128) issue the same four MMAs,
+    # so spans hold equal stage counts
     for mode in (0, 1):
         sb, info = sp.spense_schedule(*QWEN, M, mode)
         n = np.diff(np.array(sb))

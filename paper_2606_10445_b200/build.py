@@ -20,13 +20,18 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not _stale():
+def build(force: bool = False, verbose: bool = False, debug_hooks: bool = False, out: str | None = None) -> str:
+    """debug_hooks: also compile the per-CTA timeline hook (spense_debug_set_trace, not declared in spense.h) into a
+    library written to `out`; the default build exports exactly what include/spense.h declares."""
+    lib = out or LIB
+    if not debug_hooks and not force and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
            "-Xcompiler", "-fPIC", "-shared", "-I", os.path.join(ROOT, "include"), "-I", CSRC,
-           "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES] + ["-lcudart"]
+           "-o", lib] + [os.path.join(CSRC, s) for s in SOURCES] + ["-lcudart"]
+    if debug_hooks:
+        cmd.insert(1, "-DSPENSE_DEBUG_HOOKS")
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
         print(" ".join(cmd))
@@ -36,7 +41,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         raise RuntimeError("nvcc failed building libspense.so")
     if verbose:
         print(r.stdout + r.stderr)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":

@@ -2,6 +2,7 @@
 // tensor-map creation and launches.  No device allocation, no synchronisation and no device reads in the GEMM calls.
 #include <cudaTypedefs.h>
 
+#include <cstdlib>
 #include <cstring>
 #include <deque>
 #include <mutex>
@@ -241,6 +242,7 @@ int make_tmap_section(CUtensorMap* map, const uint8_t* base, size_t bytes, int b
 // bytes of span k that the PREVIOUS launch pulls into L2 during its tail: at least one ring
 constexpr uint32_t kPfNextBytes = 640u * 1024u, kPfSelfBytes = 160u * 1024u;
 constexpr int kPfPaceNs = 750;
+constexpr int kPfAheadStages = 12;   // wide kernel: L2 prefetch distance of the producer, in stages
 uint32_t next_prefetch_bytes(const Schedule& sc, int k) {
   uint32_t n = sc.span_pre[k] > kPfNextBytes ? sc.span_pre[k] : kPfNextBytes;
   return n < sc.span_len[k] ? n : sc.span_len[k];
@@ -250,6 +252,7 @@ void fill_common(GemmParams& p, const Schedule& sc, const Plan& pl, const spense
 #ifdef SPENSE_DEBUG_HOOKS
   p.trace = g_trace;
   if (g_trace) g_trace += (size_t)kMaxSpans * 16;   // debug: consecutive launches fill consecutive timelines
+  { const char* e = std::getenv("SPENSE_DBG"); p.dbg = e ? std::atoi(e) : 0; }
 #endif
   p.hdr = reinterpret_cast<const BlobHeader*>(d_blob);
   p.H = shape->H; p.I = shape->I; p.I_d = shape->I_dense;
@@ -273,6 +276,7 @@ void fill_common(GemmParams& p, const Schedule& sc, const Plan& pl, const spense
   if (pl.wide) {
     p.acc_stride = kWideMaxTokens;                            // 2 buffers x 240 columns, metadata at 480
     p.num_acc_bufs = 2;
+    p.pf_ahead = kPfAheadStages;
   } else {
     p.acc_stride = pl.n_pad <= 32 ? 32 : (pl.n_pad <= 64 ? 64 : (pl.n_pad <= 96 ? 96 : 112));
     p.num_acc_bufs = 2;                                       // 2 buffers x 2 accumulators x 112 columns = 448, metadata at 480
@@ -329,9 +333,9 @@ int gate_up_impl(const Launch& L, const spense_shape_t* shape, const void* d_blo
     p.h_f32 = d_h_f32;
     p.amax_part = dynamic ? reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes) : nullptr;
     p.ld_out = g.I; p.out_rows = g.I;
+    if (down_follows && blk0 + pl.par >= pl.nb)                // the same layer's down projection streams next
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + g.down_off, get_schedule(1, g, pl));
     if (!pl.wide) {
-      if (down_follows)                                        // the same layer's down projection streams next
-        fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + g.down_off, get_schedule(1, g, pl));
       st = launch_gemm(p, tm, pdl, L.dev, L.sms, stream);
     } else {
       st = launch_gemm_wide(p, tm, tws, twd, pdl, L.dev, L.sms, stream);
@@ -379,9 +383,9 @@ int down_impl(const Launch& L, const spense_shape_t* shape, const void* d_blob, 
     p.y = d_y;
     p.y_dtype = y_dtype;
     p.ld_out = g.H; p.out_rows = g.H;
+    if (d_next_blob && blk0 + pl.par >= pl.nb)                 // the next layer's gate/up weights stream next
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + g.gate_up_off, get_schedule(0, g, pl));
     if (!pl.wide) {
-      if (d_next_blob)                                         // the next layer's gate/up weights stream next
-        fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + g.gate_up_off, get_schedule(0, g, pl));
       st = launch_gemm(p, tm, pdl, L.dev, L.sms, stream);
     } else {
       st = launch_gemm_wide(p, tm, tws, twd, pdl, L.dev, L.sms, stream);

@@ -252,37 +252,6 @@ __device__ __forceinline__ void epilogue_tables(const GemmParams& p, const Ctx& 
   }
 }
 
-// 8 token columns of both accumulators of a pair tile, as one thread holds them.
-//   MODE 1 (32x32b loads): v[8 a + i] = operand a, lane 32 q + t, column c + i.
-//   MODE 0 (16x256b loads of the gate half and the up half of the quadrant): v[8 a + 4 gu + k] = operand a,
-//          lane 32 q + 16 gu + t/4 + 8 (k >> 1), column c + 2 (t % 4) + (k & 1)   (gu = 0 gate, 1 up).
-template <int MODE>
-__device__ __forceinline__ void load_acc(uint32_t t0, uint32_t t1, int c, float (&v)[16]) {
-  if (MODE == 1) {
-    uint32_t r0[8], r1[8];
-    tmem_ld8(t0 + c, r0);
-    tmem_ld8(t1 + c, r1);
-    tmem_ld_wait();
-#pragma unroll
-    for (int i = 0; i < 8; ++i) { v[i] = __uint_as_float(r0[i]); v[8 + i] = __uint_as_float(r1[i]); }
-  } else {
-    uint32_t r[4][4];
-    tmem_ld_16x256b(t0 + c, r[0]);
-    tmem_ld_16x256b(t0 + (16u << 16) + c, r[1]);
-    tmem_ld_16x256b(t1 + c, r[2]);
-    tmem_ld_16x256b(t1 + (16u << 16) + c, r[3]);
-    tmem_ld_wait();
-#pragma unroll
-    for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i >> 2][i & 3]);
-  }
-}
-// (lane, column) of element i of load_acc inside a [col][128 lanes] partial image; q = lane quadrant, t = lane of the warp
-template <int MODE>
-__device__ __forceinline__ int part_index(int i, int q, int t, int c) {
-  if (MODE == 1) return (c + (i & 7)) * 128 + 32 * q + t;
-  return (c + 2 * (t & 3) + (i & 1)) * 128 + 32 * q + 16 * ((i >> 2) & 1) + (t >> 2) + 8 * ((i >> 1) & 1);
-}
-
 // ===================== epilogue (16 warps) =====================
 // warp & 3 selects the TMEM lane quadrant, (warp - 4) >> 2 the quarter of the token columns.  Once the CTA's last
 // accumulator is complete the stage ring is idle and stages the partials (bulk copies).
@@ -328,43 +297,22 @@ __device__ __forceinline__ void epilogue(const GemmParams& p, const Ctx& cx, int
     const uint32_t t1 = t0 + (uint32_t)p.acc_stride;
 
     if (a == b || (b == a + 1 && span == a)) {
-      // the whole tile is ours, or we own a tile whose tail the next span has (usually long ago) dumped: that is the
-      // last segment of this span, every MMA of the CTA is complete and the ring stages the partner's partial
-      const bool add = a != b;
-      if (add) {
-        const float* part = partials + (size_t)b * 2 * part_floats;   // span b starts inside the tile: its first segment
-        if (et == 0) {
-          wait_flag(p, flags + b * 2, epoch);
-          asm volatile("fence.proxy.async.global;" ::: "memory");   // partner's generic-proxy stores -> our async-proxy read
-          mbar_expect_tx(cx.red_bar(), 2u * (uint32_t)cols_used * 512u);
-          bulk_g2s(cx.smem_base, part, (uint32_t)cols_used * 512u, cx.red_bar(), policy_evict_first());
-          bulk_g2s(cx.smem_base + (uint32_t)cols_used * 512u, part + (size_t)p.n_pad * 128, (uint32_t)cols_used * 512u, cx.red_bar(), policy_evict_first());
-        }
-        wait_bar(p, cx.red_bar(), red_round & 1u);
-        ++red_round;
+      // the whole tile is ours, or we own a tile whose tail the next span has (usually long ago) dumped
+      const float* part = nullptr;
+      if (a != b) {
+        wait_flag(p, flags + b * 2, epoch);                // every thread: one ld.acquire when the partner is done (the usual case)
+        part = partials + (size_t)b * 2 * part_floats;     // span b starts inside the tile: its first segment
         if (et == 0) trace(p, span, 8);
       }
       if (seg_end == se && n_groups == 0 && et == 0) *cx.epi_done_ptr() = 1;   // last epilogue of this CTA: stop prefetching now
+#pragma unroll
+      for (int opnd = 0; opnd < 2; ++opnd) {
+        const uint32_t t_op = opnd ? t1 : t0;
+        const float* part_op = part ? part + (size_t)opnd * p.n_pad * 128 : nullptr;
+        int c = c_begin;
 #pragma unroll 1
-      for (int c = c_begin; c < c_end; c += 8) {
-        float v[16];
-        load_acc<MODE>(t0, t1, c, v);
-        if (add) {
-#pragma unroll
-          for (int i = 0; i < 16; ++i) v[i] += stg[(size_t)(i >> 3) * cols_used * 128 + part_index<MODE>(i, q, lane, c)];
-        }
-        if (MODE == 0) {
-          glu_chunk<DYN>(p, sc4, cur.tile, 16 * q, c, Mb, 0, reinterpret_cast<const float(&)[4]>(v[0]), reinterpret_cast<const float(&)[4]>(v[4]));
-          glu_chunk<DYN>(p, sc4, cur.tile, 64 + 16 * q, c, Mb, 0, reinterpret_cast<const float(&)[4]>(v[8]), reinterpret_cast<const float(&)[4]>(v[12]));
-        } else {
-#pragma unroll
-          for (int i = 0; i < 8; ++i)
-            if (c + i < Mb) {
-              const float kx = sc1[c + i];
-              store_y(p, cur.tile * 256 + 32 * q + lane, c + i, v[i] * kx);
-              store_y(p, cur.tile * 256 + 128 + 32 * q + lane, c + i, v[8 + i] * kx);
-            }
-        }
+        for (; c + 16 <= c_end; c += 16) tile_block<MODE, DYN, 2>(p, sc4, sc1, t_op, part_op, cur.tile, opnd, q, lane, c, Mb, 0);
+        if (c < c_end) tile_block<MODE, DYN, 1>(p, sc4, sc1, t_op, part_op, cur.tile, opnd, q, lane, c, Mb, 0);
       }
       tc_fence_before();
       mbar_arrive(cx.acce_bar(buf));

@@ -125,8 +125,10 @@ __device__ __forceinline__ void wait_bar(const GemmParams& p, uint32_t bar, uint
 #pragma unroll 1
   for (;;) {
 #pragma unroll 1
-    for (int i = 0; i < 32; ++i)
+    for (int i = 0; i < 32; ++i) {
       if (mbar_try(bar, parity)) return;
+      if ((p.dbg & 4) && threadIdx.x >= 128) __nanosleep(200);
+    }
     if (globaltimer() - t0 > kWaitBudgetNs) give_up(p.status, SPENSE_ERR_TIMEOUT);
   }
 }
@@ -184,30 +186,66 @@ __device__ __forceinline__ float finish_glu(const GemmParams& p, const float4* s
   return 0.0f;
 }
 
-// Epilogue of one 8-column chunk of ONE gate_up operand read with two tcgen05.ld.16x256b (gate half, up half of the
-// warp's lane quadrant): thread t holds lanes t/4 (k = 0, 1) and t/4 + 8 (k = 2, 3), columns c + 2 (t % 4) + (k & 1).
-// j0 = index inside the pair tile of the quadrant's first lane (64 a + 16 q).  Called by all 32 lanes.
-template <bool DYN>
-__device__ __forceinline__ void glu_chunk(const GemmParams& p, float4* sc4, int tile, int j0, int c, int Mb, int m_base,
-                                          const float (&g)[4], const float (&u)[4]) {
-  const int t = threadIdx.x & 31;
-  float mx[2] = {0.0f, 0.0f};
-#pragma unroll
-  for (int k = 0; k < 4; ++k) {
-    const int col = c + 2 * (t & 3) + (k & 1);
-    const int j = j0 + (t >> 2) + 8 * (k >> 1);
-    if (col < Mb) mx[k & 1] = fmaxf(mx[k & 1], finish_glu<DYN>(p, sc4, tile, j, col, m_base + col, g[k], u[k]));
+// NG groups of 8 token columns of ONE gate_up operand, read with two tcgen05.ld.16x256b.xNG (gate half, up half of the
+// warp's lane quadrant): thread t holds, for group j, lanes t/4 (k = 4 j + 0, 1) and t/4 + 8 (k = 4 j + 2, 3), columns
+// c + 8 j + 2 (t % 4) + (k & 1).
+template <int NG>
+__device__ __forceinline__ void load_glu(uint32_t t_gate, int c, float (&g)[4 * NG], float (&u)[4 * NG]) {
+  uint32_t rg[4 * NG], ru[4 * NG];
+  if (NG == 1) {
+    tmem_ld_16x256b(t_gate + c, reinterpret_cast<uint32_t(&)[4]>(rg[0]));
+    tmem_ld_16x256b(t_gate + (16u << 16) + c, reinterpret_cast<uint32_t(&)[4]>(ru[0]));
+  } else if (NG == 2) {
+    tmem_ld_16x256b_x2(t_gate + c, reinterpret_cast<uint32_t(&)[8]>(rg[0]));
+    tmem_ld_16x256b_x2(t_gate + (16u << 16) + c, reinterpret_cast<uint32_t(&)[8]>(ru[0]));
+  } else {
+    tmem_ld_16x256b_x4(t_gate + c, reinterpret_cast<uint32_t(&)[16]>(rg[0]));
+    tmem_ld_16x256b_x4(t_gate + (16u << 16) + c, reinterpret_cast<uint32_t(&)[16]>(ru[0]));
   }
-  if (DYN) {
-    // max|h| of the 16 indices per token column: over the 8 threads that share t % 4, then one shared atomic each
+  tmem_ld_wait();
+#pragma unroll
+  for (int i = 0; i < 4 * NG; ++i) { g[i] = __uint_as_float(rg[i]); u[i] = __uint_as_float(ru[i]); }
+}
+// index of element k of load_glu (gu = 0 gate, 1 up) inside a [col][128 lanes] partial image; q = lane quadrant
+__device__ __forceinline__ int glu_part_index(int k, int gu, int q, int t, int c) {
+  return (c + 8 * (k >> 2) + 2 * (t & 3) + (k & 1)) * 128 + 32 * q + 16 * gu + (t >> 2) + 8 * ((k >> 1) & 1);
+}
+// their epilogue.  j0 = index inside the pair tile of the quadrant's first lane (64 a + 16 q); sc4 = float4 per token column
+// {s_x*s_gate, s_x*s_up, s_h, RN(1/s_h)}.  Called by all 32 lanes.
+template <bool DYN, int NG>
+__device__ __forceinline__ void glu_block(const GemmParams& p, float4* sc4, int tile, int j0, int c, int Mb, int m_base,
+                                          const float (&g)[4 * NG], const float (&u)[4 * NG]) {
+  const int t = threadIdx.x & 31;
+  const int jr = tile * 128 + j0 + (t >> 2);
+#pragma unroll
+  for (int j = 0; j < NG; ++j) {
 #pragma unroll
     for (int e = 0; e < 2; ++e) {
-      float m = mx[e];
-      m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 4));
-      m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 8));
-      m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 16));
-      const int col = c + 2 * t + e;
-      if (t < 4 && col < Mb) atomicMax(reinterpret_cast<int*>(sc4 + col) + 2, __float_as_int(m));   // |h| >= 0: int order == float order
+      const int col = c + 8 * j + 2 * (t & 3) + e;
+      float mx = 0.0f;
+      if (col < Mb) {
+        const float4 k = sc4[col];
+        const size_t o = (size_t)(m_base + col) * p.ld_out + jr;
+#pragma unroll
+        for (int li = 0; li < 2; ++li) {
+          const int i = 4 * j + 2 * li + e;
+          const float h = silu_mul(g[i] * k.x, u[i] * k.y);
+          if (DYN) {
+            p.h_f32[o + 8 * li] = h;
+            mx = fmaxf(mx, fabsf(h));
+          } else {
+            if (p.h_f32) p.h_f32[o + 8 * li] = h;
+            p.hq[o + 8 * li] = (uint8_t)(to_e4m3x2(div_by(h, k.z, k.w), 0.0f) & 0xFFu);
+          }
+        }
+      }
+      if (DYN) {
+        // max|h| of the 16 indices per token column: over the 8 threads that share t % 4, then one shared atomic each
+        mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 4));
+        mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 8));
+        mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 16));
+        if (t < 4 && col < Mb) atomicMax(reinterpret_cast<int*>(sc4 + col) + 2, __float_as_int(mx));   // |h| >= 0: int order == float order
+      }
     }
   }
 }
@@ -218,6 +256,45 @@ __device__ __forceinline__ void store_y(const GemmParams& p, int out_row, int m_
   const size_t o = (size_t)m_out * p.ld_out + out_row;
   if (p.y_dtype == SPENSE_F32) reinterpret_cast<float*>(p.y)[o] = y;
   else reinterpret_cast<__nv_bfloat16*>(p.y)[o] = __float2bfloat16_rn(y);
+}
+
+// Epilogue of NG groups of 8 token columns of ONE accumulator (operand `opnd` of the pair tile; one lane quadrant per
+// warp); `part` = the partner's partial [col][lane] of that operand to add first (owner of a tile split over two spans),
+// read straight from L2, or nullptr.
+template <int MODE, bool DYN, int NG>
+__device__ __forceinline__ void tile_block(const GemmParams& p, float4* sc4, const float* sc1, uint32_t t0, const float* part, int tile,
+                                           int opnd, int q, int lane, int c, int Mb, int m_base) {
+  if (MODE == 0) {
+    float g[4 * NG], u[4 * NG], pg[4 * NG], pu[4 * NG];
+    if (part) {
+#pragma unroll
+      for (int i = 0; i < 4 * NG; ++i) {
+        pg[i] = __ldcg(part + glu_part_index(i, 0, q, lane, c));
+        pu[i] = __ldcg(part + glu_part_index(i, 1, q, lane, c));
+      }
+    }
+    load_glu<NG>(t0, c, g, u);
+    if (part) {
+#pragma unroll
+      for (int i = 0; i < 4 * NG; ++i) { g[i] += pg[i]; u[i] += pu[i]; }
+    }
+    glu_block<DYN, NG>(p, sc4, tile, 64 * opnd + 16 * q, c, Mb, m_base, g, u);
+  } else {
+    uint32_t r[8 * NG];
+    float pv[8 * NG];
+    if (part) {
+#pragma unroll
+      for (int i = 0; i < 8 * NG; ++i) pv[i] = __ldcg(part + (size_t)(c + i) * 128 + 32 * q + lane);
+    }
+    if (NG == 1) tmem_ld8(t0 + c, reinterpret_cast<uint32_t(&)[8]>(r[0]));
+    else if (NG == 2) tmem_ld16(t0 + c, reinterpret_cast<uint32_t(&)[16]>(r[0]));
+    else tmem_ld32(t0 + c, reinterpret_cast<uint32_t(&)[32]>(r[0]));
+    tmem_ld_wait();
+    const int row = tile * 256 + 128 * opnd + 32 * q + lane;
+#pragma unroll
+    for (int i = 0; i < 8 * NG; ++i)
+      if (c + i < Mb) store_y(p, row, m_base + c + i, (__uint_as_float(r[i]) + (part ? pv[i] : 0.0f)) * sc1[c + i]);
+  }
 }
 
 // where operand row `lane` of a gate_up operand comes from (blob layout, spense_internal.cuh): index inside the operand's

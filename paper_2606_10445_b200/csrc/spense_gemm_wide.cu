@@ -16,8 +16,9 @@
 //     only cp.async.bulk.tensor has the .cta_group::2 form whose completion counts on the LEADER CTA's barrier: the
 //     leader's MMA thread waits on one barrier for both CTAs' halves of a stage.
 //
-// Roles per CTA (640 threads): warp 0 producer (its operand + its half of the token tile), warp 1 MMA issuer (leader CTA
-// only), warp 2 TMEM allocator, warps 4-19 epilogue of the CTA's own 128 accumulator lanes.  The split-K fix-up is the
+// Roles per CTA (640 threads): warp 0 weight producer (the CTA's operand), warp 3 activation producer (its half of the
+// token tile), warp 1 MMA issuer (leader CTA only), warp 2 TMEM allocator, warps 4-19 epilogue of the CTA's own 128
+// accumulator lanes.  The split-K fix-up is the
 // decode kernel's, per CTA: its partners are the CTAs of the same rank in the neighbouring spans of the same token block.
 #include <mutex>
 
@@ -53,141 +54,199 @@ struct Ctx {
   __device__ __forceinline__ uint32_t red_bar() const { return bar_base + 8u * 22; }
   __device__ __forceinline__ volatile uint32_t* tmem_slot_ptr() const { return reinterpret_cast<volatile uint32_t*>(smem_gen + ring_bytes + 8 * 20); }
   __device__ __forceinline__ volatile int* epoch_ptr() const { return reinterpret_cast<volatile int*>(smem_gen + ring_bytes + 8 * 21); }
+  __device__ __forceinline__ volatile int* epi_done_ptr() const { return reinterpret_cast<volatile int*>(smem_gen + ring_bytes + 8 * 23); }
   __device__ __forceinline__ float4* sc0() const { return reinterpret_cast<float4*>(smem_gen + ring_bytes + 256); }
   __device__ __forceinline__ float* sc1(int n_pad) const { return reinterpret_cast<float*>(smem_gen + ring_bytes + 256 + 16 * n_pad); }
 };
 
 struct Group { int a, b, tile, first; };
 
-// ===================== producer (one thread per CTA) =====================
+// The three roles below run with their WHOLE warp converged and one elected lane issuing: every value they compute is
+// warp-uniform (the compiler keeps it in uniform registers, which is where TMA / tcgen05 instructions take their operands
+// from), and their loops are a few dozen instructions per stage.  That matters here: a stage is only 4 MMAs of 64-120
+// cycles, and a single thread working through ~150 dependent instructions per stage (descriptor construction, cursor
+// bookkeeping) was the bottleneck of the first version of this kernel (measured: the MMA thread busy 350 ns per stage
+// with the tensor pipe 26 % active).
+
 // Slot image: [operand: values 16 KB | metadata 4 KB] [token half-tile(s): n_pad/2 rows x 128 B, two for a sparse stage].
-// Every copy counts on the LEADER's full barrier; the leader's producer arms it with the bytes of both CTAs.
+// Every copy counts on the LEADER's full barrier; the leader's weight producer arms it with the bytes of both CTAs.
+
+// ===================== weight producer (warp 0 of each CTA) =====================
+// This CTA's operand of every stage of the span; weights never depend on the previous kernel of the stream.
 template <int MODE>
-__device__ __forceinline__ void producer(const GemmParams& p, const CUtensorMap* tmap_b, const CUtensorMap* tmap_ws,
-                                         const CUtensorMap* tmap_wd, const Ctx& cx, int span) {
+__device__ __forceinline__ void producer_weights(const GemmParams& p, const CUtensorMap* tmap_ws, const CUtensorMap* tmap_wd,
+                                                 const Ctx& cx, int span) {
+  const bool issuer = elect_one();
   const int S = cx.S;
   const int sb = p.span_begin[span];
   const int n = p.span_begin[span + 1] - sb;
   // one token block: a weight byte is used once (evict first); several: the pairs of the other blocks read the same
   // stage at about the same time and should find it in L2
   const uint64_t pol_w = p.nb == 1 ? policy_evict_first() : policy_evict_normal();
-  const uint64_t pol_a = policy_evict_last();
   unsigned long long off;
   Cursor c = cursor_at<MODE>(p, sb, &off);
-  uint32_t row = (uint32_t)(off >> 7);                     // position in the section, in rows of 128 bytes
-  uint32_t info[8];                                        // stages whose weights are in flight: K coordinate | sparse << 31
-  const int tok0 = cx.blk * p.n_pad + (int)cx.rank * (p.n_pad >> 1);   // first token row of this CTA's half
-
-  int w = 0;
-  uint32_t inf_last = 0;
-  int w_slot = 0, w_round = 0, b_slot = 0;
-  auto issue_weight = [&](bool blocking) -> bool {
+  uint32_t row = (uint32_t)(off >> 7) + cx.rank * (uint32_t)(c.j < c.ns ? kSparseOperandBytes >> 7 : kOperandBytes >> 7);
+  const uint32_t lead_full0 = mapa_shared(cx.full_bar(0), 0);
+  const uint32_t tx_s = 2u * ((uint32_t)kSparseOperandBytes + 2u * cx.b_half_bytes), tx_d = 2u * ((uint32_t)kOperandBytes + cx.b_half_bytes);
+  // L2 prefetch of this CTA's operand pf_ahead stages ahead of the copies (pairs of the launch's first token block)
+  const bool do_pf = p.pf_ahead > 0 && cx.blk == p.blk0;
+  Cursor cp = c;
+  uint32_t row_pf = row;
+  int pf = 0;
+  auto prefetch_to = [&](int upto) {
+    if (upto > n) upto = n;
+#pragma unroll 1
+    for (; pf < upto; ++pf) {
+      const bool sp = cp.j < cp.ns;
+      const uint32_t rows = sp ? (uint32_t)(kSparseOperandBytes >> 7) : (uint32_t)(kOperandBytes >> 7);
+      if (pf >= S && issuer)                               // the first ring is fetched by the copies themselves
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p.section + ((size_t)row_pf << 7)), "r"(rows << 7) : "memory");
+      row_pf += 2u * rows;
+      if (++cp.j == cp.ns + cp.nd) next_tile<MODE>(p, cp);
+      if ((cp.j < cp.ns) != sp) row_pf += cx.rank * (uint32_t)(sp ? -32 : 32);   // the other stage kind: operand 1 starts 32 rows earlier / later
+    }
+  };
+  int slot = 0;
+  uint32_t par = 1;                                        // parity a fresh empty barrier passes
+  uint32_t dst = cx.smem_base, fb_lead = lead_full0, fb = cx.full_bar(0), eb = cx.empty_bar(0);
+#pragma unroll 1
+  for (int w = 0; w < n; ++w) {
     const bool sp = c.j < c.ns;
-    const uint32_t inf = (uint32_t)(sp ? c.j * kSparseStageK : p.dense_k0 + (c.j - c.ns) * kDenseStageK) | (sp ? 0x80000000u : 0u);
-    const uint32_t opb = sp ? (uint32_t)kSparseOperandBytes : (uint32_t)kOperandBytes;
-    const uint32_t tx = 2u * (opb + (sp ? 2u : 1u) * cx.b_half_bytes);
-    const uint32_t fb = mapa_shared(cx.full_bar(w_slot), 0);
-    const uint32_t dst = cx.smem_base + (uint32_t)w_slot * cx.slot_bytes;
-    if (w_round > 0) {
-      const uint32_t par = ((uint32_t)w_round & 1u) ^ 1u;
-      if (blocking) wait_bar(p, cx.empty_bar(w_slot), par);
-      else if (!mbar_try(cx.empty_bar(w_slot), par)) return false;
+    const uint32_t rows = sp ? (uint32_t)(kSparseOperandBytes >> 7) : (uint32_t)(kOperandBytes >> 7);
+    if (w >= S) wait_bar(p, eb, par);
+    if (issuer) {
+      if (cx.rank == 0) mbar_expect_tx(fb, sp ? tx_s : tx_d);
+      tma_load_2d_pair(dst, sp ? tmap_ws : tmap_wd, 0, (int)row, fb_lead, pol_w);
     }
-    if (cx.rank == 0) mbar_expect_tx(cx.full_bar(w_slot), tx);
-    tma_load_2d_pair(dst, sp ? tmap_ws : tmap_wd, 0, (int)(row + cx.rank * (opb >> 7)), fb, pol_w);
-    inf_last = inf;
-    if (!blocking) {
-#pragma unroll
-      for (int k = 0; k < 8; ++k)
-        if (k == (w & 7)) info[k] = inf;
-    }
-    row += 2u * (opb >> 7);
+    row += 2u * rows;
     if (++c.j == c.ns + c.nd) next_tile<MODE>(p, c);
-    ++w;
-    if (++w_slot == S) { w_slot = 0; ++w_round; }
-    return true;
-  };
-  auto load_b = [&](int slot, uint32_t inf) {
-    const uint32_t b_dst = cx.smem_base + (uint32_t)slot * cx.slot_bytes + kSparseOperandBytes;
-    const uint32_t fb = mapa_shared(cx.full_bar(slot), 0);
-    const int k0 = (int)(inf & 0x7FFFFFFFu);
-    tma_load_2d_pair(b_dst, tmap_b, k0, tok0, fb, pol_a);
-    if (inf >> 31) tma_load_2d_pair(b_dst + cx.b_half_bytes, tmap_b, k0 + 128, tok0, fb, pol_a);
-  };
-
-  // weights never depend on the previous kernel of the stream, activations do
-#pragma unroll 1
-  while (w < n && w < S && issue_weight(false)) {}
-  trace(p, span, 1);
-  pdl_wait();
-#pragma unroll 1
-  for (int b = 0; b < n; ++b) {
-    uint32_t inf = 0;
-    if (w <= b) {
-      issue_weight(true);
-      inf = inf_last;
-    } else {
-#pragma unroll
-      for (int k = 0; k < 8; ++k)
-        if (k == (b & 7)) inf = info[k];
-    }
-    load_b(b_slot, inf);
-    if (++b_slot == S) b_slot = 0;
+    if ((c.j < c.ns) != sp) row += cx.rank * (uint32_t)(sp ? -32 : 32);   // the other stage kind: operand 1 starts 32 rows earlier / later
+    if (++slot == S) { slot = 0; par ^= 1u; dst = cx.smem_base; fb_lead = lead_full0; fb = cx.full_bar(0); eb = cx.empty_bar(0); }
+    else { dst += cx.slot_bytes; fb_lead += 8u; fb += 8u; eb += 8u; }
+    if (do_pf) prefetch_to(w + 1 + p.pf_ahead);
+    if (w == 0) trace(p, span, 1);
   }
 }
 
-// ===================== MMA issuer (one thread of the leader CTA) =====================
+// ===================== activation producer (warp 3 of each CTA) =====================
+// This CTA's half of the token tile of every stage; waits for the previous kernel of the stream first.
+template <int MODE>
+__device__ __forceinline__ void producer_tokens(const GemmParams& p, const CUtensorMap* tmap_b, const Ctx& cx, int span) {
+  const bool issuer = elect_one();
+  const int S = cx.S;
+  const int sb = p.span_begin[span];
+  const int n = p.span_begin[span + 1] - sb;
+  const uint64_t pol_a = policy_evict_last();
+  unsigned long long off;
+  Cursor c = cursor_at<MODE>(p, sb, &off);
+  const uint32_t lead_full0 = mapa_shared(cx.full_bar(0), 0);
+  const int tok0 = cx.blk * p.n_pad + (int)cx.rank * (p.n_pad >> 1);   // first token row of this CTA's half
+  pdl_wait();
+  int slot = 0;
+  uint32_t par = 1;
+  uint32_t dst = cx.smem_base + kSparseOperandBytes, fb_lead = lead_full0, eb = cx.empty_bar(0);
+#pragma unroll 1
+  for (int b = 0; b < n; ++b) {
+    const bool sp = c.j < c.ns;
+    const int k0 = sp ? c.j * kSparseStageK : p.dense_k0 + (c.j - c.ns) * kDenseStageK;
+    if (b >= S) wait_bar(p, eb, par);
+    if (issuer) {
+      tma_load_2d_pair(dst, tmap_b, k0, tok0, fb_lead, pol_a);
+      if (sp) tma_load_2d_pair(dst + cx.b_half_bytes, tmap_b, k0 + 128, tok0, fb_lead, pol_a);
+    }
+    if (++c.j == c.ns + c.nd) next_tile<MODE>(p, c);
+    if (++slot == S) { slot = 0; par ^= 1u; dst = cx.smem_base + kSparseOperandBytes; fb_lead = lead_full0; eb = cx.empty_bar(0); }
+    else { dst += cx.slot_bytes; fb_lead += 8u; eb += 8u; }
+  }
+}
+
+// L2 prefetch of what the NEXT kernel of the stream streams first, issued while this CTA runs its fix-up tail (pairs of the
+// launch's first token block; each CTA of the pair takes half of the span's range): one 32 KB chunk per pf_pace_ns so the
+// fix-up traffic is not queued behind it; stops with the epilogue.
+__device__ __forceinline__ void prefetch_next(const GemmParams& p, const Ctx& cx, int span) {
+  if (!p.next_base || cx.blk != p.blk0) return;
+  const uint32_t half = (p.next_len[span] >> 1) & ~1023u;
+  const uint8_t* nb = p.next_base + (size_t)p.next_off[span] + (size_t)cx.rank * half;
+  long long t_next = globaltimer();
+#pragma unroll 1
+  for (uint32_t o = 0; o < half && *cx.epi_done_ptr() == 0; o += 32768u) {
+    const uint32_t chunk = half - o < 32768u ? half - o : 32768u;
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(nb + o), "r"(chunk) : "memory");
+    t_next += p.pf_pace_ns;
+    while (globaltimer() < t_next && *cx.epi_done_ptr() == 0) __nanosleep(64);
+  }
+}
+
+// shared-memory matrix descriptors as two words: lo = address >> 4 | LBO >> 4 << 16 (so stepping through a slot or the ring
+// is an add on lo), hi = SBO >> 4 | version | layout (constant)
+__device__ __forceinline__ uint32_t desc_lo(uint32_t saddr, uint32_t lbo_bytes) { return ((saddr >> 4) & 0x3FFFu) | (((lbo_bytes >> 4) & 0x3FFFu) << 16); }
+__device__ __forceinline__ uint32_t desc_hi(uint32_t sbo_bytes, uint32_t layout) { return ((sbo_bytes >> 4) & 0x3FFFu) | (1u << 14) | (layout << 29); }
+__device__ __forceinline__ uint64_t desc_of(uint32_t lo, uint32_t hi) { return (uint64_t)lo | ((uint64_t)hi << 32); }
+
+// ===================== MMA issuer (warp 1 of the leader CTA) =====================
 template <int MODE>
 __device__ __forceinline__ void mma_issuer(const GemmParams& p, const Ctx& cx, int span) {
+  const bool issuer = elect_one();
   const int S = cx.S;
   const uint32_t idesc_d = (1u << 4) | ((uint32_t)(p.n_pad >> 3) << 17) | ((256u >> 4) << 24);
   const uint32_t idesc_s = idesc_d | (1u << 2);
   const int sb = p.span_begin[span], se = p.span_begin[span + 1];
   unsigned long long off;
   Cursor c = cursor_at<MODE>(p, sb, &off);
-  int slot = 0, it = 0, seg = 0;
-  uint32_t ph = 0;
+  const uint32_t hi_sw = desc_hi(1024, kLayoutSW128), hi_meta = desc_hi(128, kLayoutNone);
+  const uint32_t a_lo0 = desc_lo(cx.smem_base, 16), slot16 = cx.slot_bytes >> 4, bh16 = cx.b_half_bytes >> 4;
+  uint32_t a_lo = a_lo0;                                    // operand of the current slot; tokens at + kSparseOperandBytes
+  int slot = 0, seg = 0;
+  uint32_t ph = 0, it = 0;
+  uint32_t fb = cx.full_bar(0), eb = cx.empty_bar(0);
+  long long t_full = 0, t_acce = 0;
 #pragma unroll 1
   for (int s = sb; s < se; ++seg) {
     const int tile_end = c.first + c.ns + c.nd;
     const int seg_end = min(se, tile_end);
     const int buf = seg & 1;
     const uint32_t use = (uint32_t)(seg >> 1);
+    long long tw0 = p.trace ? globaltimer() : 0;
     wait_bar(p, cx.acce_bar(buf), (use & 1u) ^ 1u);        // both CTAs' epilogues have drained this accumulator
+    if (p.trace) t_acce += globaltimer() - tw0;
     tc_fence_after();
     const uint32_t d = cx.tmem_base + (uint32_t)(buf * p.acc_stride);
     uint32_t acc = 0;
 #pragma unroll 1
     for (; s < seg_end; ++s, ++it, ++c.j) {
-      wait_bar(p, cx.full_bar(slot), ph);
+      if (p.trace) tw0 = globaltimer();
+      wait_bar(p, fb, ph);
+      if (p.trace) t_full += globaltimer() - tw0;
       tc_fence_after();
       if (s == sb) trace(p, span, 3);
-      const uint32_t a0 = cx.smem_base + (uint32_t)slot * cx.slot_bytes;
-      const uint32_t b0 = a0 + kSparseOperandBytes;
-      if (c.j < c.ns) {
-        const uint32_t e_base = cx.tmem_base + kMetaCol + (uint32_t)(it & 1) * 8u;
-        tc_cp_128x128b_pair(e_base, make_desc(a0 + kOperandBytes, 0, 128, kLayoutNone));
-        tc_cp_128x128b_pair(e_base + 4u, make_desc(a0 + kOperandBytes + 2048u, 0, 128, kLayoutNone));
+      const uint32_t b_lo = a_lo + (kSparseOperandBytes >> 4);
+      if (issuer && !(p.dbg & 2)) {
+        if (c.j < c.ns) {
+          const uint32_t e_base = cx.tmem_base + kMetaCol + (it & 1u) * 8u;
+          const uint32_t m_lo = (a_lo & 0x3FFFu) + (kOperandBytes >> 4);     // metadata atoms: LBO 0
+          tc_cp_128x128b_pair(e_base, desc_of(m_lo, hi_meta));
+          tc_cp_128x128b_pair(e_base + 4u, desc_of(m_lo + (2048u >> 4), hi_meta));
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {                     // 4 sparse MMAs of K = 64 logical (32 B of A, 64 B of B)
-          const uint64_t bd = make_desc(b0 + (uint32_t)(k >> 1) * cx.b_half_bytes + (uint32_t)(k & 1) * 64u, 16, 1024, kLayoutSW128);
-          mma_f8_sparse_pair(d, make_desc(a0 + 32u * k, 16, 1024, kLayoutSW128), bd, e_base + 2u * k, idesc_s, acc);
-          acc = 1;
-        }
-      } else {
+          for (uint32_t k = 0; k < 4; ++k) {              // 4 sparse MMAs of K = 64 logical (32 B of A, 64 B of B)
+            mma_f8_sparse_pair(d, desc_of(a_lo + 2u * k, hi_sw), desc_of(b_lo + (k >> 1) * bh16 + (k & 1u) * 4u, hi_sw), e_base + 2u * k,
+                               idesc_s, acc | k);
+          }
+        } else {
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {                     // 4 dense MMAs of K = 32
-          mma_f8_dense_pair(d, make_desc(a0 + 32u * k, 16, 1024, kLayoutSW128), make_desc(b0 + 32u * k, 16, 1024, kLayoutSW128), idesc_d, acc);
-          acc = 1;
+          for (uint32_t k = 0; k < 4; ++k)                // 4 dense MMAs of K = 32
+            mma_f8_dense_pair(d, desc_of(a_lo + 2u * k, hi_sw), desc_of(b_lo + 2u * k, hi_sw), idesc_d, acc | k);
         }
       }
-      tc_commit_pair(cx.empty_bar(slot), 3);              // both CTAs' slots are free once these MMAs have read them
-      if (++slot == S) { slot = 0; ph ^= 1u; }
+      acc = 1;
+      if (issuer) tc_commit_pair(eb, 3);                  // both CTAs' slots are free once these MMAs have read them
+      if (++slot == S) { slot = 0; ph ^= 1u; a_lo = a_lo0; fb = cx.full_bar(0); eb = cx.empty_bar(0); }
+      else { a_lo += slot16; fb += 8u; eb += 8u; }
     }
-    tc_commit_pair(cx.accf_bar(buf), 3);                  // accumulator complete in both CTAs
+    if (issuer) tc_commit_pair(cx.accf_bar(buf), 3);      // accumulator complete in both CTAs
     if (s == tile_end) next_tile<MODE>(p, c);
   }
   trace(p, span, 4);
+  if (p.trace && cx.blk == p.blk0 && issuer) { p.trace[(size_t)span * 16 + 11] = t_full; p.trace[(size_t)span * 16 + 12] = t_acce; }
 }
 
 // scale tables of the pair's token block (weight scales come from the blob header, on the device)
@@ -206,29 +265,6 @@ __device__ __forceinline__ void epilogue_tables(const GemmParams& p, const Ctx& 
   }
 }
 
-// 8 token columns of the CTA's accumulator as one thread holds them.
-//   MODE 1 (32x32b): v[i] = lane 32 q + t, column c + i.
-//   MODE 0 (16x256b of the gate half and of the up half of the quadrant): v[4 gu + k] = lane 32 q + 16 gu + t/4 + 8 (k >> 1),
-//          column c + 2 (t % 4) + (k & 1).
-template <int MODE>
-__device__ __forceinline__ void load_acc(uint32_t t0, int c, float (&v)[8]) {
-  uint32_t r[8];
-  if (MODE == 1) {
-    tmem_ld8(t0 + c, r);
-  } else {
-    tmem_ld_16x256b(t0 + c, reinterpret_cast<uint32_t(&)[4]>(r[0]));
-    tmem_ld_16x256b(t0 + (16u << 16) + c, reinterpret_cast<uint32_t(&)[4]>(r[4]));
-  }
-  tmem_ld_wait();
-#pragma unroll
-  for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
-}
-template <int MODE>
-__device__ __forceinline__ int part_index(int i, int q, int t, int c) {
-  if (MODE == 1) return (c + i) * 128 + 32 * q + t;
-  return (c + 2 * (t & 3) + (i & 1)) * 128 + 32 * q + 16 * (i >> 2) + (t >> 2) + 8 * ((i >> 1) & 1);
-}
-
 // ===================== epilogue (16 warps per CTA, the CTA's own 128 lanes) =====================
 template <int MODE, bool DYN>
 __device__ __forceinline__ void epilogue(const GemmParams& p, const Ctx& cx, int span, int epoch) {
@@ -241,7 +277,7 @@ __device__ __forceinline__ void epilogue(const GemmParams& p, const Ctx& cx, int
   const int cols_per = (((p.n_pad + 3) >> 2) + 7) & ~7;
   const int c_begin = ((warp - 4) >> 2) * cols_per;
   const int c_end = min(c_begin + cols_per, cols_used);
-  const float* stg = reinterpret_cast<const float*>(cx.smem_gen);
+  const float* stg = reinterpret_cast<const float*>(cx.smem_gen);   // the idle stage ring stages the reduce-scatter slices
   const size_t part_floats = (size_t)p.n_pad * 128;        // one partial: [col][lane]
   const int sb = p.span_begin[span], se = p.span_begin[span + 1];
   float4* const sc4 = cx.sc0();
@@ -273,36 +309,21 @@ __device__ __forceinline__ void epilogue(const GemmParams& p, const Ctx& cx, int
     const uint32_t t0 = cx.tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * p.acc_stride);
 
     if (a == b || (b == a + 1 && span == a)) {
-      const bool add = a != b;
-      if (add) {
-        // last segment of this span: every MMA that reads this CTA's ring is complete, the ring stages the partner's partial
-        if (et == 0) {
-          wait_flag(p, flag_of(b, 0), epoch);
-          asm volatile("fence.proxy.async.global;" ::: "memory");
-          mbar_expect_tx(cx.red_bar(), (uint32_t)cols_used * 512u);
-          bulk_g2s(cx.smem_base, part_of(b, 0), (uint32_t)cols_used * 512u, cx.red_bar(), policy_evict_first());
-        }
-        wait_bar(p, cx.red_bar(), red_round & 1u);
-        ++red_round;
+      // the whole tile is ours, or we own a tile whose tail the next span has (usually long ago) dumped
+      const float* part = nullptr;
+      if (a != b) {
+        wait_flag(p, flag_of(b, 0), epoch);                // every thread: one ld.acquire when the partner is done (the usual case)
+        part = part_of(b, 0);
         if (et == 0) trace(p, span, 8);
       }
+      int c = c_begin;
+      if (part == nullptr) {
 #pragma unroll 1
-      for (int c = c_begin; c < c_end; c += 8) {
-        float v[8];
-        load_acc<MODE>(t0, c, v);
-        if (add) {
-#pragma unroll
-          for (int i = 0; i < 8; ++i) v[i] += stg[part_index<MODE>(i, q, lane, c)];
-        }
-        if (MODE == 0) {
-          glu_chunk<DYN>(p, sc4, cur.tile, 64 * rank + 16 * q, c, Mb, m_base, reinterpret_cast<const float(&)[4]>(v[0]),
-                         reinterpret_cast<const float(&)[4]>(v[4]));
-        } else {
-#pragma unroll
-          for (int i = 0; i < 8; ++i)
-            if (c + i < Mb) store_y(p, cur.tile * 256 + 128 * rank + 32 * q + lane, m_base + c + i, v[i] * sc1[c + i]);
-        }
+        for (; c + 32 <= c_end; c += 32) tile_block<MODE, DYN, 4>(p, sc4, sc1, t0, part, cur.tile, rank, q, lane, c, Mb, m_base);
       }
+#pragma unroll 1
+      for (; c + 16 <= c_end; c += 16) tile_block<MODE, DYN, 2>(p, sc4, sc1, t0, part, cur.tile, rank, q, lane, c, Mb, m_base);
+      if (c < c_end) tile_block<MODE, DYN, 1>(p, sc4, sc1, t0, part, cur.tile, rank, q, lane, c, Mb, m_base);
     } else {
       // split tile, not (solely) ours to finish: dump the raw fp32 partial [col][lane] and publish it
       const int which = (sb >= cur.first) ? 0 : 1;
@@ -430,6 +451,7 @@ spense_gemm_wide_kernel(const __grid_constant__ GemmParams p, const __grid_const
     for (int s = 0; s < cx.S; ++s) { mbar_init(cx.full_bar(s), 1); mbar_init(cx.empty_bar(s), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(cx.accf_bar(b), 1); mbar_init(cx.acce_bar(b), 2 * kEpiWarps); }
     mbar_init(cx.red_bar(), 1);
+    *cx.epi_done_ptr() = 0;
     fence_barrier_init();
   }
   if (warp == 2) tmem_alloc_pair(cx.tmem_slot(), kTmemCols);
@@ -445,12 +467,13 @@ spense_gemm_wide_kernel(const __grid_constant__ GemmParams p, const __grid_const
   }
 
   if (warp == 0) {
-    if (lane == 0) {
-      producer<MODE>(p, &tmap_b, &tmap_ws, &tmap_wd, cx, span);
-      trace(p, span, 2);
-    }
+    producer_weights<MODE>(p, &tmap_ws, &tmap_wd, cx, span);
+    trace(p, span, 2);
+    if (lane == 0) prefetch_next(p, cx, span);
+  } else if (warp == 3) {
+    producer_tokens<MODE>(p, &tmap_b, cx, span);
   } else if (warp == 1) {
-    if (lane == 0 && cx.rank == 0) mma_issuer<MODE>(p, cx, span);
+    if (cx.rank == 0) mma_issuer<MODE>(p, cx, span);
   } else if (warp >= 4) {
     const int et = threadIdx.x - 128;
     pdl_wait();
@@ -467,6 +490,7 @@ spense_gemm_wide_kernel(const __grid_constant__ GemmParams p, const __grid_const
       const int Mb = min(p.n_pad, p.M - cx.blk * p.n_pad);
       if (et < p.n_pad) p.amax_part[(size_t)(cx.slot0 + 2 * span) * p.n_pad + et] = et < Mb ? cx.sc0()[et].z : 0.0f;
     }
+    if (et == 0) *cx.epi_done_ptr() = 1;
     if (p.trace && et == 0 && bp == 0 && cx.rank == 0) p.trace[(size_t)span * 16 + 10] = globaltimer();
   }
 

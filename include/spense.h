@@ -97,6 +97,10 @@ int spense_device_status(int clear);
  * indices to the back, keeping ascending original order inside both regions.  h_perm[new] = old. */
 int spense_perm_from_dense_idx(int32_t I, const int32_t* h_dense_idx, int32_t n_dense, int32_t* h_perm);
 
+/* Host helper: the SpenseGPT choice of dense indices (Eq. 5, reading Q1): the LAST n_dense of the
+ * I intermediate indices, ascending.  (SpenseGPT+'s choice is spense_select_dense.)                          */
+int spense_dense_idx_last(int32_t I, int32_t n_dense, int32_t* h_dense_idx);
+
 /* Bytes of the packed blob and of the pack workspace for a shape. */
 int spense_pack_sizes(const spense_shape_t* shape, size_t* blob_bytes, size_t* workspace_bytes);
 
@@ -200,6 +204,17 @@ int spense_select_workspace_size(const spense_shape_t* shape, size_t* bytes);
 int spense_select_dense(const spense_shape_t* shape, const float* d_wgate, const float* d_wup, const float* d_wdown,
                         const float* d_hdiag_x, const float* d_hdiag_h, float eps, float* d_score,
                         int32_t* d_dense_idx, int32_t* d_perm, void* d_ws, size_t ws_bytes, spense_stream_t stream);
+
+/* spense_prune_2to4_magnitude -- pruning front-end, first slice: magnitude 2:4 pruning of the
+ * SPARSE region in PERMUTED intermediate order ("permute ... then apply [the pruner] while protecting the selected dense
+ * indices"; Eq. 1): of every 4 consecutive weights along K the 2 of largest |w| are kept
+ * (ties to the lower index), the others become +0.  K is H for rows [0, I_s) of P^T W_gate / P^T W_up and the permuted
+ * intermediate dimension for columns [0, I_s) of W_down P (reading Q9b).  Magnitude stands in for SparseGPT's OBS mask
+ * and weight update (Eqs. 2-3), which need calibration activations.
+ * In place on DEVICE fp32 matrices in ORIGINAL index order: d_wgate, d_wup [I, H], d_wdown [H, I]; d_perm [I] new -> old
+ * or NULL (identity).  Integer / comparison work only: bit-exact against the oracle.  No synchronisation.        */
+int spense_prune_2to4_magnitude(const spense_shape_t* shape, float* d_wgate, float* d_wup, float* d_wdown,
+                                const int32_t* d_perm, spense_stream_t stream);
 
 /* spense_quantize_e4m3 -- helper (reading Q5): scale = amax / 448 (1 if amax == 0), per tensor or
  * per row; out = E4M3_rne_sat(in / scale) with an IEEE fp32 division.  d_scales: 1 or rows floats.

@@ -147,6 +147,42 @@ def spensegpt_dense_idx(I: int, I_d: int) -> np.ndarray:
     return np.arange(I - I_d, I, dtype=np.int64)
 
 
+def prune_2to4_group(vals):
+    """Magnitude 2:4 mask of ONE group of 4 weights (the test generator's rule; stands in for the
+    mask SparseGPT would choose): keep the 2 of largest |w|, ties to the lower index.  Plain Python."""
+    order = sorted(range(4), key=lambda i: (-abs(float(vals[i])), i))
+    keep = sorted(order[:2])
+    return [i in keep for i in range(4)]
+
+
+def prune_2to4_magnitude(wgate, wup, wdown, perm, I_dense: int):
+    """NEXT-4 front-end, first slice: magnitude 2:4 pruning of the SPARSE region in PERMUTED intermediate order
+    ("permute ... then apply [the pruner] while protecting the selected dense indices", PAPER.md:202; Eq. 1
+    PAPER.md:67-72: groups of 4 along K): rows [0, I_s) of P^T W_gate / P^T W_up along H, columns [0, I_s) of W_down P
+    along the permuted intermediate dimension (reading Q9b).  Pruned entries become +0.  Returns new arrays in the
+    ORIGINAL index order (the layout spense_pack takes)."""
+    wgate, wup, wdown = (np.array(a, copy=True) for a in (wgate, wup, wdown))
+    I, H = wgate.shape
+    perm = np.arange(I) if perm is None else np.asarray(perm, dtype=np.int64)
+    I_s = I - I_dense
+
+    def mask_lastdim(a):                                   # a [..., 4 g + i]: keep mask by the scalar rule, vectorised
+        g = np.abs(a.reshape(-1, 4)).astype(np.float64)
+        idx = np.arange(4)
+        # rank of element i = number of elements that beat it (larger |w|, or equal |w| and lower index)
+        beats = (g[:, None, :] > g[:, :, None]) | ((g[:, None, :] == g[:, :, None]) & (idx[None, None, :] < idx[None, :, None]))
+        return (beats.sum(axis=2) < 2).reshape(a.shape)
+
+    for w in (wgate, wup):
+        rows = perm[:I_s]
+        blk = w[rows]
+        w[rows] = np.where(mask_lastdim(blk), blk, 0)
+    cols = perm[:I_s]
+    blk = wdown[:, cols]
+    wdown[:, cols] = np.where(mask_lastdim(blk), blk, 0)
+    return wgate, wup, wdown
+
+
 def check_perm(perm: np.ndarray, I: int):
     perm = np.asarray(perm)
     if perm.shape != (I,) or perm.min(initial=0) < 0 or perm.max(initial=0) >= I \

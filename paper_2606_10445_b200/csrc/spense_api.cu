@@ -484,6 +484,12 @@ int spense_perm_from_dense_idx(int32_t I, const int32_t* h_dense_idx, int32_t n_
   return SPENSE_OK;
 }
 
+int spense_dense_idx_last(int32_t I, int32_t n_dense, int32_t* h_dense_idx) {
+  if (I < 0 || n_dense < 0 || n_dense > I || (n_dense && !h_dense_idx)) return SPENSE_ERR_ARG;
+  for (int i = 0; i < n_dense; ++i) h_dense_idx[i] = I - n_dense + i;
+  return SPENSE_OK;
+}
+
 int spense_pack_sizes(const spense_shape_t* shape, size_t* blob_bytes, size_t* workspace_bytes) {
   int st = check_shape(shape);
   if (st) return st;
@@ -648,6 +654,17 @@ int spense_select_dense(const spense_shape_t* shape, const float* d_wgate, const
   if (st) return st;
   return launch_select(shape, d_wgate, d_wup, d_wdown, d_hdiag_x, d_hdiag_h, eps, d_score, d_dense_idx, d_perm, d_ws,
                        reinterpret_cast<cudaStream_t>(stream));
+}
+
+int spense_prune_2to4_magnitude(const spense_shape_t* shape, float* d_wgate, float* d_wup, float* d_wdown, const int32_t* d_perm,
+                                spense_stream_t stream) {
+  int st = check_shape(shape);
+  if (st) return st;
+  if (!d_wgate || !d_wup || !d_wdown) return SPENSE_ERR_ARG;
+  if (!aligned(d_wgate, 16) || !aligned(d_wup, 16) || !aligned(d_wdown, 16) || (d_perm && !aligned(d_perm, 4))) return SPENSE_ERR_ALIGN;
+  st = check_device(nullptr, nullptr);
+  if (st) return st;
+  return launch_prune(shape, d_wgate, d_wup, d_wdown, d_perm, reinterpret_cast<cudaStream_t>(stream));
 }
 
 int spense_quantize_e4m3(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out, float* d_scales,

@@ -4,6 +4,7 @@
 //   D = the I_dense indices of largest s (ties to the lower index), ascending; perm = stable partition         (Eq. 12, Q9)
 // All three passes are HBM-bound reads of the fp32 weights (3 * I * H * 4 bytes, once).  Every reduction runs in
 // a fixed order, so the scores and the selection are bitwise reproducible.
+// Also the first slice of the pruning front-end (NEXT-4): magnitude 2:4 pruning of the sparse region in permuted order.
 #include "spense_internal.cuh"
 
 namespace spense {
@@ -146,7 +147,65 @@ __global__ void __launch_bounds__(1024) partition_kernel(const float* __restrict
   }
 }
 
+// ---------------------------------------------------------------- magnitude 2:4 pruning (first slice)
+// keep mask of one group of 4: the 2 entries of largest |w|, ties to the lower index
+__device__ __forceinline__ int keep_mask_2of4(float a0, float a1, float a2, float a3) {
+  const float m[4] = {fabsf(a0), fabsf(a1), fabsf(a2), fabsf(a3)};
+  int mask = 0;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    int beats = 0;
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      if (j != i) beats += (m[j] > m[i] || (m[j] == m[i] && j < i)) ? 1 : 0;
+    if (beats < 2) mask |= 1 << i;
+  }
+  return mask;
+}
+
+// rows [0, I_s) of P^T W (gate or up), groups of 4 along H: one thread per group, in place
+__global__ void __launch_bounds__(256) prune_rows_kernel(float* __restrict__ w, const int32_t* __restrict__ perm, int H, int I_s) {
+  const int groups = H >> 2;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (long long)I_s * groups) return;
+  const int r = (int)(i / groups), g = (int)(i - (long long)r * groups);
+  float4* ptr = reinterpret_cast<float4*>(w + (size_t)(perm ? perm[r] : r) * H) + g;
+  float4 v = *ptr;
+  const int k = keep_mask_2of4(v.x, v.y, v.z, v.w);
+  if (!(k & 1)) v.x = 0.0f;
+  if (!(k & 2)) v.y = 0.0f;
+  if (!(k & 4)) v.z = 0.0f;
+  if (!(k & 8)) v.w = 0.0f;
+  *ptr = v;
+}
+
+// columns [0, I_s) of W_down P, groups of 4 along the PERMUTED intermediate dimension: one thread per (row, group)
+__global__ void __launch_bounds__(256) prune_cols_kernel(float* __restrict__ w, const int32_t* __restrict__ perm, int I, int I_s, int H) {
+  const int groups = I_s >> 2;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (long long)H * groups) return;
+  const int n = (int)(i / groups), g = (int)(i - (long long)n * groups);
+  float* row = w + (size_t)n * I;
+  int c[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) c[k] = perm ? perm[4 * g + k] : 4 * g + k;
+  const int keep = keep_mask_2of4(row[c[0]], row[c[1]], row[c[2]], row[c[3]]);
+#pragma unroll
+  for (int k = 0; k < 4; ++k)
+    if (!(keep & (1 << k))) row[c[k]] = 0.0f;
+}
+
 }  // namespace
+
+int launch_prune(const spense_shape_t* shape, float* d_wgate, float* d_wup, float* d_wdown, const int32_t* d_perm, cudaStream_t stream) {
+  const int H = shape->H, I = shape->I, I_s = shape->I - shape->I_dense;
+  if (I_s == 0) return SPENSE_OK;
+  const long long n_rows = (long long)I_s * (H >> 2), n_cols = (long long)H * (I_s >> 2);
+  prune_rows_kernel<<<(unsigned)((n_rows + 255) / 256), 256, 0, stream>>>(d_wgate, d_perm, H, I_s);
+  prune_rows_kernel<<<(unsigned)((n_rows + 255) / 256), 256, 0, stream>>>(d_wup, d_perm, H, I_s);
+  prune_cols_kernel<<<(unsigned)((n_cols + 255) / 256), 256, 0, stream>>>(d_wdown, d_perm, I, I_s, H);
+  return cudaGetLastError() == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;
+}
 
 int launch_select(const spense_shape_t* shape, const float* d_wgate, const float* d_wup, const float* d_wdown,
                   const float* d_hdiag_x, const float* d_hdiag_h, float eps, float* d_score, int32_t* d_dense_idx,

@@ -24,7 +24,7 @@ STATUS = {0: "SPENSE_OK", -1: "SPENSE_ERR_ARG", -2: "SPENSE_ERR_ALIGN", -3: "SPE
 
 EXPORTS = ["spense_version", "spense_strerror", "spense_device_status", "spense_schedule", "spense_perm_from_dense_idx", "spense_pack_sizes", "spense_pack",
            "spense_workspace_size", "spense_workspace_init", "spense_gate_up", "spense_down", "spense_mlp",
-           "spense_mlp_dyn", "spense_mlp_host", "spense_quantize_e4m3", "spense_select_workspace_size",
+           "spense_mlp_dyn", "spense_mlp_host", "spense_quantize_e4m3", "spense_prune_2to4_magnitude", "spense_dense_idx_last", "spense_select_workspace_size",
            "spense_select_dense"]
 
 
@@ -81,6 +81,8 @@ def lib() -> ctypes.CDLL:
         L.spense_select_workspace_size.argtypes = [POINTER(Shape), POINTER(c_size_t)]
         L.spense_select_dense.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_float, c_void_p,
                                           c_void_p, c_void_p, c_void_p, c_size_t, c_void_p]
+        L.spense_prune_2to4_magnitude.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
+        L.spense_dense_idx_last.argtypes = [c_int32, c_int32, POINTER(c_int32)]
         L.spense_quantize_e4m3.argtypes = [c_void_p, c_int64, c_int64, c_int32, c_void_p, c_void_p, c_void_p,
                                            c_size_t, c_void_p]
         for name in EXPORTS:
@@ -135,6 +137,23 @@ def spense_perm_from_dense_idx(I: int, dense_idx) -> torch.Tensor:
     out = (c_int32 * I)()
     _check(lib().spense_perm_from_dense_idx(I, idx, len(dense_idx), out))
     return torch.tensor(list(out), dtype=torch.int32)
+
+
+def spense_dense_idx_last(I: int, n_dense: int) -> torch.Tensor:
+    out = (c_int32 * max(n_dense, 1))()
+    _check(lib().spense_dense_idx_last(I, n_dense, out))
+    return torch.tensor(list(out[:n_dense]), dtype=torch.int32)
+
+
+def spense_prune_2to4_magnitude(wgate, wup, wdown, perm, I_dense: int):
+    """In place magnitude 2:4 pruning of the sparse region (permuted order) of fp32 CUDA weights in original order."""
+    for t in (wgate, wup, wdown):
+        _dev(t, torch.float32)
+    if perm is not None:
+        _dev(perm, torch.int32)
+    I, H = wgate.shape
+    _check(lib().spense_prune_2to4_magnitude(ctypes.byref(Shape(H, I, I_dense)), _ptr(wgate), _ptr(wup), _ptr(wdown), _ptr(perm), _stream()))
+    return wgate, wup, wdown
 
 
 def spense_pack_sizes(H: int, I: int, I_dense: int):

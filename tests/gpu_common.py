@@ -7,6 +7,14 @@ import spense_inputs as si
 from oracle import spense_oracle as o
 
 
+# Share of Hq bytes that may differ from the ORACLE's Hq: the kernel's fp32 h differs from the oracle's float64 h in the
+# last bits (accumulation order, hardware exp2 / rcp in SiLU), so a value sitting on an E4M3 rounding boundary can land
+# on the neighbouring byte.  Measured on B200 over all 56 cases of the GPU suite (each prints an [hq-mismatch] line):
+# 0 to 9e-6 at full size, worst 2.96e-5 (one byte of a 33 792-byte case); the bound is ~3x the worst, which is also what
+# SURVEY.md 8c-O6 expected ("<~ 1e-4").  The dynamic path (its scale can be one ulp off) measured at most 9.4e-6 and is allowed 4x the bound.
+HQ_MISMATCH_BOUND = 1e-4
+
+
 def cuda(t):
     return t.cuda().contiguous()
 
@@ -50,6 +58,7 @@ def assert_gate_up_parity(r, h_gpu, hq_gpu, s_h, label=""):
     assert np.array_equal(own, hq_gpu), f"{label}: Hq is not the RNE E4M3 cast of the kernel's own h"
     diff = hq_gpu != r["hq"]
     frac = diff.mean()
+    print(f"[hq-mismatch] {label}: {frac:.3e} of {diff.size} bytes")
     if diff.any():
         a, b = o.e4m3_decode(hq_gpu[diff]), o.e4m3_decode(r["hq"][diff])
         # neighbours on the E4M3 grid: |a-b| <= one step of the larger magnitude (2^-3 relative), or both tiny

@@ -9,7 +9,7 @@ import torch
 
 import spense_inputs as si
 from oracle import spense_oracle as o
-from tests.gpu_common import Case, assert_down_parity, cuda
+from tests.gpu_common import HQ_MISMATCH_BOUND, Case, assert_down_parity, cuda
 
 pytestmark = pytest.mark.gpu
 
@@ -53,7 +53,8 @@ def test_mlp_dyn_parity(sp, H, I, p, M):
     if M > 2:
         assert sh_gpu[1] == 1.0 and not hq_gpu[1].any() and not y_gpu[1].any()
     diff = (hq_gpu != ref["hq"]).mean()
-    assert diff < 2e-2, diff                              # a scale one ulp off moves a few rounding boundaries
+    print(f"[hq-mismatch] dynamic requant {H}x{I} p={p} M={M}: {diff:.3e}")
+    assert diff < 4 * HQ_MISMATCH_BOUND, diff             # a scale one ulp off moves a few more rounding boundaries
     # y against the oracle's down fed the GPU's own bytes and scale
     assert_down_parity(y_gpu, hq_gpu, sh_gpu, c.wd, c.L.w_scale[2], "down after dynamic requant")
     # reproducible, and bf16 = RNE of fp32

@@ -74,16 +74,59 @@ def test_select_ties_and_planted_indices(sp):
     assert perm.cpu().tolist()[-128:] == d.cpu().tolist()
 
 
-def test_select_feeds_pack(sp):
-    """selection -> prune the sparse region in permuted order -> quantise -> pack -> the dense block is D."""
+def test_select_prune_quantise_pack_chain(sp):
+    """The offline chain on the GPU, step by step against the oracle's: SpenseGPT+ selection (Eqs. 8-12) -> magnitude 2:4
+    pruning of the sparse region in PERMUTED order -> per-tensor E4M3 quantisation -> spense_pack.  Every
+    step is bit-exact (scores aside, which decide the same index set), the packed layer passes Eq. 1, its dense block holds
+    exactly the selected indices D, and the packed layer computes the oracle's MLP."""
+    I, H, I_d, M = 1024, 256, 256, 8
+    wg, wu, wd, hx, hh = _case(I, H, seed=11)
+    # 1. selection
+    _, d, perm = sp.spense_select_dense(wg.cuda(), wu.cuda(), wd.cuda(), hx.cuda(), hh.cuda(), I_d)
+    d_or = o.spensegpt_plus_dense_idx(wg.numpy(), wu.numpy(), wd.numpy(), hx.numpy(), hh.numpy(), I_d)
+    d_ref = d.cpu().numpy()                                # fp32 scores may swap indices that tie at the threshold: go on with the GPU's set
+    assert len(np.setxor1d(d_ref, d_or)) <= 2
+    perm_ref = o.perm_from_dense_idx(I, d_ref)
+    assert np.array_equal(perm.cpu().numpy(), perm_ref)
+    # 2. prune (in place on device copies)
+    g_d, u_d, d_d = wg.cuda().clone(), wu.cuda().clone(), wd.cuda().clone()
+    sp.spense_prune_2to4_magnitude(g_d, u_d, d_d, perm, I_d)
+    g_ref, u_ref, dn_ref = o.prune_2to4_magnitude(wg.numpy(), wu.numpy(), wd.numpy(), perm_ref, I_d)
+    for got, ref in ((g_d, g_ref), (u_d, u_ref), (d_d, dn_ref)):
+        assert np.array_equal(got.cpu().numpy().view(np.uint32), ref.astype(np.float32).view(np.uint32))
+    # 3. quantise, per tensor
+    q, scales = zip(*[sp.spense_quantize_e4m3(t, sp.SPENSE_PER_TENSOR) for t in (g_d, u_d, d_d)])
+    for (qb, sc), ref in zip(zip(q, scales), (g_ref, u_ref, dn_ref)):
+        rb, rs = o.quantize_per_tensor(ref.astype(np.float32))
+        assert float(sc) == float(rs) and np.array_equal(qb.cpu().numpy(), rb)
+    w_scale = tuple(float(s) for s in scales)
+    # 4. pack: accepts the layer (Eq. 1 holds in permuted order), canonical arrays equal the oracle's
+    pk = sp.spense_pack(q[0], q[1], q[2], w_scale, perm, I_d, want_canon=True)
+    canon = o.pack_canonical(q[0].cpu().numpy(), q[1].cpu().numpy(), q[2].cpu().numpy(), perm_ref, I_d)
+    for k, ref in canon.items():
+        assert np.array_equal(pk.canon[k].cpu().numpy(), ref), k
+    assert np.array_equal(pk.canon["perm"].cpu().numpy()[I - I_d:], d_ref)      # the dense block is D, ascending (Q8, Q9)
+    assert np.array_equal(pk.canon["gate_dn"].cpu().numpy(), q[0].cpu().numpy()[d_ref])
+    # 5. and the packed layer runs: y against the oracle's down fed the GPU's Hq
     import spense_inputs as si
-    L = si.make_layer(256, 1024, 0.25, seed=0, prune=False)       # unpruned fp8 bytes; use them as fp32 weights here
-    dec = lambda b: torch.from_numpy(o.e4m3_decode(b.numpy()).astype(np.float32))
-    wg, wu, wd = dec(L.wgate), dec(L.wup), dec(L.wdown)
-    hx, hh = torch.rand(256) + 0.5, torch.rand(1024) + 0.5
-    _, d, perm = sp.spense_select_dense(wg.cuda(), wu.cuda(), wd.cuda(), hx.cuda(), hh.cuda(), 256)
-    ref_perm = sp.spense_perm_from_dense_idx(1024, d.cpu().tolist())
-    assert torch.equal(perm.cpu(), ref_perm)
+    x, s_x = si.make_activations(M, H, seed=3)
+    ug, uu, ud = o.unpack_canonical(canon)
+    r1 = o.gate_up(x.numpy(), s_x.numpy(), ug, uu, w_scale[0], w_scale[1], 1.0)
+    s_h = o.requant_scale_from_h(r1["h"])
+    ws = sp.spense_workspace(pk, M)
+    hq = torch.empty(M, I, dtype=torch.uint8, device="cuda")
+    y = sp.spense_mlp(pk, x.cuda(), s_x.cuda(), torch.from_numpy(s_h).cuda(), ws, hq_scratch=hq)
+    torch.cuda.synchronize()
+    ref = o.down(hq.cpu().numpy(), s_h, ud, w_scale[2])
+    assert (np.abs(y.cpu().numpy() - ref["y"]) <= o.tol_gemm(ref["absY"])).all()
+
+
+def test_dense_idx_last_is_eq5(sp):
+    """SpenseGPT's choice (Eq. 5, reading Q1): the last n indices; feeds the same permutation helper."""
+    d = sp.spense_dense_idx_last(1024, 256)
+    assert np.array_equal(d.numpy(), o.spensegpt_dense_idx(1024, 256))
+    assert np.array_equal(sp.spense_perm_from_dense_idx(1024, d.tolist()).numpy(), np.arange(1024))   # already at the back
+    assert sp.spense_dense_idx_last(128, 0).numel() == 0
 
 
 def test_select_argument_errors(sp):

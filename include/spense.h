@@ -190,6 +190,17 @@ int spense_mlp_host(const spense_shape_t* shape, const void* d_blob, const uint8
                     uint8_t* d_x, float* d_scales, uint8_t* d_hq_scratch, void* d_y, void* d_ws,
                     size_t ws_bytes, const void* d_next_blob, spense_stream_t stream);
 
+/* spense_mlp_stack_host -- the same HOST activations through n_layers packed layers of one shape, one after the other
+ * on the stream (every layer reads x, the last one's y is returned): ONE host-to-device copy of the inputs, n_layers x
+ * spense_mlp (each naming the next blob as L2 prefetch hint), ONE device-to-host copy of y, ONE synchronise.  This is
+ * the unit bench.py times end to end (a decode step of several layers whose inputs arrive from the host); a real model
+ * chains its layers on the device with spense_mlp.  d_blobs: HOST array of n_layers DEVICE blob pointers.  Staging
+ * buffers and the other arguments as in spense_mlp_host.                                                      */
+int spense_mlp_stack_host(const spense_shape_t* shape, const void* const* d_blobs, int32_t n_layers, const uint8_t* h_x,
+                          const float* h_sx, int32_t M, const float* h_sh, int32_t sh_stride, void* h_y, int32_t y_dtype,
+                          uint8_t* d_x, float* d_scales, uint8_t* d_hq_scratch, void* d_y, void* d_ws, size_t ws_bytes,
+                          spense_stream_t stream);
+
 /* spense_select_dense -- SpenseGPT+ dense-index selection (Eqs. 8-12):
  *   s^gate_i = 1/H sum_j |Wg[i,j]| sqrt(Hx[j]),  s^up likewise,  s^down_i = sqrt(Hh[i]) / H sum_n |Wd[n,i]|   (Eq. 9)
  *   s_i = sum over the three projections of s^mlp_i / (mean(s^mlp) + eps)                            (Eqs. 10, 11)

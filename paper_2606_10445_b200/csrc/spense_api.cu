@@ -94,12 +94,13 @@ int ring_of(bool wide, int n_pad, int* slot_bytes) {
 
 // how many of `nb` blocks one launch takes: the largest split within 5 % of the best occupancy over all rounds
 // (every round is a launch with its own start-up and fix-up tail, so fewer rounds win a near tie)
-int par_of(int nb, int units) {
+int par_of(int nb, int units, int cap) {
   auto eff = [&](int c) {
     const int rounds = (nb + c - 1) / c, k = units / c;
     return (double)nb / (rounds * c) * ((double)(c * k) / units);
   };
-  const int cmax = nb < 37 ? (nb < units ? nb : units) : (37 < units ? 37 : units);
+  int cmax = nb < units ? nb : units;
+  if (cmax > cap) cmax = cap;
   double best = 0;
   for (int c = 1; c <= cmax; ++c) best = eff(c) > best ? eff(c) : best;
   int pick = 1;
@@ -108,7 +109,12 @@ int par_of(int nb, int units) {
   return pick;
 }
 
-Plan plan_of(int M, int sms) {
+// act_row_bytes: bytes of one token row of the activation operand (H for gate_up, I for down).  The token tiles of the
+// blocks of one launch are re-read from L2 once per weight tile, so a launch takes only as many blocks as keep that
+// working set (blocks x n_pad x act_row_bytes) well inside the 126 MB L2: measured at M = 8192, 18 blocks of Hq (110 MB)
+// side by side made down HBM-bound on activation re-reads (1020 us against 4 x 167 us at M = 2048).
+constexpr size_t kActWorkingSetBytes = 64u << 20;
+Plan plan_of(int M, int sms, int act_row_bytes) {
   Plan pl = {};
   if (M <= kDecodeMaxTokens) {
     pl.wide = false;
@@ -119,7 +125,9 @@ Plan plan_of(int M, int sms) {
     pl.nb = (M + kWideMaxTokens - 1) / kWideMaxTokens;
     pl.n_pad = ((M + pl.nb - 1) / pl.nb + 15) / 16 * 16;
     const int pairs = sms / 2;
-    pl.par = par_of(pl.nb, pairs);
+    size_t cap = kActWorkingSetBytes / ((size_t)pl.n_pad * act_row_bytes);
+    cap = cap < 1 ? 1 : (cap > 12 ? 12 : cap);
+    pl.par = par_of(pl.nb, pairs, (int)cap);
     pl.spans = pairs / pl.par;
   }
   pl.ring = ring_of(pl.wide, pl.n_pad, &pl.slot_bytes);
@@ -306,7 +314,7 @@ int gate_up_impl(const Launch& L, const spense_shape_t* shape, const void* d_blo
                  const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32, void* d_ws, bool pdl, bool down_follows,
                  cudaStream_t stream, bool dynamic = false, float* d_sh_out = nullptr) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const Plan pl = plan_of(M, L.sms);
+  const Plan pl = plan_of(M, L.sms, g.H);
   const Schedule& sc = get_schedule(0, g, pl);
   const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + g.gate_up_off;
   CUtensorMap tm, tws, twd;
@@ -334,7 +342,7 @@ int gate_up_impl(const Launch& L, const spense_shape_t* shape, const void* d_blo
     p.amax_part = dynamic ? reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes) : nullptr;
     p.ld_out = g.I; p.out_rows = g.I;
     if (down_follows && blk0 + pl.par >= pl.nb)                // the same layer's down projection streams next
-      fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + g.down_off, get_schedule(1, g, pl));
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + g.down_off, get_schedule(1, g, plan_of(M, L.sms, g.I)));
     if (!pl.wide) {
       st = launch_gemm(p, tm, pdl, L.dev, L.sms, stream);
     } else {
@@ -358,7 +366,7 @@ int down_impl(const Launch& L, const spense_shape_t* shape, const void* d_blob, 
               int32_t sh_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, bool pdl, const void* d_next_blob,
               cudaStream_t stream) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const Plan pl = plan_of(M, L.sms);
+  const Plan pl = plan_of(M, L.sms, g.I);
   const Schedule& sc = get_schedule(1, g, pl);
   const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + g.down_off;
   CUtensorMap tm, tws, twd;
@@ -384,7 +392,7 @@ int down_impl(const Launch& L, const spense_shape_t* shape, const void* d_blob, 
     p.y_dtype = y_dtype;
     p.ld_out = g.H; p.out_rows = g.H;
     if (d_next_blob && blk0 + pl.par >= pl.nb)                 // the next layer's gate/up weights stream next
-      fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + g.gate_up_off, get_schedule(0, g, pl));
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + g.gate_up_off, get_schedule(0, g, plan_of(M, L.sms, g.H)));
     if (!pl.wide) {
       st = launch_gemm(p, tm, pdl, L.dev, L.sms, stream);
     } else {
@@ -456,7 +464,7 @@ int spense_schedule(const spense_shape_t* shape, int32_t M, int32_t mode, int32_
   if (st) return st;
   if (M < 1 || M > kMaxTokens || (mode != 0 && mode != 1) || sms < 2 || sms > kMaxSpans || !out_span_begin) return SPENSE_ERR_ARG;
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const Plan pl = plan_of(M, sms);
+  const Plan pl = plan_of(M, sms, mode == 0 ? g.H : g.I);
   const Schedule& sc = get_schedule(mode, g, pl);
   for (int i = 0; i <= sc.n_spans; ++i) out_span_begin[i] = sc.span_begin[i];
   if (out_info) {
@@ -622,6 +630,30 @@ int spense_mlp_host(const spense_shape_t* shape, const void* d_blob, const uint8
   st = spense_mlp(shape, d_blob, d_x, d_scales, M, d_scales + M, sh_stride, d_hq_scratch, nullptr, d_y, y_dtype, d_ws,
                   ws_bytes, d_next_blob, stream);
   if (st) return st;
+  const size_t esz = y_dtype == SPENSE_F32 ? 4 : 2;
+  if (cudaMemcpyAsync(h_y, d_y, (size_t)M * shape->H * esz, cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPENSE_ERR_CUDA;
+  if (cudaStreamSynchronize(s) != cudaSuccess) return SPENSE_ERR_CUDA;
+  return pending_device_error();
+}
+
+int spense_mlp_stack_host(const spense_shape_t* shape, const void* const* d_blobs, int32_t n_layers, const uint8_t* h_x,
+                          const float* h_sx, int32_t M, const float* h_sh, int32_t sh_stride, void* h_y, int32_t y_dtype, uint8_t* d_x,
+                          float* d_scales, uint8_t* d_hq_scratch, void* d_y, void* d_ws, size_t ws_bytes, spense_stream_t stream) {
+  int st = check_shape(shape);
+  if (st) return st;
+  if (!d_blobs || n_layers < 1 || !h_x || !h_sx || !h_sh || !h_y || !d_x || !d_scales || M < 1 || M > kMaxTokens ||
+      (sh_stride != 0 && sh_stride != 1) || (y_dtype != SPENSE_F32 && y_dtype != SPENSE_BF16))
+    return SPENSE_ERR_ARG;
+  cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
+  const size_t n_sh = sh_stride ? (size_t)M : 1;
+  if (cudaMemcpyAsync(d_x, h_x, (size_t)M * shape->H, cudaMemcpyHostToDevice, s) != cudaSuccess) return SPENSE_ERR_CUDA;
+  if (cudaMemcpyAsync(d_scales, h_sx, (size_t)M * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) return SPENSE_ERR_CUDA;
+  if (cudaMemcpyAsync(d_scales + M, h_sh, n_sh * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) return SPENSE_ERR_CUDA;
+  for (int i = 0; i < n_layers; ++i) {
+    st = spense_mlp(shape, d_blobs[i], d_x, d_scales, M, d_scales + M, sh_stride, d_hq_scratch, nullptr, d_y, y_dtype, d_ws, ws_bytes,
+                    d_blobs[(i + 1) % n_layers], stream);
+    if (st) return st;
+  }
   const size_t esz = y_dtype == SPENSE_F32 ? 4 : 2;
   if (cudaMemcpyAsync(h_y, d_y, (size_t)M * shape->H * esz, cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPENSE_ERR_CUDA;
   if (cudaStreamSynchronize(s) != cudaSuccess) return SPENSE_ERR_CUDA;

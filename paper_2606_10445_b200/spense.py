@@ -24,7 +24,7 @@ STATUS = {0: "SPENSE_OK", -1: "SPENSE_ERR_ARG", -2: "SPENSE_ERR_ALIGN", -3: "SPE
 
 EXPORTS = ["spense_version", "spense_strerror", "spense_device_status", "spense_schedule", "spense_perm_from_dense_idx", "spense_pack_sizes", "spense_pack",
            "spense_workspace_size", "spense_workspace_init", "spense_gate_up", "spense_down", "spense_mlp",
-           "spense_mlp_dyn", "spense_mlp_host", "spense_quantize_e4m3", "spense_prune_2to4_magnitude", "spense_dense_idx_last", "spense_select_workspace_size",
+           "spense_mlp_dyn", "spense_mlp_host", "spense_mlp_stack_host", "spense_quantize_e4m3", "spense_prune_2to4_magnitude", "spense_dense_idx_last", "spense_select_workspace_size",
            "spense_select_dense"]
 
 
@@ -78,6 +78,9 @@ def lib() -> ctypes.CDLL:
         L.spense_mlp_host.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_int32, c_void_p, c_int32,
                                       c_void_p, c_int32, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_size_t,
                                       c_void_p, c_void_p]
+        L.spense_mlp_stack_host.argtypes = [POINTER(Shape), POINTER(c_void_p), c_int32, c_void_p, c_void_p, c_int32, c_void_p,
+                                            c_int32, c_void_p, c_int32, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p,
+                                            c_size_t, c_void_p]
         L.spense_select_workspace_size.argtypes = [POINTER(Shape), POINTER(c_size_t)]
         L.spense_select_dense.argtypes = [POINTER(Shape), c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_float, c_void_p,
                                           c_void_p, c_void_p, c_void_p, c_size_t, c_void_p]
@@ -283,6 +286,19 @@ def spense_mlp_host(layer: PackedLayer, h_x, h_sx, h_sh, h_y, staging, ws, next_
                                  stride, _ptr(h_y), SPENSE_F32 if h_y.dtype == torch.float32 else SPENSE_BF16,
                                  _ptr(staging["d_x"]), _ptr(staging["d_scales"]), _ptr(staging["d_hq"]),
                                  _ptr(staging["d_y"]), _ptr(ws), ws.numel(), _next(next_layer), _stream()))
+    return h_y
+
+
+def spense_mlp_stack_host(layers, h_x, h_sx, h_sh, h_y, staging, ws):
+    """HOST (pinned) x, s_x, s_h through every PackedLayer of `layers` (same shape) -> HOST y of the last one: one H2D
+    copy, len(layers) x spense_mlp, one D2H copy, one synchronise."""
+    M = h_x.shape[0]
+    stride = 0 if h_sh.numel() == 1 else 1
+    blobs = (c_void_p * len(layers))(*[l.blob.data_ptr() for l in layers])
+    _check(lib().spense_mlp_stack_host(ctypes.byref(layers[0].shape), blobs, len(layers), _ptr(h_x), _ptr(h_sx), M, _ptr(h_sh),
+                                       stride, _ptr(h_y), SPENSE_F32 if h_y.dtype == torch.float32 else SPENSE_BF16,
+                                       _ptr(staging["d_x"]), _ptr(staging["d_scales"]), _ptr(staging["d_hq"]),
+                                       _ptr(staging["d_y"]), _ptr(ws), ws.numel(), _stream()))
     return h_y
 
 

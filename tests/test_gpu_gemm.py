@@ -231,3 +231,6 @@ def test_mlp_host_buffers_equal_device_call(sp):
                        d_hq=torch.empty(M, I, dtype=torch.uint8, device="cuda"), d_y=torch.empty(M, H, dtype=dtype, device="cuda"))
         sp.spense_mlp_host(pk, hx, hsx, hsh, hy, staging, ws)
         assert torch.equal(hy, y_dev.cpu())
+        hy.zero_()
+        sp.spense_mlp_stack_host([pk, pk, pk], hx, hsx, hsh, hy, staging, ws)     # every layer reads x: the last y is the same
+        assert torch.equal(hy, y_dev.cpu())

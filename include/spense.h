@@ -233,6 +233,62 @@ int spense_prune_2to4_magnitude(const spense_shape_t* shape, float* d_wgate, flo
 int spense_quantize_e4m3(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out,
                          float* d_scales, void* d_ws, size_t ws_bytes, spense_stream_t stream);
 
+/* ---- Stand-alone Spense linears: the format is defined per weight matrix -- "Spense splits the
+ * weight matrix into two parts: the semi-structured sparse part and the dense part" (Sec. 3.2) -- and comes
+ * in two orientations: OUTPUT-split (the rows of W in R^{N x K} are split: "the input is multiplied
+ * separately by the semi-structured sparse and dense weights, and the outputs are concatenated") and INPUT-split (the
+ * reduction dimension is split: "a sparse matrix multiplication is performed first ... followed by a dense matrix
+ * multiplication that accumulates into the same output").  No GLU, no re-quantisation: y = (x W^T) * s_x[m] * s_w.
+ *   N, K multiples of 128.  n_dense = dense rows (out-split) or dense columns (in-split), a multiple of 128; for the
+ *   out-split the sparse row count N - n_dense must be a multiple of 256 (sparse and dense rows never share a 256-row
+ *   MMA tile).  In PERMUTED order the sparse region comes first, the dense region last.             */
+enum { SPENSE_SPLIT_OUT = 0, SPENSE_SPLIT_IN = 1 };
+typedef struct {
+  int32_t N;       /* output features (rows of W)                                      */
+  int32_t K;       /* input features  (columns of W, the reduction dimension)          */
+  int32_t n_dense; /* dense rows (SPENSE_SPLIT_OUT) / dense columns (SPENSE_SPLIT_IN)  */
+  int32_t split;   /* SPENSE_SPLIT_OUT | SPENSE_SPLIT_IN                               */
+} spense_linear_shape_t;
+
+/* Canonical result of spense_pack_linear (DEVICE, caller-owned, members nullable); encoding as in spense_canon_t.
+ *   out-split: perm [N]; sp_val [N_s, K/2]; sp_meta [N_s, K/8]; dn [n_dense, K]       (N_s = N - n_dense)
+ *   in-split : perm [K]; sp_val [N, K_s/2]; sp_meta [N, K_s/8]; dn [N, n_dense]       (K_s = K - n_dense)            */
+typedef struct {
+  int32_t* perm;
+  uint8_t* sp_val;
+  uint8_t* sp_meta;
+  uint8_t* dn;
+} spense_linear_canon_t;
+
+/* Bytes of the packed blob and of the pack workspace of one linear. */
+int spense_linear_pack_sizes(const spense_linear_shape_t* shape, size_t* blob_bytes, size_t* workspace_bytes);
+
+/* spense_pack_linear -- spense_pack for ONE matrix: P1 permute (rows of W for the out-split, columns for the in-split;
+ * d_perm new -> old over N resp. K, or NULL), P2 validate Eq. 1 on the sparse region -- 2:4 along K, for the
+ * in-split along the PERMUTED K -- and compress it, P3 re-tile into the stage images the GEMM streams.
+ *   d_w [N, K] E4M3 bytes in ORIGINAL order; w_scale: the per-tensor fp32 scale, stored in the blob header.
+ *   h_err_where[4] as in spense_pack with matrix = 0.  Synchronises the stream once.  Other arguments as in spense_pack. */
+int spense_pack_linear(const spense_linear_shape_t* shape, const uint8_t* d_w, float w_scale, const int32_t* d_perm,
+                       void* d_blob, size_t blob_bytes, const spense_linear_canon_t* canon, void* d_ws, size_t ws_bytes,
+                       int64_t* h_err_where, spense_stream_t stream);
+
+/* Workspace of the linear GEMM calls at up to M tokens: same rules as spense_workspace_size / spense_workspace_init. */
+int spense_linear_workspace_size(const spense_linear_shape_t* shape, int32_t M, size_t* bytes);
+
+/* spense_linear_out_split -- y[m, n] = (sum_k x[m, k] W'[n, k]) * s_x[m * sx_stride] * s_w with W' = the row-permuted
+ * weight: 256-row tiles below N_s run on 2:4 sparse MMAs, the others on dense MMAs (output-split).
+ * y is in PERMUTED row order: y[:, new] belongs to original output feature perm[new].
+ * spense_linear_in_split -- the same sum with the K loop running the sparse range [0, K_s) on sparse MMAs and continuing
+ * with the dense range into the same accumulator (input-split); x is in PERMUTED column order.
+ *   d_x [M, K] E4M3; d_sx fp32, sx_stride 0 = one scalar, 1 = per token; d_y [M, N] fp32 or bf16.  The blob must come from
+ *   spense_pack_linear with the same shape (checked on the device: SPENSE_ERR_BAD_BLOB).  No synchronisation.          */
+int spense_linear_out_split(const spense_linear_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx,
+                            int32_t sx_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, size_t ws_bytes,
+                            spense_stream_t stream);
+int spense_linear_in_split(const spense_linear_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx,
+                           int32_t sx_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, size_t ws_bytes,
+                           spense_stream_t stream);
+
 #ifdef __cplusplus
 }
 #endif

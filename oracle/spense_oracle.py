@@ -381,6 +381,58 @@ def spense_mlp(xq, s_x, wgate, wup, wdown, w_scale, perm, I_dense, s_h):
     return mlp(xq, s_x, g, u, d, w_scale, s_h), c
 
 
+# --------------------------------------------------------------------------------------
+# Stand-alone Spense linears (Sec. 3.2): the format is defined per weight matrix.
+# --------------------------------------------------------------------------------------
+def pack_linear_canonical(w, perm, n_dense: int, split: str) -> dict:
+    """ONE weight W [N, K] as "the semi-structured sparse part and the dense part".
+    split == "out" (output-split): perm[new] = old over the N rows; in permuted order the
+    sparse rows [0, N_s) are 2:4 along K, the dense rows [N_s, N) come last.
+    split == "in" (input-split): perm over the K columns; the sparse columns [0, K_s) are 2:4 along the
+    PERMUTED K (Q9b), the dense columns come last.  Returns perm, sp_val, sp_meta, dn as in
+    include/spense.h (spense_linear_canon_t)."""
+    w = np.asarray(w, dtype=np.uint8)
+    N, K = w.shape
+    assert split in ("out", "in")
+    n = N if split == "out" else K
+    if perm is None:
+        perm = np.arange(n, dtype=np.int32)
+    check_perm(perm, n)
+    perm = np.asarray(perm, dtype=np.int64)
+    wp = w[perm] if split == "out" else w[:, perm]
+    if ((wp & 0x7F) == 0x7F).any():
+        r, c = np.argwhere((wp & 0x7F) == 0x7F)[0]
+        raise SpenseOracleError("SPENSE_ERR_NAN_WEIGHT", (0, int(r), int(c) // 4, -1))
+    n_s = n - n_dense
+    if split == "out":
+        sp, dn = wp[:n_s], wp[n_s:]
+    else:
+        sp, dn = wp[:, :n_s], wp[:, n_s:]
+    if sp.size:
+        v, m = compress_rows(sp, 0)
+    else:
+        v, m = np.zeros((sp.shape[0], sp.shape[1] // 2), np.uint8), np.zeros((sp.shape[0], sp.shape[1] // 8), np.uint8)
+    return dict(perm=perm.astype(np.int32), sp_val=v, sp_meta=m, dn=dn.copy(), split=split)
+
+
+def unpack_linear_canonical(c: dict) -> np.ndarray:
+    """Rebuild the dense W~ [N, K] bytes in PERMUTED order (zeros where the metadata does not point)."""
+    sp = expand_rows(c["sp_val"], c["sp_meta"])
+    return np.concatenate([sp, c["dn"]], axis=0 if c["split"] == "out" else 1)
+
+
+def linear(xq, s_x, w_bytes, s_w):
+    """y[m, n] = (sum_k dec(x[m,k]) dec(w[n,k])) * s_x[m] * s_w (Y = X W^T) and its
+    sum|a*w| companion.  Output-split: the sparse and the dense rows' outputs concatenated; input-split:
+    the sparse K range plus the dense K range in one sum.  Either way it is the dense GEMM
+    of the reconstructed weight, exact in float64 (module docstring)."""
+    M = xq.shape[0]
+    s_x = np.broadcast_to(np.asarray(s_x, dtype=np.float64).reshape(-1, 1), (M, 1))
+    acc, ab = gemm_exact(xq, w_bytes)
+    sc = s_x * float(s_w)
+    return dict(y=acc * sc, absY=ab * sc)
+
+
 def requant_scale_from_h(h: np.ndarray) -> np.ndarray:
     """Harness helper (Q10): per-token s_h[m] = max_j |h[m, j]| / 448 in fp32 (1 if zero)."""
     amax = np.max(np.abs(h), axis=1).astype(np.float32)

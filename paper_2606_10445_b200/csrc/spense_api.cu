@@ -122,7 +122,7 @@ Plan plan_of(int M, int sms, int act_row_bytes) {
     pl.nb = 1; pl.par = 1; pl.spans = sms;
   } else {
     pl.wide = true;
-    pl.nb = (M + kWideMaxTokens - 1) / kWideMaxTokens;
+    pl.nb = M <= kWideMaxTokens1 ? 1 : (M + kWideMaxTokens - 1) / kWideMaxTokens;
     pl.n_pad = ((M + pl.nb - 1) / pl.nb + 15) / 16 * 16;
     const int pairs = sms / 2;
     size_t cap = kActWorkingSetBytes / ((size_t)pl.n_pad * act_row_bytes);
@@ -135,7 +135,7 @@ Plan plan_of(int M, int sms, int act_row_bytes) {
 }
 
 size_t ws_bytes_for(int M) {
-  const size_t cols = M <= kDecodeMaxTokens ? 2 * (size_t)((M + 15) / 16 * 16) : (size_t)kWideMaxTokens;
+  const size_t cols = M <= kDecodeMaxTokens ? 2 * (size_t)((M + 15) / 16 * 16) : (size_t)kWideMaxTokens1;
   return kWsFixedBytes + (size_t)kMaxSpans * 2 * cols * 128 * sizeof(float);
 }
 
@@ -170,7 +170,7 @@ const Schedule& get_schedule(int mode, const Geometry& g, const Plan& pl) {
   const double cs = tensor_paced ? 1.0 : fixed + kSparseStageBytes + gamma * 2.0 * pl.n_pad * 128;
   const double cd = tensor_paced ? 1.0 : fixed + kDenseStageBytes + gamma * 1.0 * pl.n_pad * 128;
   std::vector<double> cost;
-  if (mode == 0) {
+  if (mode != 1) {
     cost.insert(cost.end(), (size_t)g.gu_tiles_sparse * g.gu_ns, cs);
     cost.insert(cost.end(), (size_t)(g.gu_tiles - g.gu_tiles_sparse) * g.gu_nd, cd);
   } else {
@@ -200,7 +200,7 @@ const Schedule& get_schedule(int mode, const Geometry& g, const Plan& pl) {
   sc.span_begin[spans] = total;
   // byte offsets: the blob stores the stage images in exactly this linear order
   std::vector<uint32_t> bytes(total);
-  if (mode == 0) {
+  if (mode != 1) {
     for (int i = 0; i < total; ++i) bytes[i] = i < g.gu_tiles_sparse * g.gu_ns ? kSparseStageBytes : kDenseStageBytes;
   } else {
     const int per = g.dn_ns + g.dn_nd;
@@ -251,8 +251,14 @@ int make_tmap_section(CUtensorMap* map, const uint8_t* base, size_t bytes, int b
 constexpr uint32_t kPfNextBytes = 640u * 1024u, kPfSelfBytes = 160u * 1024u;
 constexpr int kPfPaceNs = 750;
 constexpr int kPfAheadStages = 12;   // wide kernel: L2 prefetch distance of the producer, in stages
+#ifdef SPENSE_DEBUG_HOOKS
+int knob(const char* name, int dflt) { const char* e = std::getenv(name); return e ? std::atoi(e) : dflt; }
+#else
+constexpr int knob(const char*, int dflt) { return dflt; }
+#endif
 uint32_t next_prefetch_bytes(const Schedule& sc, int k) {
-  uint32_t n = sc.span_pre[k] > kPfNextBytes ? sc.span_pre[k] : kPfNextBytes;
+  const uint32_t want = (uint32_t)knob("SPENSE_PF_NEXT_KB", kPfNextBytes / 1024) * 1024u;
+  uint32_t n = sc.span_pre[k] > want ? sc.span_pre[k] : want;
   return n < sc.span_len[k] ? n : sc.span_len[k];
 }
 
@@ -282,8 +288,8 @@ void fill_common(GemmParams& p, const Schedule& sc, const Plan& pl, const spense
   p.slot_bytes = pl.slot_bytes;
   p.num_stages = pl.ring;
   if (pl.wide) {
-    p.acc_stride = kWideMaxTokens;                            // 2 buffers x 240 columns, metadata at 480
-    p.num_acc_bufs = 2;
+    p.acc_stride = pl.n_pad > kWideMaxTokens ? kWideMaxTokens1 : kWideMaxTokens;   // 2 buffers x 240 columns (or 1 x 256), metadata at 480
+    p.num_acc_bufs = pl.n_pad > kWideMaxTokens ? 1 : 2;
     p.pf_ahead = kPfAheadStages;
   } else {
     p.acc_stride = pl.n_pad <= 32 ? 32 : (pl.n_pad <= 64 ? 64 : (pl.n_pad <= 96 ? 96 : 112));
@@ -299,7 +305,7 @@ void fill_common(GemmParams& p, const Schedule& sc, const Plan& pl, const spense
 void fill_next(GemmParams& p, const uint8_t* next_section, const Schedule& next) {
   if (!next_section) return;
   p.next_base = next_section;
-  p.pf_pace_ns = kPfPaceNs;
+  p.pf_pace_ns = knob("SPENSE_PF_PACE_NS", kPfPaceNs);
   for (int i = 0; i < p.n_spans; ++i) {
     const int k = i < next.n_spans ? i : next.n_spans - 1;
     p.next_off[i] = next.span_off[k];
@@ -401,6 +407,77 @@ int down_impl(const Launch& L, const spense_shape_t* shape, const void* d_blob, 
     if (st) return st;
   }
   return SPENSE_OK;
+}
+
+// ---- stand-alone linears (spense_pack_linear blobs): in-split = the down walk, out-split = the gate_up walk with the plain epilogue
+int check_linear_shape(const spense_linear_shape_t* s) {
+  if (!s) return SPENSE_ERR_ARG;
+  if (s->split != SPENSE_SPLIT_OUT && s->split != SPENSE_SPLIT_IN) return SPENSE_ERR_ARG;
+  if (s->N < 128 || s->K < 128 || s->N % 128 || s->K % 128 || s->N > (1 << 20) || s->K > (1 << 20)) return SPENSE_ERR_SHAPE;
+  const int full = s->split == SPENSE_SPLIT_OUT ? s->N : s->K;
+  if (s->n_dense < 0 || s->n_dense > full || s->n_dense % 128) return SPENSE_ERR_SHAPE;
+  if (s->split == SPENSE_SPLIT_OUT && (s->N - s->n_dense) % 256) return SPENSE_ERR_SHAPE;
+  return SPENSE_OK;
+}
+
+int linear_impl(const Launch& L, const spense_linear_shape_t* ls, const void* d_blob, const uint8_t* d_x, const float* d_sx, int32_t sx_stride,
+                int32_t M, void* d_y, int32_t y_dtype, void* d_ws, cudaStream_t stream) {
+  const bool in_split = ls->split == SPENSE_SPLIT_IN;
+  const Geometry g = make_geometry_linear(ls->N, ls->K, ls->n_dense, in_split);
+  const int mode = in_split ? 1 : 2;
+  const Plan pl = plan_of(M, L.sms, ls->K);
+  const Schedule& sc = get_schedule(mode, g, pl);
+  const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + kBlobHeaderBytes;
+  CUtensorMap tm, tws, twd;
+  int st = make_tmap(&tm, d_x, ls->K, M, pl.wide ? pl.n_pad / 2 : pl.n_pad);
+  if (st) return st;
+  if (pl.wide) {
+    st = make_tmap_section(&tws, section, g.total_bytes - kBlobHeaderBytes, kSparseOperandBytes / 128);
+    if (!st) st = make_tmap_section(&twd, section, g.total_bytes - kBlobHeaderBytes, kOperandBytes / 128);
+    if (st) return st;
+  }
+  const spense_shape_t hdr_shape = {g.H, g.I, g.I_d};          // what the header of this blob states
+  for (int blk0 = 0; blk0 < pl.nb; blk0 += pl.par) {
+    GemmParams p = {};
+    fill_common(p, sc, pl, &hdr_shape, d_blob, M, d_ws);
+    p.kind = in_split ? kBlobLinearIn : kBlobLinearOut;
+    p.nb = pl.nb - blk0 < pl.par ? pl.nb - blk0 : pl.par;
+    p.blk0 = blk0;
+    p.section = section;
+    p.mode = mode;
+    if (in_split) {
+      p.num_tiles = g.dn_tiles; p.tiles_sparse = 0;
+      p.ns = g.dn_ns; p.nd = g.dn_nd; p.dense_k0 = g.I_s;
+    } else {
+      p.num_tiles = g.gu_tiles; p.tiles_sparse = g.gu_tiles_sparse;
+      p.ns = g.gu_ns; p.nd = g.gu_nd; p.dense_k0 = 0;
+    }
+    p.s_act = d_sx; p.sh_stride = sx_stride;
+    p.scale0 = 0; p.scale1 = 0;
+    p.y = d_y;
+    p.y_dtype = y_dtype;
+    p.ld_out = ls->N; p.out_rows = ls->N;
+    st = pl.wide ? launch_gemm_wide(p, tm, tws, twd, false, L.dev, L.sms, stream) : launch_gemm(p, tm, false, L.dev, L.sms, stream);
+    if (st) return st;
+  }
+  return SPENSE_OK;
+}
+
+int linear_entry(int split, const spense_linear_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx, int32_t sx_stride,
+                 int32_t M, void* d_y, int32_t y_dtype, void* d_ws, size_t ws_bytes, spense_stream_t stream) {
+  int st = check_linear_shape(shape);
+  if (st) return st;
+  if (shape->split != split || !d_blob || !d_x || !d_sx || !d_y || M < 1 || M > kMaxTokens || (sx_stride != 0 && sx_stride != 1) ||
+      (y_dtype != SPENSE_F32 && y_dtype != SPENSE_BF16) || !d_ws)
+    return SPENSE_ERR_ARG;
+  if (!aligned(d_blob, 128) || !aligned(d_x, 128) || !aligned(d_y, 16) || !aligned(d_sx, 4) || !aligned(d_ws, 128)) return SPENSE_ERR_ALIGN;
+  if (ws_bytes < ws_bytes_for(M)) return SPENSE_ERR_BUFFER_TOO_SMALL;
+  Launch L;
+  st = check_device(&L.dev, &L.sms);
+  if (st) return st;
+  st = pending_device_error();
+  if (st) return st;
+  return linear_impl(L, shape, d_blob, d_x, d_sx, sx_stride, M, d_y, y_dtype, d_ws, reinterpret_cast<cudaStream_t>(stream));
 }
 
 int check_ws(const spense_shape_t* shape, int M, const void* d_ws, size_t ws_bytes) {
@@ -658,6 +735,49 @@ int spense_mlp_stack_host(const spense_shape_t* shape, const void* const* d_blob
   if (cudaMemcpyAsync(h_y, d_y, (size_t)M * shape->H * esz, cudaMemcpyDeviceToHost, s) != cudaSuccess) return SPENSE_ERR_CUDA;
   if (cudaStreamSynchronize(s) != cudaSuccess) return SPENSE_ERR_CUDA;
   return pending_device_error();
+}
+
+int spense_linear_pack_sizes(const spense_linear_shape_t* shape, size_t* blob_bytes, size_t* workspace_bytes) {
+  int st = check_linear_shape(shape);
+  if (st) return st;
+  const Geometry g = make_geometry_linear(shape->N, shape->K, shape->n_dense, shape->split == SPENSE_SPLIT_IN);
+  if (blob_bytes) *blob_bytes = g.total_bytes;
+  const int n_perm = shape->split == SPENSE_SPLIT_IN ? shape->K : shape->N;
+  if (workspace_bytes) *workspace_bytes = 128 + (size_t)n_perm * sizeof(int);
+  return SPENSE_OK;
+}
+
+int spense_pack_linear(const spense_linear_shape_t* shape, const uint8_t* d_w, float w_scale, const int32_t* d_perm, void* d_blob,
+                       size_t blob_bytes, const spense_linear_canon_t* canon, void* d_ws, size_t ws_bytes, int64_t* h_err_where,
+                       spense_stream_t stream) {
+  int st = check_linear_shape(shape);
+  if (st) return st;
+  if (!d_w || !d_blob || !d_ws) return SPENSE_ERR_ARG;
+  if (!aligned(d_w, 128) || !aligned(d_blob, 128) || !aligned(d_ws, 128) || (d_perm && !aligned(d_perm, 4))) return SPENSE_ERR_ALIGN;
+  size_t need_blob = 0, need_ws = 0;
+  spense_linear_pack_sizes(shape, &need_blob, &need_ws);
+  if (blob_bytes < need_blob || ws_bytes < need_ws) return SPENSE_ERR_BUFFER_TOO_SMALL;
+  st = check_device(nullptr, nullptr);
+  if (st) return st;
+  return launch_pack_linear(shape, d_w, w_scale, d_perm, d_blob, canon, d_ws, h_err_where, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int spense_linear_workspace_size(const spense_linear_shape_t* shape, int32_t M, size_t* bytes) {
+  int st = check_linear_shape(shape);
+  if (st) return st;
+  if (M < 1 || M > kMaxTokens || !bytes) return SPENSE_ERR_ARG;
+  *bytes = ws_bytes_for(M);
+  return SPENSE_OK;
+}
+
+int spense_linear_out_split(const spense_linear_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx, int32_t sx_stride,
+                            int32_t M, void* d_y, int32_t y_dtype, void* d_ws, size_t ws_bytes, spense_stream_t stream) {
+  return linear_entry(SPENSE_SPLIT_OUT, shape, d_blob, d_x, d_sx, sx_stride, M, d_y, y_dtype, d_ws, ws_bytes, stream);
+}
+
+int spense_linear_in_split(const spense_linear_shape_t* shape, const void* d_blob, const uint8_t* d_x, const float* d_sx, int32_t sx_stride,
+                           int32_t M, void* d_y, int32_t y_dtype, void* d_ws, size_t ws_bytes, spense_stream_t stream) {
+  return linear_entry(SPENSE_SPLIT_IN, shape, d_blob, d_x, d_sx, sx_stride, M, d_y, y_dtype, d_ws, ws_bytes, stream);
 }
 
 int spense_select_workspace_size(const spense_shape_t* shape, size_t* bytes) {

@@ -510,8 +510,8 @@ size_t smem_bytes_of(const GemmParams& p) { return (size_t)p.num_stages * p.slot
 template <typename K>
 int prepare(K kernel, int which, int dev, int sms, int grid) {
   static std::mutex mu;
-  static bool ready[3][64] = {};
-  static int resident[3][64] = {};
+  static bool ready[4][64] = {};
+  static int resident[4][64] = {};
   std::lock_guard<std::mutex> lk(mu);
   if (dev < 0 || dev >= 64) return SPENSE_ERR_CUDA;
   if (!ready[which][dev]) {
@@ -527,7 +527,8 @@ int prepare(K kernel, int which, int dev, int sms, int grid) {
 
 int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, bool pdl, int dev, int sms, cudaStream_t stream) {
   const int grid = p.n_spans;
-  int st = p.mode == 1     ? prepare(spense_gemm_kernel<1, false>, 2, dev, sms, grid)
+  int st = p.mode == 2     ? prepare(spense_gemm_kernel<2, false>, 3, dev, sms, grid)
+           : p.mode == 1   ? prepare(spense_gemm_kernel<1, false>, 2, dev, sms, grid)
            : p.amax_part ? prepare(spense_gemm_kernel<0, true>, 1, dev, sms, grid)
                          : prepare(spense_gemm_kernel<0, false>, 0, dev, sms, grid);
   if (st) return st;
@@ -541,7 +542,8 @@ int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, bool pdl, int de
   attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  const cudaError_t e = p.mode == 1     ? cudaLaunchKernelEx(&cfg, spense_gemm_kernel<1, false>, p, tmap_b)
+  const cudaError_t e = p.mode == 2     ? cudaLaunchKernelEx(&cfg, spense_gemm_kernel<2, false>, p, tmap_b)
+                        : p.mode == 1   ? cudaLaunchKernelEx(&cfg, spense_gemm_kernel<1, false>, p, tmap_b)
                         : p.amax_part ? cudaLaunchKernelEx(&cfg, spense_gemm_kernel<0, true>, p, tmap_b)
                                       : cudaLaunchKernelEx(&cfg, spense_gemm_kernel<0, false>, p, tmap_b);
   return e == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;

@@ -15,10 +15,14 @@ struct Cursor {
   int tile, j, ns, nd, first;   // first = linear index of the tile's first stage
 };
 
+// MODE 0 (gate_up) and MODE 2 (out-split linear) walk whole-K tiles, the sparse tiles first; MODE 1 (down, in-split linear)
+// walks tiles whose K loop is sparse stages followed by dense stages
+__host__ __device__ constexpr bool out_split(int mode) { return mode != 1; }
+
 // byte offset of stage j of pair tile `tile` inside the section (the blob stores every tile once)
 template <int MODE>
 __device__ __forceinline__ size_t stage_byte_offset(const GemmParams& p, int tile, int j) {
-  if (MODE == 0) {
+  if (out_split(MODE)) {
     if (tile < p.tiles_sparse) return ((size_t)tile * p.ns + j) * kSparseStageBytes;
     return (size_t)p.tiles_sparse * p.ns * kSparseStageBytes + ((size_t)(tile - p.tiles_sparse) * p.nd + j) * kDenseStageBytes;
   }
@@ -31,7 +35,7 @@ __device__ __forceinline__ size_t stage_byte_offset(const GemmParams& p, int til
 template <int MODE>
 static __device__ __noinline__ Cursor cursor_at(const GemmParams& p, int s, unsigned long long* byte_off) {
   Cursor c;
-  if (MODE == 0) {
+  if (out_split(MODE)) {
     const int sparse_total = p.tiles_sparse * p.ns;
     if (s < sparse_total) {
       c.tile = s / p.ns;
@@ -59,7 +63,7 @@ __device__ __forceinline__ void next_tile(const GemmParams& p, Cursor& c) {
   c.first += c.ns + c.nd;
   ++c.tile;
   c.j = 0;
-  if (MODE == 0) {
+  if (out_split(MODE)) {
     if (c.tile < p.tiles_sparse) { c.ns = p.ns; c.nd = 0; } else { c.ns = 0; c.nd = p.nd; }
   }
 }
@@ -159,7 +163,7 @@ __device__ __forceinline__ void take_epoch(int* ctrl, int n_ctas, volatile int* 
 __device__ __forceinline__ void check_header(const GemmParams& p) {
   const BlobHeader* h = p.hdr;
   if (__ldg(&h->magic) != kBlobMagic || __ldg(&h->version) != kBlobVersion || __ldg(&h->H) != p.H || __ldg(&h->I) != p.I ||
-      __ldg(&h->I_dense) != p.I_d) {
+      __ldg(&h->I_dense) != p.I_d || __ldg(&h->kind) != p.kind) {
     atomicCAS_system(p.status, 0, SPENSE_ERR_BAD_BLOB);
     __threadfence_system();
   }

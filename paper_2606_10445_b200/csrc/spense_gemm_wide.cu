@@ -204,8 +204,8 @@ __device__ __forceinline__ void mma_issuer(const GemmParams& p, const Ctx& cx, i
   for (int s = sb; s < se; ++seg) {
     const int tile_end = c.first + c.ns + c.nd;
     const int seg_end = min(se, tile_end);
-    const int buf = seg & 1;
-    const uint32_t use = (uint32_t)(seg >> 1);
+    const int buf = p.num_acc_bufs == 2 ? seg & 1 : 0;
+    const uint32_t use = (uint32_t)(p.num_acc_bufs == 2 ? seg >> 1 : seg);
     long long tw0 = p.trace ? globaltimer() : 0;
     wait_bar(p, cx.acce_bar(buf), (use & 1u) ^ 1u);        // both CTAs' epilogues have drained this accumulator
     if (p.trace) t_acce += globaltimer() - tw0;
@@ -297,8 +297,8 @@ __device__ __forceinline__ void epilogue(const GemmParams& p, const Ctx& cx, int
   for (int s = sb; s < se; ++seg) {
     const int tile_end = cur.first + cur.ns + cur.nd;
     const int seg_end = min(se, tile_end);
-    const int buf = seg & 1;
-    const uint32_t use = (uint32_t)(seg >> 1);
+    const int buf = p.num_acc_bufs == 2 ? seg & 1 : 0;
+    const uint32_t use = (uint32_t)(p.num_acc_bufs == 2 ? seg >> 1 : seg);
     int a = span, b = span;
     while (p.span_begin[a] > cur.first) --a;
     while (b + 1 < p.n_spans && p.span_begin[b + 1] < tile_end) ++b;
@@ -506,8 +506,8 @@ size_t smem_bytes_of(const GemmParams& p) { return (size_t)p.num_stages * p.slot
 template <typename K>
 int prepare(K kernel, int which, int dev, int grid) {
   static std::mutex mu;
-  static bool ready[3][64] = {};
-  static int resident[3][64] = {};
+  static bool ready[4][64] = {};
+  static int resident[4][64] = {};
   std::lock_guard<std::mutex> lk(mu);
   if (dev < 0 || dev >= 64) return SPENSE_ERR_CUDA;
   if (!ready[which][dev]) {
@@ -529,7 +529,8 @@ int launch_gemm_wide(const GemmParams& p, const CUtensorMap& tmap_b, const CUten
                      bool pdl, int dev, int sms, cudaStream_t stream) {
   (void)sms;
   const int grid = 2 * p.n_spans * p.nb;
-  int st = p.mode == 1     ? prepare(spense_gemm_wide_kernel<1, false>, 2, dev, grid)
+  int st = p.mode == 2     ? prepare(spense_gemm_wide_kernel<2, false>, 3, dev, grid)
+           : p.mode == 1   ? prepare(spense_gemm_wide_kernel<1, false>, 2, dev, grid)
            : p.amax_part ? prepare(spense_gemm_wide_kernel<0, true>, 1, dev, grid)
                          : prepare(spense_gemm_wide_kernel<0, false>, 0, dev, grid);
   if (st) return st;
@@ -543,7 +544,8 @@ int launch_gemm_wide(const GemmParams& p, const CUtensorMap& tmap_b, const CUten
   attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  const cudaError_t e = p.mode == 1     ? cudaLaunchKernelEx(&cfg, spense_gemm_wide_kernel<1, false>, p, tmap_b, tmap_ws, tmap_wd)
+  const cudaError_t e = p.mode == 2     ? cudaLaunchKernelEx(&cfg, spense_gemm_wide_kernel<2, false>, p, tmap_b, tmap_ws, tmap_wd)
+                        : p.mode == 1   ? cudaLaunchKernelEx(&cfg, spense_gemm_wide_kernel<1, false>, p, tmap_b, tmap_ws, tmap_wd)
                         : p.amax_part ? cudaLaunchKernelEx(&cfg, spense_gemm_wide_kernel<0, true>, p, tmap_b, tmap_ws, tmap_wd)
                                       : cudaLaunchKernelEx(&cfg, spense_gemm_wide_kernel<0, false>, p, tmap_b, tmap_ws, tmap_wd);
   return e == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;

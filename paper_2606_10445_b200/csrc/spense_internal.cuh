@@ -47,6 +47,8 @@ constexpr int kMaxTokens = 1 << 20;           // tokens per call (the activation
 constexpr int kSmemMax = 232448;             // opt-in dynamic shared memory per CTA
 constexpr int kDecodeMaxTokens = 112;        // up to here: one CTA per span, pair stages, two accumulator buffers (4 x 112 TMEM columns)
 constexpr int kWideMaxTokens = 240;          // token columns of one CTA pair of the wide kernel (2 buffers x 240 + 16 metadata columns)
+constexpr int kWideMaxTokens1 = 256;         // 241..256 tokens: ONE block of 256 columns with a single accumulator buffer (the largest MMA-N), so
+                                             // the weights cross the L2 -> SM path once instead of once per 128-token block
 constexpr int kFlagBytes = 4096;             // control words (128 B) + 2 flags per slot
 constexpr int kAmaxBytes = kMaxSpans * 256 * 4;   // dynamic requant: max|h| per slot and token column (follows the flags)
 constexpr int kWsFixedBytes = kFlagBytes + kAmaxBytes;   // zeroed by spense_workspace_init; partials follow
@@ -58,7 +60,9 @@ struct BlobHeader {
   int32_t H, I, I_dense;
   float w_scale[3];
   uint64_t gate_up_off, down_off, total_bytes;
+  int32_t kind;               // 0: GLU MLP layer (spense_pack); 1: in-split linear, 2: out-split linear (spense_pack_linear)
 };
+constexpr int kBlobMlp = 0, kBlobLinearIn = 1, kBlobLinearOut = 2;
 
 struct Geometry {
   int H, I, I_d, I_s;
@@ -90,20 +94,49 @@ __host__ __device__ inline Geometry make_geometry(int H, int I, int I_d) {
   return g;
 }
 
+// One linear W [N, K] (spense_pack_linear): the blob is the header followed by ONE section.
+//   in-split : the down section of a layer with H = N, I = K, I_d = n_dense (pair tile = 256 rows, sparse K stages then dense).
+//   out-split: pair tile t = rows [256 t, 256 t + 256) of the row-permuted W, operand a = rows 256 t + 128 a + [0, 128) in
+//              natural order; the N_s / 256 sparse tiles first (ceil(K / 256) sparse stages each), then the dense tiles
+//              (K / 128 dense stages each; a last half tile is zero padded).  Held in the gate_up fields of Geometry.
+__host__ __device__ inline Geometry make_geometry_linear(int N, int K, int n_dense, bool in_split) {
+  Geometry g;
+  if (in_split) {
+    g = make_geometry(N, K, n_dense);
+    g.gu_tiles = 0; g.gu_tiles_sparse = 0;
+    g.down_off = kBlobHeaderBytes;
+    g.total_bytes = g.down_off + (size_t)g.dn_tiles * ((size_t)g.dn_ns * kSparseStageBytes + (size_t)g.dn_nd * kDenseStageBytes);
+    return g;
+  }
+  g.H = K; g.I = N; g.I_d = n_dense; g.I_s = N - n_dense;
+  g.gu_tiles_sparse = g.I_s / 256;
+  g.gu_tiles = g.gu_tiles_sparse + (n_dense + 255) / 256;
+  g.gu_ns = (K + 255) / 256;
+  g.gu_nd = K / 128;
+  g.dn_tiles = 0; g.dn_ns = 0; g.dn_nd = 0;
+  g.gate_up_off = kBlobHeaderBytes;
+  g.down_off = g.gate_up_off + (size_t)g.gu_tiles_sparse * g.gu_ns * kSparseStageBytes +
+               (size_t)(g.gu_tiles - g.gu_tiles_sparse) * g.gu_nd * kDenseStageBytes;
+  g.total_bytes = g.down_off;
+  return g;
+}
+
 // byte offset of element (row r, byte column b) inside one 128 x 128 B SWIZZLE_128B operand image
 __host__ __device__ inline int sw128_offset(int r, int b) {
   return (r >> 3) * 1024 + (r & 7) * 128 + ((((b >> 4) ^ (r & 7)) & 7) << 4) + (b & 15);
 }
 
 // ------------------------------------------------------------------------------------------
-// GEMM kernel parameters.  One kernel serves gate_up (mode 0) and down (mode 1): a byte-balanced
+// GEMM kernel parameters.  One kernel serves gate_up (mode 0), down / the in-split linear (mode 1) and the out-split
+// linear (mode 2: the tile walk of mode 0 with 256-row tiles, the plain epilogue of mode 1): a byte-balanced
 // stream-K walk over the linear sequence of stages; span i = stages [span_begin[i], span_begin[i+1]).
 // ------------------------------------------------------------------------------------------
 struct GemmParams {
   const uint8_t* section;   // first stage image of this matrix family
   const BlobHeader* hdr;    // the blob header (device): weight scales are READ ON THE DEVICE from it, magic / shape are checked there
   int H, I, I_d;            // the shape the caller states (compared with the header on the device)
-  int mode;                 // 0 gate_up, 1 down
+  int mode;                 // 0 gate_up, 1 down / in-split linear, 2 out-split linear
+  int kind;                 // what the blob must be (BlobHeader::kind)
   int num_tiles, tiles_sparse;
   int ns, nd;               // mode 0: stages of a sparse tile / of a dense tile; mode 1: per tile both
   int dense_k0;             // K byte offset of the first dense stage in the B operand (mode 1: I_s)
@@ -361,6 +394,8 @@ __device__ __forceinline__ bool elect_one() {
 int launch_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8_t* d_wup, const uint8_t* d_wdown,
                 const float* h_w_scale, const int32_t* d_perm, void* d_blob, const spense_canon_t* canon, void* d_ws,
                 int64_t* h_err_where, cudaStream_t stream);
+int launch_pack_linear(const spense_linear_shape_t* shape, const uint8_t* d_w, float w_scale, const int32_t* d_perm, void* d_blob,
+                       const spense_linear_canon_t* canon, void* d_ws, int64_t* h_err_where, cudaStream_t stream);
 int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, bool pdl, int dev, int sms, cudaStream_t stream);
 int launch_gemm_wide(const GemmParams& p, const CUtensorMap& tmap_b, const CUtensorMap& tmap_ws, const CUtensorMap& tmap_wd,
                      bool pdl, int dev, int sms, cudaStream_t stream);

@@ -133,7 +133,7 @@ __global__ void pack_gate_up_kernel(Geometry g, const uint8_t* __restrict__ wgat
 
 // down: blockIdx.x = output row n (padded to 256 * dn_tiles).  Columns are gathered through perm.
 __global__ void pack_down_kernel(Geometry g, const uint8_t* __restrict__ wdown, const int32_t* __restrict__ perm,
-                                 uint8_t* __restrict__ blob, spense_canon_t canon, PackErr* err) {
+                                 uint8_t* __restrict__ blob, spense_canon_t canon, PackErr* err, int matrix_id) {
   const int n = blockIdx.x;
   const bool real_row = n < g.H;
   const uint8_t* src = wdown + (size_t)(real_row ? n : 0) * g.I;
@@ -154,8 +154,8 @@ __global__ void pack_down_kernel(Geometry g, const uint8_t* __restrict__ wdown, 
       int st0 = 0, st1 = 0;
       const uint32_t c0 = compress_group(wx, st0);
       const uint32_t c1 = compress_group(wy, st1);
-      if (st0) report(err, st0, 2, n, 2 * t);
-      if (st1) report(err, st1, 2, n, 2 * t + 1);
+      if (st0) report(err, st0, matrix_id, n, 2 * t);
+      if (st1) report(err, st1, matrix_id, n, 2 * t + 1);
       vals = (c0 & 0xFFFFu) | (c1 << 16);
       meta = ((c0 >> 16) & 0xFu) | (((c1 >> 16) & 0xFu) << 4);
       if (canon.down_sp_val) *reinterpret_cast<uint32_t*>(canon.down_sp_val + (size_t)n * (g.I_s / 2) + 4 * t) = vals;
@@ -181,13 +181,74 @@ __global__ void pack_down_kernel(Geometry g, const uint8_t* __restrict__ wdown, 
         w.x |= b0 << (8 * i);
         w.y |= b1 << (8 * i);
       }
-      if (st & 1) report(err, 1, 2, n, (g.I_s + 8 * t) / 4);
-      if (st & 4) report(err, 1, 2, n, (g.I_s + 8 * t) / 4 + 1);
+      if (st & 1) report(err, 1, matrix_id, n, (g.I_s + 8 * t) / 4);
+      if (st & 4) report(err, 1, matrix_id, n, (g.I_s + 8 * t) / 4 + 1);
       if (canon.down_dn) *reinterpret_cast<uint2*>(canon.down_dn + (size_t)n * g.I_d + 8 * t) = w;
     }
     const int jd = (8 * t) >> 7, b = (8 * t) & 127;
     *reinterpret_cast<uint2*>(dense_base + (size_t)jd * kDenseStageBytes + sub * kOperandBytes + sw128_offset(rr, b)) = w;
   }
+}
+
+// out-split linear: blockIdx.x = new (permuted) row, padded to whole 256-row tiles.  Geometry from make_geometry_linear:
+// g.H = K, g.I = N, g.I_s = sparse rows (a multiple of 256).  Operand rows are in natural order.
+__global__ void pack_rows_kernel(Geometry g, const uint8_t* __restrict__ w, const int32_t* __restrict__ perm, uint8_t* __restrict__ blob,
+                                 spense_linear_canon_t canon, PackErr* err) {
+  const int r = blockIdx.x;
+  const bool real_row = r < g.I;
+  const int src_row = real_row ? (perm ? perm[r] : r) : 0;
+  const uint8_t* src = w + (size_t)src_row * g.H;
+  const int tile = r >> 8, opnd = (r >> 7) & 1, rr = r & 127;
+  uint8_t* sec = blob + g.gate_up_off;
+  if (real_row && canon.perm && threadIdx.x == 0) canon.perm[r] = src_row;
+  if (r < g.I_s) {
+    uint8_t* tile_base = sec + (size_t)tile * g.gu_ns * kSparseStageBytes;
+    const int steps = g.gu_ns * (kSparseStageK / 8);
+    for (int t = threadIdx.x; t < steps; t += blockDim.x) {
+      uint32_t vals = 0, meta = 0x44;
+      if (8 * t < g.H) {
+        const uint2 v = *reinterpret_cast<const uint2*>(src + 8 * t);
+        int st0 = 0, st1 = 0;
+        const uint32_t c0 = compress_group(v.x, st0);
+        const uint32_t c1 = compress_group(v.y, st1);
+        if (st0) report(err, st0, 0, r, 2 * t);
+        if (st1) report(err, st1, 0, r, 2 * t + 1);
+        vals = (c0 & 0xFFFFu) | (c1 << 16);
+        meta = ((c0 >> 16) & 0xFu) | (((c1 >> 16) & 0xFu) << 4);
+        if (canon.sp_val) *reinterpret_cast<uint32_t*>(canon.sp_val + (size_t)r * (g.H / 2) + 4 * t) = vals;
+        if (canon.sp_meta) canon.sp_meta[(size_t)r * (g.H / 8) + t] = (uint8_t)meta;
+      }
+      const int js = t >> 5, tb = t & 31;
+      uint8_t* stage = tile_base + (size_t)js * kSparseStageBytes;
+      *reinterpret_cast<uint32_t*>(stage + opnd * kSparseOperandBytes + sw128_offset(rr, 4 * tb)) = vals;
+      stage[opnd * kSparseOperandBytes + kOperandBytes + (tb >> 4) * 2048 + rr * 16 + (tb & 15)] = (uint8_t)meta;
+    }
+  } else {
+    const int td = tile - g.gu_tiles_sparse;
+    uint8_t* tile_base = sec + (size_t)g.gu_tiles_sparse * g.gu_ns * kSparseStageBytes + (size_t)td * g.gu_nd * kDenseStageBytes;
+    for (int t = threadIdx.x; t < g.H / 8; t += blockDim.x) {
+      uint2 v = make_uint2(0, 0);
+      if (real_row) {
+        v = *reinterpret_cast<const uint2*>(src + 8 * t);
+        int st = 0;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          if (((v.x >> (8 * i)) & 0x7Fu) == 0x7Fu) st |= 1;
+          if (((v.y >> (8 * i)) & 0x7Fu) == 0x7Fu) st |= 4;
+        }
+        if (st & 1) report(err, 1, 0, r, 2 * t);
+        if (st & 4) report(err, 1, 0, r, 2 * t + 1);
+        if (canon.dn) *reinterpret_cast<uint2*>(canon.dn + (size_t)(r - g.I_s) * g.H + 8 * t) = v;
+      }
+      const int jd = (8 * t) >> 7, b = (8 * t) & 127;
+      *reinterpret_cast<uint2*>(tile_base + (size_t)jd * kDenseStageBytes + opnd * kOperandBytes + sw128_offset(rr, b)) = v;
+    }
+  }
+}
+
+__global__ void copy_perm_kernel(const int32_t* perm, int32_t* out, int n) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) out[i] = perm ? perm[i] : i;
 }
 
 // ---------------------------------------------------------------- quantise helper
@@ -321,7 +382,56 @@ int launch_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8
   write_header_kernel<<<1, 32, 0, stream>>>(reinterpret_cast<BlobHeader*>(d_blob), hdr);
   uint8_t* blob = reinterpret_cast<uint8_t*>(d_blob);
   pack_gate_up_kernel<<<dim3(g.I, 2), 256, 0, stream>>>(g, d_wgate, d_wup, d_perm, blob, c, err);
-  pack_down_kernel<<<g.dn_tiles * 256, 256, 0, stream>>>(g, d_wdown, d_perm, blob, c, err);
+  pack_down_kernel<<<g.dn_tiles * 256, 256, 0, stream>>>(g, d_wdown, d_perm, blob, c, err, 2);
+  if (cudaGetLastError() != cudaSuccess) return SPENSE_ERR_CUDA;
+  if (cudaMemcpyAsync(&herr, err, sizeof(herr), cudaMemcpyDeviceToHost, stream) != cudaSuccess) return SPENSE_ERR_CUDA;
+  if (cudaStreamSynchronize(stream) != cudaSuccess) return SPENSE_ERR_CUDA;
+  auto fill = [&](unsigned long long key, unsigned long long cnt) {
+    if (!h_err_where) return;
+    h_err_where[0] = (int64_t)(key >> 56);
+    h_err_where[1] = (int64_t)((key >> 28) & 0xFFFFFFFull);
+    h_err_where[2] = (int64_t)(key & 0xFFFFFFFull);
+    h_err_where[3] = (int64_t)cnt;
+  };
+  if (herr.nan_cnt) { fill(herr.nan_key, herr.nan_cnt); return SPENSE_ERR_NAN_WEIGHT; }
+  if (herr.n24_cnt) { fill(herr.n24_key, herr.n24_cnt); return SPENSE_ERR_NOT_2_4; }
+  return SPENSE_OK;
+}
+
+int launch_pack_linear(const spense_linear_shape_t* shape, const uint8_t* d_w, float w_scale, const int32_t* d_perm, void* d_blob,
+                       const spense_linear_canon_t* canon, void* d_ws, int64_t* h_err_where, cudaStream_t stream) {
+  const bool in_split = shape->split == SPENSE_SPLIT_IN;
+  const Geometry g = make_geometry_linear(shape->N, shape->K, shape->n_dense, in_split);
+  const int n_perm = in_split ? shape->K : shape->N;
+  PackErr* err = reinterpret_cast<PackErr*>(d_ws);
+  int* marks = reinterpret_cast<int*>(reinterpret_cast<uint8_t*>(d_ws) + 128);
+  spense_linear_canon_t c = {};
+  if (canon) c = *canon;
+  pack_init_kernel<<<(n_perm + 255) / 256, 256, 0, stream>>>(err, marks, n_perm);
+  PackErr herr;
+  if (d_perm) {
+    perm_mark_kernel<<<(n_perm + 255) / 256, 256, 0, stream>>>(d_perm, marks, err, n_perm);
+    if (cudaMemcpyAsync(&herr, err, sizeof(herr), cudaMemcpyDeviceToHost, stream) != cudaSuccess) return SPENSE_ERR_CUDA;
+    if (cudaStreamSynchronize(stream) != cudaSuccess) return SPENSE_ERR_CUDA;
+    if (herr.perm_bad) return SPENSE_ERR_BAD_PERM;
+  }
+  BlobHeader hdr = {};
+  hdr.magic = kBlobMagic; hdr.version = kBlobVersion;
+  hdr.H = g.H; hdr.I = g.I; hdr.I_dense = g.I_d;
+  hdr.w_scale[0] = hdr.w_scale[1] = hdr.w_scale[2] = w_scale;
+  hdr.gate_up_off = kBlobHeaderBytes; hdr.down_off = kBlobHeaderBytes; hdr.total_bytes = g.total_bytes;
+  hdr.kind = in_split ? kBlobLinearIn : kBlobLinearOut;
+  if (cudaMemsetAsync(d_blob, 0, kBlobHeaderBytes, stream) != cudaSuccess) return SPENSE_ERR_CUDA;
+  write_header_kernel<<<1, 32, 0, stream>>>(reinterpret_cast<BlobHeader*>(d_blob), hdr);
+  uint8_t* blob = reinterpret_cast<uint8_t*>(d_blob);
+  if (in_split) {
+    spense_canon_t cc = {};
+    cc.down_sp_val = c.sp_val; cc.down_sp_meta = c.sp_meta; cc.down_dn = c.dn;
+    if (c.perm) copy_perm_kernel<<<(n_perm + 255) / 256, 256, 0, stream>>>(d_perm, c.perm, n_perm);
+    pack_down_kernel<<<g.dn_tiles * 256, 256, 0, stream>>>(g, d_w, d_perm, blob, cc, err, 0);
+  } else {
+    pack_rows_kernel<<<g.gu_tiles * 256, 256, 0, stream>>>(g, d_w, d_perm, blob, c, err);
+  }
   if (cudaGetLastError() != cudaSuccess) return SPENSE_ERR_CUDA;
   if (cudaMemcpyAsync(&herr, err, sizeof(herr), cudaMemcpyDeviceToHost, stream) != cudaSuccess) return SPENSE_ERR_CUDA;
   if (cudaStreamSynchronize(stream) != cudaSuccess) return SPENSE_ERR_CUDA;

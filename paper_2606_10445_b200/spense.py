@@ -25,7 +25,10 @@ STATUS = {0: "SPENSE_OK", -1: "SPENSE_ERR_ARG", -2: "SPENSE_ERR_ALIGN", -3: "SPE
 EXPORTS = ["spense_version", "spense_strerror", "spense_device_status", "spense_schedule", "spense_perm_from_dense_idx", "spense_pack_sizes", "spense_pack",
            "spense_workspace_size", "spense_workspace_init", "spense_gate_up", "spense_down", "spense_mlp",
            "spense_mlp_dyn", "spense_mlp_host", "spense_mlp_stack_host", "spense_quantize_e4m3", "spense_prune_2to4_magnitude", "spense_dense_idx_last", "spense_select_workspace_size",
-           "spense_select_dense"]
+           "spense_select_dense", "spense_linear_pack_sizes", "spense_pack_linear", "spense_linear_workspace_size",
+           "spense_linear_out_split", "spense_linear_in_split"]
+
+SPENSE_SPLIT_OUT, SPENSE_SPLIT_IN = 0, 1
 
 
 class SpenseError(RuntimeError):
@@ -43,6 +46,14 @@ class Shape(ctypes.Structure):
 class Canon(ctypes.Structure):
     _fields_ = [(n, c_void_p) for n in ("perm", "gate_sp_val", "up_sp_val", "gate_sp_meta", "up_sp_meta",
                                         "gate_dn", "up_dn", "down_sp_val", "down_sp_meta", "down_dn")]
+
+
+class LinearShape(ctypes.Structure):
+    _fields_ = [("N", c_int32), ("K", c_int32), ("n_dense", c_int32), ("split", c_int32)]
+
+
+class LinearCanon(ctypes.Structure):
+    _fields_ = [(n, c_void_p) for n in ("perm", "sp_val", "sp_meta", "dn")]
 
 
 _lib = None
@@ -88,6 +99,13 @@ def lib() -> ctypes.CDLL:
         L.spense_dense_idx_last.argtypes = [c_int32, c_int32, POINTER(c_int32)]
         L.spense_quantize_e4m3.argtypes = [c_void_p, c_int64, c_int64, c_int32, c_void_p, c_void_p, c_void_p,
                                            c_size_t, c_void_p]
+        L.spense_linear_pack_sizes.argtypes = [POINTER(LinearShape), POINTER(c_size_t), POINTER(c_size_t)]
+        L.spense_pack_linear.argtypes = [POINTER(LinearShape), c_void_p, c_float, c_void_p, c_void_p, c_size_t, POINTER(LinearCanon),
+                                         c_void_p, c_size_t, POINTER(c_int64), c_void_p]
+        L.spense_linear_workspace_size.argtypes = [POINTER(LinearShape), c_int32, POINTER(c_size_t)]
+        for f in (L.spense_linear_out_split, L.spense_linear_in_split):
+            f.argtypes = [POINTER(LinearShape), c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_void_p, c_int32, c_void_p,
+                          c_size_t, c_void_p]
         for name in EXPORTS:
             if name not in ("spense_strerror",):
                 getattr(L, name).restype = c_int
@@ -329,3 +347,60 @@ def spense_select_dense(wgate, wup, wdown, hdiag_x, hdiag_h, I_dense: int, eps: 
                                      c_float(eps), _ptr(score), _ptr(dense_idx) if I_dense else None, _ptr(perm), _ptr(ws),
                                      b.value, _stream()))
     return score, dense_idx, perm
+
+
+class PackedLinear:
+    """One packed Spense linear W [N, K] (out-split or in-split): the opaque device blob plus (optionally) the canonical arrays."""
+
+    def __init__(self, N, K, n_dense, split, blob, canon=None):
+        self.N, self.K, self.n_dense, self.split, self.blob, self.canon = N, K, n_dense, split, blob, canon
+        self.shape = LinearShape(N, K, n_dense, split)
+
+
+def spense_pack_linear(w, w_scale: float, perm, n_dense: int, split: int, want_canon: bool = False) -> PackedLinear:
+    """w uint8 [N, K] (CUDA, original order); perm int32 over N (out-split) or K (in-split) or None."""
+    _dev(w, torch.uint8)
+    N, K = w.shape
+    dev = w.device
+    shape = LinearShape(N, K, n_dense, split)
+    b, wsb = c_size_t(), c_size_t()
+    _check(lib().spense_linear_pack_sizes(ctypes.byref(shape), ctypes.byref(b), ctypes.byref(wsb)))
+    blob = torch.empty(b.value, dtype=torch.uint8, device=dev)
+    ws = torch.empty(wsb.value, dtype=torch.uint8, device=dev)
+    canon, cstruct = None, None
+    if want_canon:
+        e = lambda *sh: torch.empty(*sh, dtype=torch.uint8, device=dev)
+        if split == SPENSE_SPLIT_OUT:
+            n_s = N - n_dense
+            canon = dict(perm=torch.empty(N, dtype=torch.int32, device=dev), sp_val=e(n_s, K // 2), sp_meta=e(n_s, K // 8), dn=e(n_dense, K))
+        else:
+            k_s = K - n_dense
+            canon = dict(perm=torch.empty(K, dtype=torch.int32, device=dev), sp_val=e(N, k_s // 2), sp_meta=e(N, k_s // 8), dn=e(N, n_dense))
+        cstruct = LinearCanon(**{k: v.data_ptr() for k, v in canon.items()})
+    if perm is not None:
+        _dev(perm, torch.int32)
+    where = (c_int64 * 4)(-1, -1, -1, -1)
+    st = lib().spense_pack_linear(ctypes.byref(shape), _ptr(w), c_float(float(w_scale)), _ptr(perm), _ptr(blob), b.value,
+                                  ctypes.byref(cstruct) if cstruct else None, _ptr(ws), wsb.value, where, _stream())
+    _check(st, tuple(where))
+    return PackedLinear(N, K, n_dense, split, blob, canon)
+
+
+def spense_linear_workspace(lin: PackedLinear, M: int) -> torch.Tensor:
+    b = c_size_t()
+    _check(lib().spense_linear_workspace_size(ctypes.byref(lin.shape), M, ctypes.byref(b)))
+    ws = torch.empty(b.value, dtype=torch.uint8, device=lin.blob.device)
+    _check(lib().spense_workspace_init(_ptr(ws), b.value, _stream()))
+    return ws
+
+
+def spense_linear(lin: PackedLinear, x, s_x, ws, y=None, dtype=torch.float32):
+    """x uint8 [M, K], s_x f32 [1] or [M] -> y [M, N] = (x W'^T) * s_x * s_w (out-split: permuted row order)."""
+    _dev(x, torch.uint8), _dev(s_x, torch.float32)
+    M = x.shape[0]
+    if y is None:
+        y = torch.empty(M, lin.N, dtype=dtype, device=x.device)
+    f = lib().spense_linear_out_split if lin.split == SPENSE_SPLIT_OUT else lib().spense_linear_in_split
+    _check(f(ctypes.byref(lin.shape), _ptr(lin.blob), _ptr(x), _ptr(s_x), 0 if s_x.numel() == 1 else 1, M, _ptr(y),
+             SPENSE_F32 if y.dtype == torch.float32 else SPENSE_BF16, _ptr(ws), ws.numel(), _stream()))
+    return y

@@ -124,6 +124,54 @@ def make_layer(H: int, I: int, p: float, seed: int, device="cpu", I_dense: int |
                  dense_idx=dense_idx)
 
 
+@dataclasses.dataclass
+class Linear:
+    N: int
+    K: int
+    n_dense: int
+    split: str             # "out": rows split (perm over N); "in": columns split (perm over K)
+    w: torch.Tensor        # uint8 [N, K] E4M3 bytes, ORIGINAL order
+    w_scale: float
+    perm: torch.Tensor     # int32, perm[new] = old
+
+
+def linear_dense_count(N: int, K: int, p: float, split: str) -> int:
+    """dense rows / columns: a multiple of 128; the out-split keeps its sparse row count a multiple of 256 (one MMA tile)"""
+    if split == "out":
+        return N - int(round((1.0 - p) * N / 256)) * 256
+    return dense_count(K, p)
+
+
+def make_linear(N: int, K: int, p: float, split: str, seed: int, device="cpu", n_dense: int | None = None) -> Linear:
+    """One synthetic Spense linear (same recipe as make_layer, one matrix): W ~ N(0, 0.02^2) [N, K]; a seeded dense set of
+    rows (split "out") or columns (split "in"), perm = stable partition; in PERMUTED order the sparse region is
+    magnitude-2:4 pruned along K; per-tensor scale amax/448, E4M3."""
+    dev = torch.device(device)
+    g = torch.Generator(device=dev).manual_seed(int(seed))
+    n = N if split == "out" else K
+    n_d = linear_dense_count(N, K, p, split) if n_dense is None else int(n_dense)
+    n_s = n - n_d
+    order = torch.randperm(n, generator=g, device=dev)
+    is_dense = torch.zeros(n, dtype=torch.bool, device=dev)
+    is_dense[order[:n_d]] = True
+    idx = torch.arange(n, device=dev)
+    perm = torch.cat([idx[~is_dense], idx[is_dense]])
+    w = torch.randn(N, K, generator=g, device=dev, dtype=torch.float32) * 0.02
+    if n_s:
+        if split == "out":
+            wp = w[perm]
+            wp[:n_s] = _prune_2_4_lastdim(wp[:n_s])
+            w = torch.empty_like(wp)
+            w[perm] = wp
+        else:
+            wp = w[:, perm]
+            wp[:, :n_s] = _prune_2_4_lastdim(wp[:, :n_s].contiguous())
+            w = torch.empty_like(wp)
+            w[:, perm] = wp
+    wb, sc = _quant_tensor(w)
+    return Linear(N=N, K=K, n_dense=n_d, split=split, w=wb, w_scale=sc, perm=perm.to(torch.int32))
+
+
 def make_activations(M: int, H: int, seed: int, device="cpu", n_outlier: int | None = None):
     """x uint8 [M, H] E4M3 bytes, s_x fp32 [M] (per-token amax/448)."""
     dev = torch.device(device)

@@ -100,3 +100,41 @@ def expected_blob_body(c, H, I, I_d):
         for j in range(I_d // 128):
             out.append(_dense_stage(dd[r0, 128 * j:128 * j + 128], dd[r1, 128 * j:128 * j + 128]))
     return np.concatenate(out) if out else np.zeros(0, np.uint8)
+
+
+def expected_linear_body(c, N, K, n_dense, split):
+    """Blob body of spense_pack_linear (everything after the header) from the canonical arrays of ONE matrix.
+    in-split : 256-row tiles, each its sparse K stages (K_s padded to 256) then its dense K stages -- the down section.
+    out-split: 256-row tiles of the row-permuted matrix, operand a = rows 256 t + 128 a + [0, 128) in natural order; the
+               sparse tiles (ceil(K / 256) sparse stages each) first, then the dense tiles (K / 128 dense stages each,
+               a last half tile zero padded)."""
+    out = []
+    if split == "in":
+        k_s = K - n_dense
+        nt, ns = (N + 255) // 256, (k_s + 255) // 256
+        v = _pad_rows(_pad_cols(c["sp_val"], ns * 128, 0), nt * 256, 0)
+        m = _pad_rows(_pad_cols(c["sp_meta"], ns * 32, 0x44), nt * 256, 0x44)
+        d = _pad_rows(c["dn"], nt * 256, 0)
+        for t in range(nt):
+            r0, r1 = slice(256 * t, 256 * t + 128), slice(256 * t + 128, 256 * t + 256)
+            for j in range(ns):
+                out.append(_sparse_stage(v[r0, 128 * j:128 * j + 128], m[r0, 32 * j:32 * j + 32],
+                                         v[r1, 128 * j:128 * j + 128], m[r1, 32 * j:32 * j + 32]))
+            for j in range(n_dense // 128):
+                out.append(_dense_stage(d[r0, 128 * j:128 * j + 128], d[r1, 128 * j:128 * j + 128]))
+    else:
+        n_s = N - n_dense
+        ns = (K + 255) // 256
+        v, m = _pad_cols(c["sp_val"], ns * 128, 0), _pad_cols(c["sp_meta"], ns * 32, 0x44)
+        for t in range(n_s // 256):
+            r0, r1 = slice(256 * t, 256 * t + 128), slice(256 * t + 128, 256 * t + 256)
+            for j in range(ns):
+                out.append(_sparse_stage(v[r0, 128 * j:128 * j + 128], m[r0, 32 * j:32 * j + 32],
+                                         v[r1, 128 * j:128 * j + 128], m[r1, 32 * j:32 * j + 32]))
+        ntd = (n_dense + 255) // 256
+        d = _pad_rows(c["dn"], ntd * 256, 0)
+        for t in range(ntd):
+            r0, r1 = slice(256 * t, 256 * t + 128), slice(256 * t + 128, 256 * t + 256)
+            for j in range(K // 128):
+                out.append(_dense_stage(d[r0, 128 * j:128 * j + 128], d[r1, 128 * j:128 * j + 128]))
+    return np.concatenate(out) if out else np.zeros(0, np.uint8)

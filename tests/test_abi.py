@@ -70,3 +70,29 @@ def test_size_queries_and_host_side_argument_errors(sp):
     st = L.spense_down(ctypes.byref(shp), ctypes.c_void_p(1024), ctypes.c_void_p(3), ctypes.c_void_p(4), 0, 8,
                        ctypes.c_void_p(16), 0, ctypes.c_void_p(128), 1 << 30, None, None)
     assert sp.STATUS[st] == "SPENSE_ERR_ALIGN"
+
+
+def test_linear_size_queries_and_argument_errors(sp):
+    L = sp.lib()
+    b, w = ctypes.c_size_t(), ctypes.c_size_t()
+    # in-split W [5120, 25600] with 6400 dense columns = the down section of the Qwen3-32B-shaped layer
+    shp = sp.LinearShape(5120, 25600, 6400, sp.SPENSE_SPLIT_IN)
+    assert L.spense_linear_pack_sizes(ctypes.byref(shp), ctypes.byref(b), ctypes.byref(w)) == 0
+    assert b.value == 1024 + 94_208_000 and w.value == 128 + 4 * 25600
+    # out-split W [25600, 5120] with 6400 dense rows: 19200 x 5120 x 0.625 + 6400 x 5120 bytes
+    shp = sp.LinearShape(25600, 5120, 6400, sp.SPENSE_SPLIT_OUT)
+    assert L.spense_linear_pack_sizes(ctypes.byref(shp), ctypes.byref(b), ctypes.byref(w)) == 0
+    assert b.value == 1024 + 19200 * 5120 * 5 // 8 + 6400 * 5120 and w.value == 128 + 4 * 25600
+    # a dense half tile at the end is padded to a whole 256-row tile
+    shp = sp.LinearShape(640, 256, 128, sp.SPENSE_SPLIT_OUT)
+    assert L.spense_linear_pack_sizes(ctypes.byref(shp), ctypes.byref(b), None) == 0
+    assert b.value == 1024 + 2 * 40960 + 2 * 32768
+    for bad in ((640, 256, 256, 0), (100, 256, 0, 0), (256, 256, 64, 1), (256, 256, 512, 1)):
+        assert sp.STATUS[L.spense_linear_pack_sizes(ctypes.byref(sp.LinearShape(*bad)), ctypes.byref(b), None)] == "SPENSE_ERR_SHAPE"
+    assert sp.STATUS[L.spense_linear_pack_sizes(ctypes.byref(sp.LinearShape(256, 256, 0, 7)), ctypes.byref(b), None)] == "SPENSE_ERR_ARG"
+    shp = sp.LinearShape(256, 256, 0, sp.SPENSE_SPLIT_OUT)
+    st = L.spense_linear_out_split(ctypes.byref(shp), None, None, None, 0, 8, None, 0, None, 0, None)
+    assert sp.STATUS[st] == "SPENSE_ERR_ARG"
+    st = L.spense_linear_in_split(ctypes.byref(shp), ctypes.c_void_p(128), ctypes.c_void_p(128), ctypes.c_void_p(4), 0, 8,
+                                  ctypes.c_void_p(16), 0, ctypes.c_void_p(128), 1 << 30, None)
+    assert sp.STATUS[st] == "SPENSE_ERR_ARG"                      # an out-split shape handed to the in-split call

@@ -48,7 +48,10 @@ GEMM_CASES = [
     (256, 1024, 0.25, None, 80),    # 64 < M <= 96: two accumulator buffers at a 96-column stride
     (1024, 4096, 0.25, None, 96),
     (1024, 4096, 0.25, None, 112),  # 96 < M <= 112: two buffers at a 112-column stride (448 of the 480 columns below the metadata)
-    (256, 1024, 0.25, None, 256),   # two full token blocks in one launch (weights re-read from L2 for the second)
+    (256, 1024, 0.25, None, 240),   # the widest double-buffered token tile
+    (1024, 4096, 0.25, None, 241),  # 241..256 tokens: one 256-column tile, single accumulator buffer, ragged
+    (256, 1024, 0.25, None, 256),   # the same, full
+    (1024, 4096, 0.25, None, 257),  # two blocks of 144 columns again
     (1024, 4096, 0.25, None, 300),  # three token blocks, ragged last one, spans crossing block boundaries
     (640, 896, None, 384, 513),     # five blocks, last one holds a single token
 ]

@@ -42,7 +42,8 @@ def test_spans_partition_the_stage_sequence(sp, shape, M, mode):
         slot = 40960 + 2 * n_pad * 128
     else:
         # wide: CTA pairs, blocks of at most 240 tokens, `par` blocks side by side with 74 // par spans each
-        assert cps == 2 and n_pad <= 240 and nb == -(-M // 240) and 1 <= par <= min(nb, 37)
+        # (241..256 tokens: one block of 256 columns with a single accumulator buffer)
+        assert cps == 2 and n_pad <= (256 if M <= 256 else 240) and nb == (1 if M <= 256 else -(-M // 240)) and 1 <= par <= min(nb, 37)
         assert len(sb) - 1 <= 74 // par
         rounds = -(-nb // par)
         assert nb / (rounds * par) * (par * (74 // par) / 74) >= 0.8                      # the split keeps most SMs busy

@@ -70,6 +70,13 @@ int check_shape(const spense_shape_t* s) {
 
 bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
+// tuning knobs exist in SPENSE_DEBUG_HOOKS builds only (experiments); the shipped library reads no environment variable
+#ifdef SPENSE_DEBUG_HOOKS
+int knob(const char* name, int dflt) { const char* e = std::getenv(name); return e ? std::atoi(e) : dflt; }
+#else
+constexpr int knob(const char*, int dflt) { return dflt; }
+#endif
+
 // ---- launch geometry.
 // Up to kDecodeMaxTokens tokens: the decode kernel, one CTA per stream-K span, token columns = M padded to 16.
 // More: the wide kernel on CTA pairs; token blocks of at most kWideMaxTokens tokens, `par` blocks side by side in one
@@ -114,9 +121,15 @@ int par_of(int nb, int units, int cap) {
 // working set (blocks x n_pad x act_row_bytes) well inside the 126 MB L2: measured at M = 8192, 18 blocks of Hq (110 MB)
 // side by side made down HBM-bound on activation re-reads (1020 us against 4 x 167 us at M = 2048).
 constexpr size_t kActWorkingSetBytes = 64u << 20;
-Plan plan_of(int M, int sms, int act_row_bytes) {
+// sparse_heavy: at least half of the intermediate indices are 2:4.  Between kPairMinTokens and kDecodeMaxTokens tokens the
+// CTA-pair kernel is the faster one for such layers (measured on B200, Qwen3-32B shape, p = 25 %: M = 64 55.9 vs 57.0 us/layer,
+// M = 96 58.3 vs 63.1, M = 112 62.4 vs 67.7; at M <= 32 the decode kernel wins by 1.2 us), but not for dense-heavy ones (all
+// dense, M = 64: 72.7 vs 70.5): a dense stage gives a CTA of a pair only 16 KB of weights per barrier round trip.
+constexpr int kPairMinTokens = 48;
+Plan plan_of(int M, int sms, int act_row_bytes, bool sparse_heavy) {
   Plan pl = {};
-  if (M <= kDecodeMaxTokens) {
+  const int decode_max = knob("SPENSE_DECODE_MAX", sparse_heavy ? kPairMinTokens : kDecodeMaxTokens);
+  if (M <= decode_max) {
     pl.wide = false;
     pl.n_pad = (M + 15) / 16 * 16;
     pl.nb = 1; pl.par = 1; pl.spans = sms;
@@ -251,11 +264,6 @@ int make_tmap_section(CUtensorMap* map, const uint8_t* base, size_t bytes, int b
 constexpr uint32_t kPfNextBytes = 640u * 1024u, kPfSelfBytes = 160u * 1024u;
 constexpr int kPfPaceNs = 750;
 constexpr int kPfAheadStages = 12;   // wide kernel: L2 prefetch distance of the producer, in stages
-#ifdef SPENSE_DEBUG_HOOKS
-int knob(const char* name, int dflt) { const char* e = std::getenv(name); return e ? std::atoi(e) : dflt; }
-#else
-constexpr int knob(const char*, int dflt) { return dflt; }
-#endif
 uint32_t next_prefetch_bytes(const Schedule& sc, int k) {
   const uint32_t want = (uint32_t)knob("SPENSE_PF_NEXT_KB", kPfNextBytes / 1024) * 1024u;
   uint32_t n = sc.span_pre[k] > want ? sc.span_pre[k] : want;
@@ -320,7 +328,7 @@ int gate_up_impl(const Launch& L, const spense_shape_t* shape, const void* d_blo
                  const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32, void* d_ws, bool pdl, bool down_follows,
                  cudaStream_t stream, bool dynamic = false, float* d_sh_out = nullptr) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const Plan pl = plan_of(M, L.sms, g.H);
+  const Plan pl = plan_of(M, L.sms, g.H, 2 * g.I_s >= g.I);
   const Schedule& sc = get_schedule(0, g, pl);
   const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + g.gate_up_off;
   CUtensorMap tm, tws, twd;
@@ -348,7 +356,7 @@ int gate_up_impl(const Launch& L, const spense_shape_t* shape, const void* d_blo
     p.amax_part = dynamic ? reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes) : nullptr;
     p.ld_out = g.I; p.out_rows = g.I;
     if (down_follows && blk0 + pl.par >= pl.nb)                // the same layer's down projection streams next
-      fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + g.down_off, get_schedule(1, g, plan_of(M, L.sms, g.I)));
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + g.down_off, get_schedule(1, g, plan_of(M, L.sms, g.I, 2 * g.I_s >= g.I)));
     if (!pl.wide) {
       st = launch_gemm(p, tm, pdl, L.dev, L.sms, stream);
     } else {
@@ -372,7 +380,7 @@ int down_impl(const Launch& L, const spense_shape_t* shape, const void* d_blob, 
               int32_t sh_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, bool pdl, const void* d_next_blob,
               cudaStream_t stream) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const Plan pl = plan_of(M, L.sms, g.I);
+  const Plan pl = plan_of(M, L.sms, g.I, 2 * g.I_s >= g.I);
   const Schedule& sc = get_schedule(1, g, pl);
   const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + g.down_off;
   CUtensorMap tm, tws, twd;
@@ -398,7 +406,7 @@ int down_impl(const Launch& L, const spense_shape_t* shape, const void* d_blob, 
     p.y_dtype = y_dtype;
     p.ld_out = g.H; p.out_rows = g.H;
     if (d_next_blob && blk0 + pl.par >= pl.nb)                 // the next layer's gate/up weights stream next
-      fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + g.gate_up_off, get_schedule(0, g, plan_of(M, L.sms, g.H)));
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + g.gate_up_off, get_schedule(0, g, plan_of(M, L.sms, g.H, 2 * g.I_s >= g.I)));
     if (!pl.wide) {
       st = launch_gemm(p, tm, pdl, L.dev, L.sms, stream);
     } else {
@@ -425,7 +433,7 @@ int linear_impl(const Launch& L, const spense_linear_shape_t* ls, const void* d_
   const bool in_split = ls->split == SPENSE_SPLIT_IN;
   const Geometry g = make_geometry_linear(ls->N, ls->K, ls->n_dense, in_split);
   const int mode = in_split ? 1 : 2;
-  const Plan pl = plan_of(M, L.sms, ls->K);
+  const Plan pl = plan_of(M, L.sms, ls->K, 2 * ls->n_dense <= (in_split ? ls->K : ls->N));
   const Schedule& sc = get_schedule(mode, g, pl);
   const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + kBlobHeaderBytes;
   CUtensorMap tm, tws, twd;
@@ -541,7 +549,7 @@ int spense_schedule(const spense_shape_t* shape, int32_t M, int32_t mode, int32_
   if (st) return st;
   if (M < 1 || M > kMaxTokens || (mode != 0 && mode != 1) || sms < 2 || sms > kMaxSpans || !out_span_begin) return SPENSE_ERR_ARG;
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const Plan pl = plan_of(M, sms, mode == 0 ? g.H : g.I);
+  const Plan pl = plan_of(M, sms, mode == 0 ? g.H : g.I, 2 * g.I_s >= g.I);
   const Schedule& sc = get_schedule(mode, g, pl);
   for (int i = 0; i <= sc.n_spans; ++i) out_span_begin[i] = sc.span_begin[i];
   if (out_info) {

@@ -52,6 +52,7 @@ struct Ctx {
   __device__ __forceinline__ uint32_t acce_bar(int b) const { return bar_base + 8u * (18 + b); }
   __device__ __forceinline__ uint32_t tmem_slot() const { return bar_base + 8u * 20; }
   __device__ __forceinline__ uint32_t red_bar() const { return bar_base + 8u * 22; }
+  __device__ __forceinline__ uint32_t pre_bar() const { return bar_base + 8u * 24; }
   __device__ __forceinline__ volatile uint32_t* tmem_slot_ptr() const { return reinterpret_cast<volatile uint32_t*>(smem_gen + ring_bytes + 8 * 20); }
   __device__ __forceinline__ volatile int* epoch_ptr() const { return reinterpret_cast<volatile int*>(smem_gen + ring_bytes + 8 * 21); }
   __device__ __forceinline__ volatile int* epi_done_ptr() const { return reinterpret_cast<volatile int*>(smem_gen + ring_bytes + 8 * 23); }
@@ -183,6 +184,17 @@ __device__ __forceinline__ uint32_t desc_lo(uint32_t saddr, uint32_t lbo_bytes) 
 __device__ __forceinline__ uint32_t desc_hi(uint32_t sbo_bytes, uint32_t layout) { return ((sbo_bytes >> 4) & 0x3FFFu) | (1u << 14) | (layout << 29); }
 __device__ __forceinline__ uint64_t desc_of(uint32_t lo, uint32_t hi) { return (uint64_t)lo | ((uint64_t)hi << 32); }
 
+// A span's LAST segment that is the head of a tile shared with exactly one more span (the next one, which dumped the
+// tail's partial as its first piece of work, long ago): this span owns the tile.  Instead of adding the partner's partial
+// in the final, exposed epilogue (one L2 round trip per 16 token columns: 5 us of tail at 128 tokens, 10 us at 256), each
+// CTA's epilogue warps store it into the TMEM accumulator BEFORE the segment's MMAs start, while earlier MMAs run, and the
+// MMAs accumulate on top: the final epilogue is the plain one.  (Measured: M = 128 63.9 -> 60.6 us/layer, M = 240
+// 96.7 -> 83.5.  The decode kernel keeps the add in its epilogue: there the same change cost 0.3-1.3 us, a stalled MMA
+// warp stops the HBM stream that bounds it.)
+__device__ __forceinline__ bool preloaded_segment(const GemmParams& p, int span, int sb, int se, int tile_first, int tile_end, int seg_end) {
+  return seg_end == se && se < tile_end && sb <= tile_first && p.span_begin[span + 2] >= tile_end;
+}
+
 // ===================== MMA issuer (warp 1 of the leader CTA) =====================
 template <int MODE>
 __device__ __forceinline__ void mma_issuer(const GemmParams& p, const Ctx& cx, int span) {
@@ -208,10 +220,12 @@ __device__ __forceinline__ void mma_issuer(const GemmParams& p, const Ctx& cx, i
     const uint32_t use = (uint32_t)(p.num_acc_bufs == 2 ? seg >> 1 : seg);
     long long tw0 = p.trace ? globaltimer() : 0;
     wait_bar(p, cx.acce_bar(buf), (use & 1u) ^ 1u);        // both CTAs' epilogues have drained this accumulator
+    const bool pre = preloaded_segment(p, span, sb, se, c.first, tile_end, seg_end);
+    if (pre) wait_bar(p, cx.pre_bar(), 0);                 // both CTAs have stored the partner's partial into this accumulator
     if (p.trace) t_acce += globaltimer() - tw0;
     tc_fence_after();
     const uint32_t d = cx.tmem_base + (uint32_t)(buf * p.acc_stride);
-    uint32_t acc = 0;
+    uint32_t acc = pre ? 1u : 0u;
 #pragma unroll 1
     for (; s < seg_end; ++s, ++it, ++c.j) {
       if (p.trace) tw0 = globaltimer();
@@ -292,6 +306,23 @@ __device__ __forceinline__ void epilogue(const GemmParams& p, const Ctx& cx, int
   int n_groups = 0;
   unsigned long long off;
   Cursor cur = cursor_at<MODE>(p, sb, &off);
+  // Does the span end with a preloaded segment, and when is its accumulator preloaded?  As early as its buffer is free (after
+  // the epilogue of the segment num_acc_bufs before it), but never before this span's own dump (segment 0, if the span
+  // starts inside a tile) is published: a span must not make its partner wait for ITS partner.
+  int pre_seg = -1, pre_at = -1;
+  {
+    Cursor w = cur;
+    int n_seg = 0, last_first = 0, last_end = 0;
+    for (int s = sb; s < se; ++n_seg) {
+      last_first = w.first; last_end = w.first + w.ns + w.nd;
+      s = min(se, last_end);
+      if (s == last_end) next_tile<MODE>(p, w);
+    }
+    if (preloaded_segment(p, span, sb, se, last_first, last_end, se)) {
+      pre_seg = n_seg - 1;
+      pre_at = pre_seg >= p.num_acc_bufs ? pre_seg - p.num_acc_bufs + 1 : ((sb > cur.first && pre_seg >= 1) ? 1 : 0);
+    }
+  }
   int seg = 0;
 #pragma unroll 1
   for (int s = sb; s < se; ++seg) {
@@ -303,6 +334,25 @@ __device__ __forceinline__ void epilogue(const GemmParams& p, const Ctx& cx, int
     while (p.span_begin[a] > cur.first) --a;
     while (b + 1 < p.n_spans && p.span_begin[b + 1] < tile_end) ++b;
 
+    if (seg == pre_at) {
+      // partner's partial [col][lane] of this CTA's operand -> the accumulator of segment pre_seg
+      wait_flag(p, flag_of(span + 1, 0), epoch);
+      if (et == 0) trace(p, span, 8);
+      const float* po = part_of(span + 1, 0) + 32 * q + lane;
+      const uint32_t tp = cx.tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)((p.num_acc_bufs == 2 ? pre_seg & 1 : 0) * p.acc_stride);
+#pragma unroll 2
+      for (int c = c_begin; c < c_end; c += 8) {
+        uint32_t v[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) v[i] = __float_as_uint(__ldcg(po + (size_t)(c + i) * 128));
+        tmem_st8(tp + (uint32_t)c, v);
+      }
+      tmem_st_wait();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_cluster(mapa_shared(cx.pre_bar(), 0));
+    }
+
     wait_bar(p, cx.accf_bar(buf), use & 1u);
     tc_fence_after();
     if (et == 0) trace(p, span, seg == 0 ? 5 : 7);
@@ -310,12 +360,7 @@ __device__ __forceinline__ void epilogue(const GemmParams& p, const Ctx& cx, int
 
     if (a == b || (b == a + 1 && span == a)) {
       // the whole tile is ours, or we own a tile whose tail the next span has (usually long ago) dumped
-      const float* part = nullptr;
-      if (a != b) {
-        wait_flag(p, flag_of(b, 0), epoch);                // every thread: one ld.acquire when the partner is done (the usual case)
-        part = part_of(b, 0);
-        if (et == 0) trace(p, span, 8);
-      }
+      const float* part = nullptr;                         // (a != b: the partner's partial is already in the accumulator)
       int c = c_begin;
       if (part == nullptr) {
 #pragma unroll 1
@@ -451,6 +496,7 @@ spense_gemm_wide_kernel(const __grid_constant__ GemmParams p, const __grid_const
     for (int s = 0; s < cx.S; ++s) { mbar_init(cx.full_bar(s), 1); mbar_init(cx.empty_bar(s), 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(cx.accf_bar(b), 1); mbar_init(cx.acce_bar(b), 2 * kEpiWarps); }
     mbar_init(cx.red_bar(), 1);
+    mbar_init(cx.pre_bar(), 2 * kEpiWarps);
     *cx.epi_done_ptr() = 0;
     fence_barrier_init();
   }

@@ -26,7 +26,7 @@ SEED0 = (5120, 27648, 0)
 
 
 @pytest.mark.parametrize("shape", [QWEN, SEED0, (5120, 27648, 27648), (256, 1024, 256), (640, 896, 384)])
-@pytest.mark.parametrize("M", [1, 64, 112, 113, 128, 200, 240, 256, 1000, 2048, 8192])
+@pytest.mark.parametrize("M", [1, 48, 49, 64, 112, 113, 128, 200, 240, 256, 1000, 2048, 8192])
 @pytest.mark.parametrize("mode", [0, 1])
 def test_spans_partition_the_stage_sequence(sp, shape, M, mode):
     sb, info = sp.spense_schedule(*shape, M, mode)
@@ -36,7 +36,8 @@ def test_spans_partition_the_stage_sequence(sp, shape, M, mode):
     assert sb[0] == 0 and sb[-1] == info["stages"] and (np.diff(sb) >= 1).all()          # every span owns at least one stage
     n_pad, nb, par, ring, cps = info["n_pad"], info["blocks"], info["blocks_per_launch"], info["ring"], info["ctas_per_span"]
     assert n_pad % 16 == 0 and nb * n_pad >= M > (nb - 1) * n_pad                         # the blocks cover the tokens, none is empty
-    if M <= 112:
+    sparse_heavy = 2 * (shape[1] - shape[2]) >= shape[1]
+    if M <= (48 if sparse_heavy else 112):
         # decode: one CTA per span, one block, pair stages (40 KB of weights + 2 x n_pad x 128 B of activations per slot)
         assert cps == 1 and nb == 1 and par == 1 and n_pad == -(-M // 16) * 16 and len(sb) - 1 <= 148
         slot = 40960 + 2 * n_pad * 128
@@ -75,8 +76,10 @@ def test_prefill_spans_are_balanced_in_stages(sp, M):
 def test_fewer_sms_and_tiny_shapes(sp):
     sb, info = sp.spense_schedule(128, 128, 0, 8, 0)
     assert info["stages"] == 1 and len(sb) == 2                          # one stage: one span
-    sb, _ = sp.spense_schedule(*QWEN, 64, 1, sms=20)
+    sb, _ = sp.spense_schedule(*QWEN, 32, 1, sms=20)
     assert len(sb) == 21
+    sb, info = sp.spense_schedule(*QWEN, 64, 1, sms=20)                  # sparse-heavy layer above 48 tokens: CTA pairs
+    assert len(sb) == 11 and info["ctas_per_span"] == 2
     sb, info = sp.spense_schedule(*QWEN, 256, 1, sms=20)
     assert info["ctas_per_span"] == 2 and info["blocks_per_launch"] * (len(sb) - 1) <= 10
     with pytest.raises(sp.SpenseError) as e:

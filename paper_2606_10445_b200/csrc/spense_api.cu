@@ -99,20 +99,21 @@ int ring_of(bool wide, int n_pad, int* slot_bytes) {
   return stages > 8 ? 8 : stages;
 }
 
-// how many of `nb` blocks one launch takes: the largest split within 5 % of the best occupancy over all rounds
-// (every round is a launch with its own start-up and fix-up tail, so fewer rounds win a near tie)
+// how many of `nb` blocks one launch takes.  In units of the time one token block needs on all `units` CTA pairs, a launch
+// of c blocks with k = units / c spans each costs c * units / (c * k) (some pairs idle when c does not divide units) plus
+// about one unit of its own: every launch re-streams the weights from HBM, ramps up and ends with a fix-up tail.  The
+// split with the smallest total wins, the larger c on a tie.  (An earlier rule -- the largest c within 5 % of the best
+// occupancy -- picked c = 2 for 35 blocks because c = 1 wastes nothing: M = 8192 ran as 18 launches.)
 int par_of(int nb, int units, int cap) {
-  auto eff = [&](int c) {
+  auto cost = [&](int c) {
     const int rounds = (nb + c - 1) / c, k = units / c;
-    return (double)nb / (rounds * c) * ((double)(c * k) / units);
+    return rounds * ((double)c * units / (c * k) + 1.0);
   };
   int cmax = nb < units ? nb : units;
   if (cmax > cap) cmax = cap;
-  double best = 0;
-  for (int c = 1; c <= cmax; ++c) best = eff(c) > best ? eff(c) : best;
   int pick = 1;
-  for (int c = 1; c <= cmax; ++c)
-    if (eff(c) >= 0.95 * best) pick = c;
+  for (int c = 2; c <= cmax; ++c)
+    if (cost(c) <= cost(pick) + 1e-9) pick = c;
   return pick;
 }
 
@@ -126,7 +127,7 @@ constexpr size_t kActWorkingSetBytes = 64u << 20;
 // M = 96 58.3 vs 63.1, M = 112 62.4 vs 67.7; at M <= 32 the decode kernel wins by 1.2 us), but not for dense-heavy ones (all
 // dense, M = 64: 72.7 vs 70.5): a dense stage gives a CTA of a pair only 16 KB of weights per barrier round trip.
 constexpr int kPairMinTokens = 48;
-Plan plan_of(int M, int sms, int act_row_bytes, bool sparse_heavy) {
+Plan plan_of(int M, int sms, int act_row_bytes, bool sparse_heavy, int mode) {
   Plan pl = {};
   const int decode_max = knob("SPENSE_DECODE_MAX", sparse_heavy ? kPairMinTokens : kDecodeMaxTokens);
   if (M <= decode_max) {
@@ -136,9 +137,11 @@ Plan plan_of(int M, int sms, int act_row_bytes, bool sparse_heavy) {
   } else {
     pl.wide = true;
     pl.nb = M <= kWideMaxTokens1 ? 1 : (M + kWideMaxTokens - 1) / kWideMaxTokens;
+    const int blk_tokens = knob(mode == 1 ? "SPENSE_WIDE_TOKENS_DOWN" : "SPENSE_WIDE_TOKENS_UP", 0);
+    if (blk_tokens > 0) pl.nb = (M + blk_tokens - 1) / blk_tokens;
     pl.n_pad = ((M + pl.nb - 1) / pl.nb + 15) / 16 * 16;
     const int pairs = sms / 2;
-    size_t cap = kActWorkingSetBytes / ((size_t)pl.n_pad * act_row_bytes);
+    size_t cap = ((size_t)knob("SPENSE_ACT_WS_MB", (int)(kActWorkingSetBytes >> 20)) << 20) / ((size_t)pl.n_pad * act_row_bytes);
     cap = cap < 1 ? 1 : (cap > 12 ? 12 : cap);
     pl.par = par_of(pl.nb, pairs, (int)cap);
     pl.spans = pairs / pl.par;
@@ -178,7 +181,7 @@ const Schedule& get_schedule(int mode, const Geometry& g, const Plan& pl) {
   // ~1.12x a 32 KB dense one => fixed part ~36 KB-equivalents; activation bytes come from L2 and weigh less.
   // From three token blocks on (M > 480) a launch is paced by the tensor pipe instead: a sparse stage (K 256) and a
   // dense one (K 128) issue the same four MMAs.
-  const double fixed = 36864.0, gamma = 0.25;
+  const double fixed = knob(pl.wide ? "SPENSE_SCHED_FIXED_WIDE" : "SPENSE_SCHED_FIXED", 36864), gamma = knob("SPENSE_SCHED_GAMMA_PCT", 25) / 100.0;
   const bool tensor_paced = pl.nb > 2;
   const double cs = tensor_paced ? 1.0 : fixed + kSparseStageBytes + gamma * 2.0 * pl.n_pad * 128;
   const double cd = tensor_paced ? 1.0 : fixed + kDenseStageBytes + gamma * 1.0 * pl.n_pad * 128;
@@ -328,7 +331,7 @@ int gate_up_impl(const Launch& L, const spense_shape_t* shape, const void* d_blo
                  const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32, void* d_ws, bool pdl, bool down_follows,
                  cudaStream_t stream, bool dynamic = false, float* d_sh_out = nullptr) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const Plan pl = plan_of(M, L.sms, g.H, 2 * g.I_s >= g.I);
+  const Plan pl = plan_of(M, L.sms, g.H, 2 * g.I_s >= g.I, 0);
   const Schedule& sc = get_schedule(0, g, pl);
   const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + g.gate_up_off;
   CUtensorMap tm, tws, twd;
@@ -356,7 +359,7 @@ int gate_up_impl(const Launch& L, const spense_shape_t* shape, const void* d_blo
     p.amax_part = dynamic ? reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes) : nullptr;
     p.ld_out = g.I; p.out_rows = g.I;
     if (down_follows && blk0 + pl.par >= pl.nb)                // the same layer's down projection streams next
-      fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + g.down_off, get_schedule(1, g, plan_of(M, L.sms, g.I, 2 * g.I_s >= g.I)));
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + g.down_off, get_schedule(1, g, plan_of(M, L.sms, g.I, 2 * g.I_s >= g.I, 1)));
     if (!pl.wide) {
       st = launch_gemm(p, tm, pdl, L.dev, L.sms, stream);
     } else {
@@ -380,7 +383,7 @@ int down_impl(const Launch& L, const spense_shape_t* shape, const void* d_blob, 
               int32_t sh_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, bool pdl, const void* d_next_blob,
               cudaStream_t stream) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const Plan pl = plan_of(M, L.sms, g.I, 2 * g.I_s >= g.I);
+  const Plan pl = plan_of(M, L.sms, g.I, 2 * g.I_s >= g.I, 1);
   const Schedule& sc = get_schedule(1, g, pl);
   const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + g.down_off;
   CUtensorMap tm, tws, twd;
@@ -406,7 +409,7 @@ int down_impl(const Launch& L, const spense_shape_t* shape, const void* d_blob, 
     p.y_dtype = y_dtype;
     p.ld_out = g.H; p.out_rows = g.H;
     if (d_next_blob && blk0 + pl.par >= pl.nb)                 // the next layer's gate/up weights stream next
-      fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + g.gate_up_off, get_schedule(0, g, plan_of(M, L.sms, g.H, 2 * g.I_s >= g.I)));
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + g.gate_up_off, get_schedule(0, g, plan_of(M, L.sms, g.H, 2 * g.I_s >= g.I, 0)));
     if (!pl.wide) {
       st = launch_gemm(p, tm, pdl, L.dev, L.sms, stream);
     } else {
@@ -433,7 +436,7 @@ int linear_impl(const Launch& L, const spense_linear_shape_t* ls, const void* d_
   const bool in_split = ls->split == SPENSE_SPLIT_IN;
   const Geometry g = make_geometry_linear(ls->N, ls->K, ls->n_dense, in_split);
   const int mode = in_split ? 1 : 2;
-  const Plan pl = plan_of(M, L.sms, ls->K, 2 * ls->n_dense <= (in_split ? ls->K : ls->N));
+  const Plan pl = plan_of(M, L.sms, ls->K, 2 * ls->n_dense <= (in_split ? ls->K : ls->N), in_split ? 1 : 0);
   const Schedule& sc = get_schedule(mode, g, pl);
   const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + kBlobHeaderBytes;
   CUtensorMap tm, tws, twd;
@@ -549,7 +552,7 @@ int spense_schedule(const spense_shape_t* shape, int32_t M, int32_t mode, int32_
   if (st) return st;
   if (M < 1 || M > kMaxTokens || (mode != 0 && mode != 1) || sms < 2 || sms > kMaxSpans || !out_span_begin) return SPENSE_ERR_ARG;
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const Plan pl = plan_of(M, sms, mode == 0 ? g.H : g.I, 2 * g.I_s >= g.I);
+  const Plan pl = plan_of(M, sms, mode == 0 ? g.H : g.I, 2 * g.I_s >= g.I, mode);
   const Schedule& sc = get_schedule(mode, g, pl);
   for (int i = 0; i <= sc.n_spans; ++i) out_span_begin[i] = sc.span_begin[i];
   if (out_info) {

@@ -528,8 +528,7 @@ def main():
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": traffic_from_profile(M), "traffic_source": os.path.relpath(TRAFFIC_CSV, ROOT) if M == TRAFFIC_M else None,
                          "peak_source": peak_src,
-                         "kernel": ("spense_gemm_kernel" if info["ctas_per_span"] == 1 else "spense_gemm_wide_kernel") +
-                                   " (gate_up + down launches of one layer)",
+                         "kernel": "spense_gemm_kernel (gate_up + down launches of one layer)",
                          "algorithmic_bytes_per_layer": algo},
             "sustained": sustained,
             "e2e": {"value": ms_e2e * 1e3 / LAYERS / world, "unit": "us/layer", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,

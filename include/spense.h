@@ -131,7 +131,7 @@ int spense_workspace_init(void* d_ws, size_t ws_bytes, spense_stream_t stream);
 
 /* Launch geometry the library uses for (shape, M tokens, mode 0 = gate_up / 1 = down) on a device with `sms` SMs
  * (host only, no device needed): the stream-K schedule cuts the linear sequence of weight stages (the byte order of
- * the blob) into spans of equal cost, one persistent CTA (M <= 112) or CTA pair (M > 112) per span.  Writes
+ * the blob) into spans of equal cost, one persistent CTA pair per span.  Writes
  * n_spans + 1 span boundaries (linear stage indices) into span_begin (room for 161 ints) and returns n_spans, or a
  * negative status.  info (nullable, 6 ints) = {stages, token blocks per launch, token columns per block, ring
  * slots, token blocks, CTAs per span}.  Every CTA of a launch must be resident at the same time: the grid is

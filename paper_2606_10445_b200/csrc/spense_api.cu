@@ -77,23 +77,21 @@ int knob(const char* name, int dflt) { const char* e = std::getenv(name); return
 constexpr int knob(const char*, int dflt) { return dflt; }
 #endif
 
-// ---- launch geometry.
-// Up to kDecodeMaxTokens tokens: the decode kernel, one CTA per stream-K span, token columns = M padded to 16.
-// More: the wide kernel on CTA pairs; token blocks of at most kWideMaxTokens tokens, `par` blocks side by side in one
-// launch with pairs / par spans each (the CTAs of different blocks walk the same schedule, so a weight stage is read from
-// HBM once and found in L2 by the other blocks); more blocks than fit run as further launches.
+// ---- launch geometry.  Every call runs on CTA pairs (spense_gemm.cu): token blocks of at most kWideMaxTokens tokens (one
+// block of kWideMaxTokens1 for 241..256 tokens), `par` blocks side by side in one launch with pairs / par stream-K spans
+// each (the pairs of different blocks walk the same schedule, so a weight stage is read from HBM once and found in L2 by
+// the other blocks); more blocks than fit run as further launches.
 struct Plan {
-  bool wide;
   int n_pad;      // token columns of one block
   int nb;         // token blocks
   int par;        // blocks per launch
-  int spans;      // stream-K spans per block (CTAs, or CTA pairs)
+  int spans;      // stream-K spans per block (CTA pairs)
   int ring;       // stage-ring slots
   int slot_bytes;
 };
 
-int ring_of(bool wide, int n_pad, int* slot_bytes) {
-  const int slot = wide ? kSparseOperandBytes + (n_pad / 2) * 256 : kSparseStageBytes + 2 * n_pad * 128;
+int ring_of(int n_pad, int* slot_bytes) {
+  const int slot = kSparseOperandBytes + (n_pad / 2) * 256;          // one operand (values + metadata) + two half token tiles
   const int stages = (kSmemMax - 1024 - 256 - 20 * n_pad) / slot;   // barriers + the scale tables
   if (slot_bytes) *slot_bytes = slot;
   return stages > 8 ? 8 : stages;
@@ -122,42 +120,28 @@ int par_of(int nb, int units, int cap) {
 // working set (blocks x n_pad x act_row_bytes) well inside the 126 MB L2: measured at M = 8192, 18 blocks of Hq (110 MB)
 // side by side made down HBM-bound on activation re-reads (1020 us against 4 x 167 us at M = 2048).
 constexpr size_t kActWorkingSetBytes = 64u << 20;
-// sparse_heavy: at least half of the intermediate indices are 2:4.  Between kPairMinTokens and kDecodeMaxTokens tokens the
-// CTA-pair kernel is the faster one for such layers (measured on B200, Qwen3-32B shape, p = 25 %: M = 64 55.9 vs 57.0 us/layer,
-// M = 96 58.3 vs 63.1, M = 112 62.4 vs 67.7; at M <= 32 the decode kernel wins by 1.2 us), but not for dense-heavy ones (all
-// dense, M = 64: 72.7 vs 70.5): a dense stage gives a CTA of a pair only 16 KB of weights per barrier round trip.
-constexpr int kPairMinTokens = 48;
-Plan plan_of(int M, int sms, int act_row_bytes, bool sparse_heavy, int mode) {
+Plan plan_of(int M, int sms, int act_row_bytes) {
   Plan pl = {};
-  const int decode_max = knob("SPENSE_DECODE_MAX", sparse_heavy ? kPairMinTokens : kDecodeMaxTokens);
-  if (M <= decode_max) {
-    pl.wide = false;
-    pl.n_pad = (M + 15) / 16 * 16;
-    pl.nb = 1; pl.par = 1; pl.spans = sms;
-  } else {
-    pl.wide = true;
-    pl.nb = M <= kWideMaxTokens1 ? 1 : (M + kWideMaxTokens - 1) / kWideMaxTokens;
-    const int blk_tokens = knob(mode == 1 ? "SPENSE_WIDE_TOKENS_DOWN" : "SPENSE_WIDE_TOKENS_UP", 0);
-    if (blk_tokens > 0) pl.nb = (M + blk_tokens - 1) / blk_tokens;
-    pl.n_pad = ((M + pl.nb - 1) / pl.nb + 15) / 16 * 16;
-    const int pairs = sms / 2;
-    size_t cap = ((size_t)knob("SPENSE_ACT_WS_MB", (int)(kActWorkingSetBytes >> 20)) << 20) / ((size_t)pl.n_pad * act_row_bytes);
-    cap = cap < 1 ? 1 : (cap > 12 ? 12 : cap);
-    pl.par = par_of(pl.nb, pairs, (int)cap);
-    pl.spans = pairs / pl.par;
-  }
-  pl.ring = ring_of(pl.wide, pl.n_pad, &pl.slot_bytes);
+  pl.nb = M <= kWideMaxTokens1 ? 1 : (M + kWideMaxTokens - 1) / kWideMaxTokens;
+  pl.n_pad = ((M + pl.nb - 1) / pl.nb + 15) / 16 * 16;
+  const int pairs = sms / 2;
+  size_t cap = ((size_t)knob("SPENSE_ACT_WS_MB", (int)(kActWorkingSetBytes >> 20)) << 20) / ((size_t)pl.n_pad * act_row_bytes);
+  cap = cap < 1 ? 1 : (cap > 12 ? 12 : cap);
+  pl.par = par_of(pl.nb, pairs, (int)cap);
+  pl.spans = pairs / pl.par;
+  pl.ring = ring_of(pl.n_pad, &pl.slot_bytes);
   return pl;
 }
 
+// token columns whose partials the workspace must hold at up to M tokens (monotone in M: 241..256 tokens run as one block)
 size_t ws_bytes_for(int M) {
-  const size_t cols = M <= kDecodeMaxTokens ? 2 * (size_t)((M + 15) / 16 * 16) : (size_t)kWideMaxTokens1;
+  const size_t cols = M >= kWideMaxTokens1 ? (size_t)kWideMaxTokens1 : (size_t)((M + 15) / 16 * 16);
   return kWsFixedBytes + (size_t)kMaxSpans * 2 * cols * 128 * sizeof(float);
 }
 
 // ---- stream-K schedule: cut the stage sequence into n_spans spans of (nearly) equal cost.
 struct Schedule {
-  int mode, H, I, I_d, n_pad, spans_req, ring, wide, nb;
+  int mode, H, I, I_d, n_pad, spans_req, ring, nb;
   int n_spans;
   int span_begin[kMaxSpans + 1];
   uint32_t span_off[kMaxSpans];   // byte offset of the span's first stage image inside its section
@@ -172,16 +156,16 @@ const Schedule& get_schedule(int mode, const Geometry& g, const Plan& pl) {
   std::lock_guard<std::mutex> lk(g_sched_mu);
   for (const Schedule& s : g_sched)
     if (s.mode == mode && s.H == g.H && s.I == g.I && s.I_d == g.I_d && s.n_pad == pl.n_pad && s.spans_req == pl.spans &&
-        s.ring == pl.ring && s.wide == (int)pl.wide && s.nb == pl.nb)
+        s.ring == pl.ring && s.nb == pl.nb)
       return s;
   Schedule sc = {};
-  sc.mode = mode; sc.H = g.H; sc.I = g.I; sc.I_d = g.I_d; sc.n_pad = pl.n_pad; sc.spans_req = pl.spans; sc.ring = pl.ring; sc.wide = pl.wide; sc.nb = pl.nb;
+  sc.mode = mode; sc.H = g.H; sc.I = g.I; sc.I_d = g.I_d; sc.n_pad = pl.n_pad; sc.spans_req = pl.spans; sc.ring = pl.ring; sc.nb = pl.nb;
   // cost of a stage.  Every CTA keeps the same number of ring slots in flight, so under HBM contention a
   // stage costs one slot latency plus its bytes: measured on B200 (profiles/) a 40 KB sparse stage takes
   // ~1.12x a 32 KB dense one => fixed part ~36 KB-equivalents; activation bytes come from L2 and weigh less.
   // From three token blocks on (M > 480) a launch is paced by the tensor pipe instead: a sparse stage (K 256) and a
   // dense one (K 128) issue the same four MMAs.
-  const double fixed = knob(pl.wide ? "SPENSE_SCHED_FIXED_WIDE" : "SPENSE_SCHED_FIXED", 36864), gamma = knob("SPENSE_SCHED_GAMMA_PCT", 25) / 100.0;
+  const double fixed = knob("SPENSE_SCHED_FIXED", 36864), gamma = knob("SPENSE_SCHED_GAMMA_PCT", 25) / 100.0;
   const bool tensor_paced = pl.nb > 2;
   const double cs = tensor_paced ? 1.0 : fixed + kSparseStageBytes + gamma * 2.0 * pl.n_pad * 128;
   const double cd = tensor_paced ? 1.0 : fixed + kDenseStageBytes + gamma * 1.0 * pl.n_pad * 128;
@@ -264,9 +248,8 @@ int make_tmap_section(CUtensorMap* map, const uint8_t* base, size_t bytes, int b
 }
 
 // bytes of span k that the PREVIOUS launch pulls into L2 during its tail: at least one ring
-constexpr uint32_t kPfNextBytes = 640u * 1024u, kPfSelfBytes = 160u * 1024u;
+constexpr uint32_t kPfNextBytes = 640u * 1024u;
 constexpr int kPfPaceNs = 750;
-constexpr int kPfAheadStages = 12;   // wide kernel: L2 prefetch distance of the producer, in stages
 uint32_t next_prefetch_bytes(const Schedule& sc, int k) {
   const uint32_t want = (uint32_t)knob("SPENSE_PF_NEXT_KB", kPfNextBytes / 1024) * 1024u;
   uint32_t n = sc.span_pre[k] > want ? sc.span_pre[k] : want;
@@ -284,28 +267,14 @@ void fill_common(GemmParams& p, const Schedule& sc, const Plan& pl, const spense
   p.status = g_status;
   p.n_spans = sc.n_spans;
   std::memcpy(p.span_begin, sc.span_begin, sizeof(int) * (sc.n_spans + 1));
-  if (!pl.wide) {
-    for (int i = 0; i < sc.n_spans; ++i) {                    // own stages pulled into L2 while waiting for the previous kernel
-      const uint32_t from = next_prefetch_bytes(sc, i);
-      const uint32_t left = sc.span_len[i] - from;
-      p.self_off[i] = from - sc.span_pre[i];
-      p.self_len[i] = kPfSelfBytes < left ? kPfSelfBytes : left;
-    }
-  }
   p.nb = 1;
   p.blk0 = 0;
   p.M = M;
   p.n_pad = pl.n_pad;
   p.slot_bytes = pl.slot_bytes;
   p.num_stages = pl.ring;
-  if (pl.wide) {
-    p.acc_stride = pl.n_pad > kWideMaxTokens ? kWideMaxTokens1 : kWideMaxTokens;   // 2 buffers x 240 columns (or 1 x 256), metadata at 480
-    p.num_acc_bufs = pl.n_pad > kWideMaxTokens ? 1 : 2;
-    p.pf_ahead = kPfAheadStages;
-  } else {
-    p.acc_stride = pl.n_pad <= 32 ? 32 : (pl.n_pad <= 64 ? 64 : (pl.n_pad <= 96 ? 96 : 112));
-    p.num_acc_bufs = 2;                                       // 2 buffers x 2 accumulators x 112 columns = 448, metadata at 480
-  }
+  p.acc_stride = pl.n_pad > kWideMaxTokens ? kWideMaxTokens1 : kWideMaxTokens;   // 2 buffers x 240 columns (or 1 x 256), metadata at 480
+  p.num_acc_bufs = pl.n_pad > kWideMaxTokens ? 1 : 2;
   uint8_t* ws = reinterpret_cast<uint8_t*>(d_ws);
   p.ws_ctrl = reinterpret_cast<int*>(ws);
   p.flags = reinterpret_cast<int*>(ws + 128);
@@ -331,17 +300,14 @@ int gate_up_impl(const Launch& L, const spense_shape_t* shape, const void* d_blo
                  const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32, void* d_ws, bool pdl, bool down_follows,
                  cudaStream_t stream, bool dynamic = false, float* d_sh_out = nullptr) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const Plan pl = plan_of(M, L.sms, g.H, 2 * g.I_s >= g.I, 0);
+  const Plan pl = plan_of(M, L.sms, g.H);
   const Schedule& sc = get_schedule(0, g, pl);
   const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + g.gate_up_off;
   CUtensorMap tm, tws, twd;
-  int st = make_tmap(&tm, d_x, g.H, M, pl.wide ? pl.n_pad / 2 : pl.n_pad);
+  int st = make_tmap(&tm, d_x, g.H, M, pl.n_pad / 2);
+  if (!st) st = make_tmap_section(&tws, section, g.down_off - g.gate_up_off, kSparseOperandBytes / 128);
+  if (!st) st = make_tmap_section(&twd, section, g.down_off - g.gate_up_off, kOperandBytes / 128);
   if (st) return st;
-  if (pl.wide) {
-    st = make_tmap_section(&tws, section, g.down_off - g.gate_up_off, kSparseOperandBytes / 128);
-    if (!st) st = make_tmap_section(&twd, section, g.down_off - g.gate_up_off, kOperandBytes / 128);
-    if (st) return st;
-  }
   for (int blk0 = 0; blk0 < pl.nb; blk0 += pl.par) {
     GemmParams p = {};
     fill_common(p, sc, pl, shape, d_blob, M, d_ws);
@@ -359,18 +325,14 @@ int gate_up_impl(const Launch& L, const spense_shape_t* shape, const void* d_blo
     p.amax_part = dynamic ? reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes) : nullptr;
     p.ld_out = g.I; p.out_rows = g.I;
     if (down_follows && blk0 + pl.par >= pl.nb)                // the same layer's down projection streams next
-      fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + g.down_off, get_schedule(1, g, plan_of(M, L.sms, g.I, 2 * g.I_s >= g.I, 1)));
-    if (!pl.wide) {
-      st = launch_gemm(p, tm, pdl, L.dev, L.sms, stream);
-    } else {
-      st = launch_gemm_wide(p, tm, tws, twd, pdl, L.dev, L.sms, stream);
-    }
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + g.down_off, get_schedule(1, g, plan_of(M, L.sms, g.I)));
+    st = launch_gemm(p, tm, tws, twd, pdl, L.dev, stream);
     if (st) return st;
     if (dynamic) {
       // rows of this launch: s_h = max over the block's slots / 448, Hq = E4M3(h / s_h)
       const int m0 = blk0 * pl.n_pad;
       const int rows = (M - m0) < p.nb * pl.n_pad ? (M - m0) : p.nb * pl.n_pad;
-      const int slots_per_block = pl.wide ? 2 * sc.n_spans : sc.n_spans;
+      const int slots_per_block = 2 * sc.n_spans;
       st = launch_requant_rows(d_h_f32 + (size_t)m0 * g.I, rows, g.I, p.amax_part, slots_per_block, pl.n_pad, pl.n_pad,
                                d_hq + (size_t)m0 * g.I, d_sh_out + m0, stream);
       if (st) return st;
@@ -383,17 +345,14 @@ int down_impl(const Launch& L, const spense_shape_t* shape, const void* d_blob, 
               int32_t sh_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, bool pdl, const void* d_next_blob,
               cudaStream_t stream) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const Plan pl = plan_of(M, L.sms, g.I, 2 * g.I_s >= g.I, 1);
+  const Plan pl = plan_of(M, L.sms, g.I);
   const Schedule& sc = get_schedule(1, g, pl);
   const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + g.down_off;
   CUtensorMap tm, tws, twd;
-  int st = make_tmap(&tm, d_hq, g.I, M, pl.wide ? pl.n_pad / 2 : pl.n_pad);
+  int st = make_tmap(&tm, d_hq, g.I, M, pl.n_pad / 2);
+  if (!st) st = make_tmap_section(&tws, section, g.total_bytes - g.down_off, kSparseOperandBytes / 128);
+  if (!st) st = make_tmap_section(&twd, section, g.total_bytes - g.down_off, kOperandBytes / 128);
   if (st) return st;
-  if (pl.wide) {
-    st = make_tmap_section(&tws, section, g.total_bytes - g.down_off, kSparseOperandBytes / 128);
-    if (!st) st = make_tmap_section(&twd, section, g.total_bytes - g.down_off, kOperandBytes / 128);
-    if (st) return st;
-  }
   for (int blk0 = 0; blk0 < pl.nb; blk0 += pl.par) {
     GemmParams p = {};
     fill_common(p, sc, pl, shape, d_blob, M, d_ws);
@@ -409,12 +368,8 @@ int down_impl(const Launch& L, const spense_shape_t* shape, const void* d_blob, 
     p.y_dtype = y_dtype;
     p.ld_out = g.H; p.out_rows = g.H;
     if (d_next_blob && blk0 + pl.par >= pl.nb)                 // the next layer's gate/up weights stream next
-      fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + g.gate_up_off, get_schedule(0, g, plan_of(M, L.sms, g.H, 2 * g.I_s >= g.I, 0)));
-    if (!pl.wide) {
-      st = launch_gemm(p, tm, pdl, L.dev, L.sms, stream);
-    } else {
-      st = launch_gemm_wide(p, tm, tws, twd, pdl, L.dev, L.sms, stream);
-    }
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + g.gate_up_off, get_schedule(0, g, plan_of(M, L.sms, g.H)));
+    st = launch_gemm(p, tm, tws, twd, pdl, L.dev, stream);
     if (st) return st;
   }
   return SPENSE_OK;
@@ -436,17 +391,14 @@ int linear_impl(const Launch& L, const spense_linear_shape_t* ls, const void* d_
   const bool in_split = ls->split == SPENSE_SPLIT_IN;
   const Geometry g = make_geometry_linear(ls->N, ls->K, ls->n_dense, in_split);
   const int mode = in_split ? 1 : 2;
-  const Plan pl = plan_of(M, L.sms, ls->K, 2 * ls->n_dense <= (in_split ? ls->K : ls->N), in_split ? 1 : 0);
+  const Plan pl = plan_of(M, L.sms, ls->K);
   const Schedule& sc = get_schedule(mode, g, pl);
   const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + kBlobHeaderBytes;
   CUtensorMap tm, tws, twd;
-  int st = make_tmap(&tm, d_x, ls->K, M, pl.wide ? pl.n_pad / 2 : pl.n_pad);
+  int st = make_tmap(&tm, d_x, ls->K, M, pl.n_pad / 2);
+  if (!st) st = make_tmap_section(&tws, section, g.total_bytes - kBlobHeaderBytes, kSparseOperandBytes / 128);
+  if (!st) st = make_tmap_section(&twd, section, g.total_bytes - kBlobHeaderBytes, kOperandBytes / 128);
   if (st) return st;
-  if (pl.wide) {
-    st = make_tmap_section(&tws, section, g.total_bytes - kBlobHeaderBytes, kSparseOperandBytes / 128);
-    if (!st) st = make_tmap_section(&twd, section, g.total_bytes - kBlobHeaderBytes, kOperandBytes / 128);
-    if (st) return st;
-  }
   const spense_shape_t hdr_shape = {g.H, g.I, g.I_d};          // what the header of this blob states
   for (int blk0 = 0; blk0 < pl.nb; blk0 += pl.par) {
     GemmParams p = {};
@@ -468,7 +420,7 @@ int linear_impl(const Launch& L, const spense_linear_shape_t* ls, const void* d_
     p.y = d_y;
     p.y_dtype = y_dtype;
     p.ld_out = ls->N; p.out_rows = ls->N;
-    st = pl.wide ? launch_gemm_wide(p, tm, tws, twd, false, L.dev, L.sms, stream) : launch_gemm(p, tm, false, L.dev, L.sms, stream);
+    st = launch_gemm(p, tm, tws, twd, false, L.dev, stream);
     if (st) return st;
   }
   return SPENSE_OK;
@@ -552,7 +504,7 @@ int spense_schedule(const spense_shape_t* shape, int32_t M, int32_t mode, int32_
   if (st) return st;
   if (M < 1 || M > kMaxTokens || (mode != 0 && mode != 1) || sms < 2 || sms > kMaxSpans || !out_span_begin) return SPENSE_ERR_ARG;
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const Plan pl = plan_of(M, sms, mode == 0 ? g.H : g.I, 2 * g.I_s >= g.I, mode);
+  const Plan pl = plan_of(M, sms, mode == 0 ? g.H : g.I);
   const Schedule& sc = get_schedule(mode, g, pl);
   for (int i = 0; i <= sc.n_spans; ++i) out_span_begin[i] = sc.span_begin[i];
   if (out_info) {
@@ -561,7 +513,7 @@ int spense_schedule(const spense_shape_t* shape, int32_t M, int32_t mode, int32_
     out_info[2] = pl.n_pad;
     out_info[3] = pl.ring;
     out_info[4] = pl.nb;
-    out_info[5] = pl.wide ? 2 : 1;
+    out_info[5] = 2;
   }
   return sc.n_spans;
 }

@@ -1,6 +1,5 @@
-// Device code shared by the two Spense GEMM kernels (spense_gemm.cu: decode, one CTA per span; spense_gemm_wide.cu:
-// wide token tiles on CTA pairs): the walk over the linear stage sequence, the element-wise epilogue (scales -> SiLU*up ->
-// E4M3, Eq. 4) and the bounded waits.  Nothing here is shared with oracle/.
+// Device helpers of the Spense GEMM kernel (spense_gemm.cu): the walk over the linear stage sequence, the element-wise
+// epilogue (scales -> SiLU*up -> E4M3, Eq. 4) and the bounded waits.  Nothing here is shared with oracle/.
 #pragma once
 
 #include <cuda_bf16.h>

@@ -21,7 +21,7 @@ namespace spense {
 //       down    : rows [256t, 256t+128) and [256t+128, 256t+256) of W_down (sparse K range, then dense)
 //   sparse stage (K = 256 logical): A0 vals 16 KB | A0 meta 4 KB | A1 vals 16 KB | A1 meta 4 KB
 //   dense  stage (K = 128)        : A0 16 KB | A1 16 KB
-//   (operand-major, so that the CTA pair of the wide-token kernel loads one operand each: 20 KB / 16 KB contiguous)
+//   (operand-major, so that each CTA of a pair loads one operand: 20 KB / 16 KB contiguous)
 //   vals / dense images: 128 rows x 128 B, canonical K-major SWIZZLE_128B (8-row x 128 B atoms,
 //       16-byte chunk index XOR (row & 7)).  meta image: 2 atoms of 128 rows x 16 B, row-major
 //       (one atom = K 128 logical = what one tcgen05.cp.128x128b moves to TMEM).
@@ -29,7 +29,7 @@ namespace spense {
 //       128 t + 64 a + [0, 64): operand row 32 q + i = gate row of index 16 q + i, operand row 32 q + 16 + i = up row of
 //       the same index (q < 4, i < 16).  g and u of one index then sit in the two 16-lane halves of ONE TMEM lane
 //       quadrant of ONE accumulator, so a warp reads both with two tcgen05.ld.16x256b and every operand is a
-//       self-contained GLU tile (what lets the wide-token kernel give each CTA of a pair one operand).
+//       self-contained GLU tile (what lets the kernel give each CTA of a pair one operand).
 // ------------------------------------------------------------------------------------------
 constexpr int kTileRows = 128;
 constexpr int kSparseStageK = 256;           // logical K per sparse stage
@@ -45,8 +45,7 @@ constexpr int kBlobVersion = 2;
 constexpr int kMaxSpans = 160;               // fix-up slots of a launch (one per CTA)
 constexpr int kMaxTokens = 1 << 20;           // tokens per call (the activation tensor map is built over all of them)
 constexpr int kSmemMax = 232448;             // opt-in dynamic shared memory per CTA
-constexpr int kDecodeMaxTokens = 112;        // up to here: one CTA per span, pair stages, two accumulator buffers (4 x 112 TMEM columns)
-constexpr int kWideMaxTokens = 240;          // token columns of one CTA pair of the wide kernel (2 buffers x 240 + 16 metadata columns)
+constexpr int kWideMaxTokens = 240;          // token columns of one CTA pair (2 accumulator buffers x 240 + 16 metadata columns of TMEM)
 constexpr int kWideMaxTokens1 = 256;         // 241..256 tokens: ONE block of 256 columns with a single accumulator buffer (the largest MMA-N), so
                                              // the weights cross the L2 -> SM path once instead of once per 128-token block
 constexpr int kFlagBytes = 4096;             // control words (128 B) + 2 flags per slot
@@ -162,15 +161,12 @@ struct GemmParams {
   float* partials;          // workspace: 2 partial tiles per slot
   int* status;              // mapped pinned host word: first device-side error (bad blob header, a peer CTA never showed up)
   int pf_pace_ns;           // next-kernel L2 prefetch: nanoseconds per 32 KB chunk (0 = all at once)
-  int pf_ahead;             // wide kernel: stages the producer's L2 prefetch runs ahead of its copies (0 = off)
   long long* trace;         // debug timeline (16 slots per span; SPENSE_DEBUG_HOOKS builds) or nullptr
   int dbg;                  // debug experiments (SPENSE_DEBUG_HOOKS builds; 0 in production)
   const uint8_t* next_base; // section the NEXT kernel of the stream will stream (L2 prefetch during our tail) or nullptr
   int span_begin[kMaxSpans + 1];
   uint32_t next_off[kMaxSpans];   // byte offset of span i's first stage in next_base ...
   uint32_t next_len[kMaxSpans];   // ... and how many bytes of it to prefetch
-  uint32_t self_off[kMaxSpans];   // own span: bytes past the ring prefill where the L2 self-prefetch starts ...
-  uint32_t self_len[kMaxSpans];   // ... and its length (issued while waiting for the previous kernel)
 };
 
 // ------------------------------------------------------------------------------------------
@@ -396,9 +392,8 @@ int launch_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8
                 int64_t* h_err_where, cudaStream_t stream);
 int launch_pack_linear(const spense_linear_shape_t* shape, const uint8_t* d_w, float w_scale, const int32_t* d_perm, void* d_blob,
                        const spense_linear_canon_t* canon, void* d_ws, int64_t* h_err_where, cudaStream_t stream);
-int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, bool pdl, int dev, int sms, cudaStream_t stream);
-int launch_gemm_wide(const GemmParams& p, const CUtensorMap& tmap_b, const CUtensorMap& tmap_ws, const CUtensorMap& tmap_wd,
-                     bool pdl, int dev, int sms, cudaStream_t stream);
+int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, const CUtensorMap& tmap_ws, const CUtensorMap& tmap_wd, bool pdl, int dev,
+                cudaStream_t stream);
 int launch_requant_rows(const float* d_h, int rows, int cols, const float* d_amax_part, int n_part, int part_stride,
                         int block_rows, uint8_t* d_hq, float* d_sh, cudaStream_t stream);
 int launch_select(const spense_shape_t* shape, const float* d_wgate, const float* d_wup, const float* d_wdown,

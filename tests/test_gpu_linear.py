@@ -26,7 +26,7 @@ def _split_id(sp, split):
 
 
 # N, K, p, split, M: several tiles and spans, ragged K (K % 256 == 128), a dense half tile, both degenerate splits,
-# the decode kernel (M <= 112) and the wide kernel on CTA pairs (M > 112, one and several token blocks)
+# one token block (down to 16 token columns) and several side by side
 LINEAR_CASES = [
     (1024, 256, 0.25, "out", 8),
     (1024, 256, 0.25, "in", 8),

@@ -248,8 +248,8 @@ int make_tmap_section(CUtensorMap* map, const uint8_t* base, size_t bytes, int b
 }
 
 // bytes of span k that the PREVIOUS launch pulls into L2 during its tail: at least one ring
-constexpr uint32_t kPfNextBytes = 640u * 1024u;
-constexpr int kPfPaceNs = 750;
+constexpr uint32_t kPfNextBytes = 1280u * 1024u;   // B200 sweep (M = 64, us/layer): 160 KB 54.2, 640 KB 53.6, 1280 KB 52.6, 2560 KB 53.0
+constexpr int kPfPaceNs = 1500;                    // per 32 KB chunk and CTA; 300 ns: 56.0, 750: 52.7, 1500: 52.5
 uint32_t next_prefetch_bytes(const Schedule& sc, int k) {
   const uint32_t want = (uint32_t)knob("SPENSE_PF_NEXT_KB", kPfNextBytes / 1024) * 1024u;
   uint32_t n = sc.span_pre[k] > want ? sc.span_pre[k] : want;

@@ -120,9 +120,13 @@ int par_of(int nb, int units, int cap) {
 // working set (blocks x n_pad x act_row_bytes) well inside the 126 MB L2: measured at M = 8192, 18 blocks of Hq (110 MB)
 // side by side made down HBM-bound on activation re-reads (1020 us against 4 x 167 us at M = 2048).
 constexpr size_t kActWorkingSetBytes = 64u << 20;
-Plan plan_of(int M, int sms, int act_row_bytes) {
+Plan plan_of(int M, int sms, int act_row_bytes, bool in_split) {
   Plan pl = {};
   pl.nb = M <= kWideMaxTokens1 ? 1 : (M + kWideMaxTokens - 1) / kWideMaxTokens;
+  // input-split walks (down): two blocks side by side leave 37 spans over the row tiles, every tile then splits three ways
+  // and ends in the reduce-scatter with large partials; three blocks (24 spans) split two ways, which the TMEM preload
+  // handles (measured: M = 300 down 67 -> 59 us, M = 480 82 -> 66 us; gate_up prefers the larger blocks: 62.6 vs 81.3 us)
+  if (in_split && pl.nb == 2) pl.nb = 3;
   pl.n_pad = ((M + pl.nb - 1) / pl.nb + 15) / 16 * 16;
   const int pairs = sms / 2;
   size_t cap = ((size_t)knob("SPENSE_ACT_WS_MB", (int)(kActWorkingSetBytes >> 20)) << 20) / ((size_t)pl.n_pad * act_row_bytes);
@@ -300,7 +304,7 @@ int gate_up_impl(const Launch& L, const spense_shape_t* shape, const void* d_blo
                  const float* d_sh, int32_t sh_stride, uint8_t* d_hq, float* d_h_f32, void* d_ws, bool pdl, bool down_follows,
                  cudaStream_t stream, bool dynamic = false, float* d_sh_out = nullptr) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const Plan pl = plan_of(M, L.sms, g.H);
+  const Plan pl = plan_of(M, L.sms, g.H, false);
   const Schedule& sc = get_schedule(0, g, pl);
   const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + g.gate_up_off;
   CUtensorMap tm, tws, twd;
@@ -325,7 +329,7 @@ int gate_up_impl(const Launch& L, const spense_shape_t* shape, const void* d_blo
     p.amax_part = dynamic ? reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(d_ws) + kFlagBytes) : nullptr;
     p.ld_out = g.I; p.out_rows = g.I;
     if (down_follows && blk0 + pl.par >= pl.nb)                // the same layer's down projection streams next
-      fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + g.down_off, get_schedule(1, g, plan_of(M, L.sms, g.I)));
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_blob) + g.down_off, get_schedule(1, g, plan_of(M, L.sms, g.I, true)));
     st = launch_gemm(p, tm, tws, twd, pdl, L.dev, stream);
     if (st) return st;
     if (dynamic) {
@@ -345,7 +349,7 @@ int down_impl(const Launch& L, const spense_shape_t* shape, const void* d_blob, 
               int32_t sh_stride, int32_t M, void* d_y, int32_t y_dtype, void* d_ws, bool pdl, const void* d_next_blob,
               cudaStream_t stream) {
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const Plan pl = plan_of(M, L.sms, g.I);
+  const Plan pl = plan_of(M, L.sms, g.I, true);
   const Schedule& sc = get_schedule(1, g, pl);
   const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + g.down_off;
   CUtensorMap tm, tws, twd;
@@ -368,7 +372,7 @@ int down_impl(const Launch& L, const spense_shape_t* shape, const void* d_blob, 
     p.y_dtype = y_dtype;
     p.ld_out = g.H; p.out_rows = g.H;
     if (d_next_blob && blk0 + pl.par >= pl.nb)                 // the next layer's gate/up weights stream next
-      fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + g.gate_up_off, get_schedule(0, g, plan_of(M, L.sms, g.H)));
+      fill_next(p, reinterpret_cast<const uint8_t*>(d_next_blob) + g.gate_up_off, get_schedule(0, g, plan_of(M, L.sms, g.H, false)));
     st = launch_gemm(p, tm, tws, twd, pdl, L.dev, stream);
     if (st) return st;
   }
@@ -391,7 +395,7 @@ int linear_impl(const Launch& L, const spense_linear_shape_t* ls, const void* d_
   const bool in_split = ls->split == SPENSE_SPLIT_IN;
   const Geometry g = make_geometry_linear(ls->N, ls->K, ls->n_dense, in_split);
   const int mode = in_split ? 1 : 2;
-  const Plan pl = plan_of(M, L.sms, ls->K);
+  const Plan pl = plan_of(M, L.sms, ls->K, in_split);
   const Schedule& sc = get_schedule(mode, g, pl);
   const uint8_t* section = reinterpret_cast<const uint8_t*>(d_blob) + kBlobHeaderBytes;
   CUtensorMap tm, tws, twd;
@@ -504,7 +508,7 @@ int spense_schedule(const spense_shape_t* shape, int32_t M, int32_t mode, int32_
   if (st) return st;
   if (M < 1 || M > kMaxTokens || (mode != 0 && mode != 1) || sms < 2 || sms > kMaxSpans || !out_span_begin) return SPENSE_ERR_ARG;
   const Geometry g = make_geometry(shape->H, shape->I, shape->I_dense);
-  const Plan pl = plan_of(M, sms, mode == 0 ? g.H : g.I);
+  const Plan pl = plan_of(M, sms, mode == 0 ? g.H : g.I, mode == 1);
   const Schedule& sc = get_schedule(mode, g, pl);
   for (int i = 0; i <= sc.n_spans; ++i) out_span_begin[i] = sc.span_begin[i];
   if (out_info) {

@@ -38,7 +38,7 @@ def test_spans_partition_the_stage_sequence(sp, shape, M, mode):
     assert n_pad % 16 == 0 and nb * n_pad >= M > (nb - 1) * n_pad                         # the blocks cover the tokens, none is empty
     # CTA pairs: one block of at most 256 tokens (241..256: one 256-column tile with a single accumulator buffer), else
     # blocks of at most 240 tokens, `par` blocks side by side with 74 // par spans each
-    assert cps == 2 and n_pad <= (256 if M <= 256 else 240) and nb == (1 if M <= 256 else -(-M // 240)) and 1 <= par <= min(nb, 37)
+    assert cps == 2 and n_pad <= (256 if M <= 256 else 240) and nb == (1 if M <= 256 else max(-(-M // 240), 3 if mode == 1 else 2)) and 1 <= par <= min(nb, 37)
     if nb == 1:
         assert n_pad == -(-M // 16) * 16
     assert len(sb) - 1 <= 74 // par
@@ -67,6 +67,17 @@ def test_prefill_spans_are_balanced_in_stages(sp, M):
         sb, info = sp.spense_schedule(*QWEN, M, mode)
         n = np.diff(np.array(sb))
         assert n.max() - n.min() <= 1
+
+
+def test_many_blocks_run_as_few_launches(sp):
+    # 35 token blocks (M = 8192): every launch streams all weights again, so the plan takes as many blocks per launch as
+    # the activation working set allows instead of the split that merely wastes no CTA pair (one or two blocks)
+    _, info = sp.spense_schedule(*QWEN, 8192, 0)
+    assert info["blocks"] == 35 and info["blocks_per_launch"] == 12
+    _, info = sp.spense_schedule(*QWEN, 8192, 1)
+    assert info["blocks"] == 35 and info["blocks_per_launch"] == 9           # 9 x 240 x 25600 B of Hq stay below 64 MB
+    _, info = sp.spense_schedule(*QWEN, 2048, 0)
+    assert info["blocks"] == 9 and info["blocks_per_launch"] == 9
 
 
 def test_fewer_sms_and_tiny_shapes(sp):

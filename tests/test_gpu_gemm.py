@@ -87,6 +87,39 @@ def test_gate_up_down_mlp_parity(sp, H, I, p, I_d, M):
     assert int(ctrl[0]) > 0 and int(ctrl[1]) == 0
 
 
+def _random_cases(n, seed):
+    """seeded random shapes: H, I multiples of 128, any dense count (multiple of 128), any token count up to 300 -- spans of a
+    single stage, tiles shared by three and more spans, half tiles, every token-column padding"""
+    rng = np.random.default_rng(seed)
+    out = []
+    for _ in range(n):
+        H = 128 * int(rng.integers(1, 9))
+        I = 128 * int(rng.integers(1, 17))
+        I_d = 128 * int(rng.integers(0, I // 128 + 1))
+        M = int(rng.choice([1, 2, 7, 15, 16, 17, 31, 33, 63, 65, 97, 113, 129, 191, 239, 241, 255, 257, 299]))
+        out.append((H, I, I_d, M))
+    return out
+
+
+@pytest.mark.parametrize("H,I,I_d,M", _random_cases(24, seed=20261105))
+def test_random_shapes_parity(sp, H, I, I_d, M):
+    c = Case(H, I, 0.0, M, seed=4000 + H + 3 * I + 7 * I_d + M, I_dense=I_d)
+    pk = c.pack_gpu(sp)
+    s_h = c.default_s_h()
+    r = c.oracle_gate_up(s_h)
+    ws = sp.spense_workspace(pk, M)
+    h_gpu, hq_gpu = run_gate_up(sp, c, pk, s_h, ws)
+    frac = assert_gate_up_parity(r, h_gpu, hq_gpu, s_h, f"random {H}x{I} I_d={I_d} M={M}")
+    assert frac < max(HQ_MISMATCH_BOUND, 2.0 / hq_gpu.size), frac      # tiny cases: one byte is already more than 1e-4
+    sh_dev = cuda(torch.from_numpy(s_h))
+    y = sp.spense_down(pk, cuda(torch.from_numpy(hq_gpu)), sh_dev, ws)
+    y2 = sp.spense_mlp(pk, cuda(c.x), cuda(c.s_x), sh_dev, ws)
+    torch.cuda.synchronize()
+    assert_down_parity(y.cpu().numpy(), hq_gpu, s_h, c.wd, c.L.w_scale[2], "down")
+    assert torch.equal(y, y2)
+    assert sp.spense_device_status() == "SPENSE_OK"
+
+
 def test_scalar_requant_scale(sp):
     c = Case(256, 1024, 0.25, 8, seed=77)
     pk = c.pack_gpu(sp)

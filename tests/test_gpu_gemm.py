@@ -120,6 +120,32 @@ def test_random_shapes_parity(sp, H, I, I_d, M):
     assert sp.spense_device_status() == "SPENSE_OK"
 
 
+def test_changing_token_counts_on_one_workspace(sp):
+    """300 back-to-back layers on ONE workspace with the token count changing every call (every launch geometry: one block,
+    the single-buffer tile, several blocks, static and dynamic requant): the epoch-valued flags need no reset in between,
+    no launch times out, and a token count seen again gives the same bits."""
+    c = Case(640, 896, 0.43, 8, seed=123)
+    pk = c.pack_gpu(sp)
+    ws = sp.spense_workspace(pk, 1024)
+    rng = np.random.default_rng(7)
+    seen = {}
+    for it in range(300):
+        M = int(rng.choice([1, 5, 16, 48, 64, 100, 128, 200, 240, 250, 256, 300, 481, 700]))
+        x, s_x = si.make_activations(M, 640, seed=M)
+        sh = torch.full((M,), 0.05, device="cuda")
+        if it % 3 == 2:
+            y, _, _, _ = sp.spense_mlp_dyn(pk, cuda(x), cuda(s_x), ws)
+            key = ("dyn", M)
+        else:
+            y = sp.spense_mlp(pk, cuda(x), cuda(s_x), sh, ws, next_layer=pk)
+            key = ("static", M)
+        if key in seen:
+            assert torch.equal(seen[key], y), key
+        seen[key] = y
+    torch.cuda.synchronize()
+    assert sp.spense_device_status() == "SPENSE_OK"
+
+
 def test_scalar_requant_scale(sp):
     c = Case(256, 1024, 0.25, 8, seed=77)
     pk = c.pack_gpu(sp)

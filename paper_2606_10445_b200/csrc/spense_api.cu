@@ -338,7 +338,7 @@ int gate_up_impl(const Launch& L, const spense_shape_t* shape, const void* d_blo
       const int rows = (M - m0) < p.nb * pl.n_pad ? (M - m0) : p.nb * pl.n_pad;
       const int slots_per_block = 2 * sc.n_spans;
       st = launch_requant_rows(d_h_f32 + (size_t)m0 * g.I, rows, g.I, p.amax_part, slots_per_block, pl.n_pad, pl.n_pad,
-                               d_hq + (size_t)m0 * g.I, d_sh_out + m0, stream);
+                               d_hq + (size_t)m0 * g.I, d_sh_out + m0, L.sms, stream);
       if (st) return st;
     }
   }

@@ -395,7 +395,7 @@ int launch_pack_linear(const spense_linear_shape_t* shape, const uint8_t* d_w, f
 int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, const CUtensorMap& tmap_ws, const CUtensorMap& tmap_wd, bool pdl, int dev,
                 cudaStream_t stream);
 int launch_requant_rows(const float* d_h, int rows, int cols, const float* d_amax_part, int n_part, int part_stride,
-                        int block_rows, uint8_t* d_hq, float* d_sh, cudaStream_t stream);
+                        int block_rows, uint8_t* d_hq, float* d_sh, int sms, cudaStream_t stream);
 int launch_select(const spense_shape_t* shape, const float* d_wgate, const float* d_wup, const float* d_wdown,
                   const float* d_hdiag_x, const float* d_hdiag_h, float eps, float* d_score, int32_t* d_dense_idx,
                   int32_t* d_perm, void* d_ws, cudaStream_t stream);

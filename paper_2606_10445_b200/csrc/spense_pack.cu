@@ -300,12 +300,14 @@ __global__ void quantize_kernel(const float* __restrict__ in, int64_t cols, cons
 // Hq[m,j] = E4M3_rne_sat(h[m,j] / s_h[m]).  The row maximum comes from the per-CTA maxima gate_up left in amax_part:
 // row m belongs to token block m / block_rows whose CTAs own the slots [blk * n_part, (blk + 1) * n_part), each
 // [part_stride] floats indexed by the token column m % block_rows (no atomics, nothing to reset).
-// grid = (column chunks of 4096, rows).
-__global__ void __launch_bounds__(256) requant_rows_kernel(const float* __restrict__ h, int cols, const float* __restrict__ amax_part,
+// grid = (column chunks of chunk_cols, rows), about two 256-thread CTAs per SM (launch_requant_rows): the kernel sits on the
+// critical path between gate_up and down, few rows must still fill the machine, and many small CTAs per SM keep the
+// next kernel's CTAs (which want to fill their weight rings meanwhile) out of the register file for longer.
+__global__ void __launch_bounds__(256) requant_rows_kernel(const float* __restrict__ h, int cols, int chunk_cols, const float* __restrict__ amax_part,
                                                            int n_part, int part_stride, int block_rows, uint8_t* __restrict__ hq,
                                                            float* __restrict__ s_h) {
-  asm volatile("griddepcontrol.wait;" ::: "memory");            // h and amax_part come from the previous kernel
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // down may become resident and stream its weights now
+  asm volatile("griddepcontrol.wait;" ::: "memory");                // h and amax_part come from the previous kernel
   const int row = blockIdx.y;
   const int blk = row / block_rows, col = row - blk * block_rows;
   const float* part = amax_part + (size_t)blk * n_part * part_stride + col;
@@ -314,25 +316,44 @@ __global__ void __launch_bounds__(256) requant_rows_kernel(const float* __restri
   m = block_max(m);
   const float s = m > 0.0f ? __fdiv_rn(m, 448.0f) : 1.0f;
   if (blockIdx.x == 0 && threadIdx.x == 0) s_h[row] = s;
-  const int c0 = blockIdx.x * 4096;
+  const int c0 = blockIdx.x * chunk_cols;
   const float4* src = reinterpret_cast<const float4*>(h + (size_t)row * cols + c0);
   uint32_t* dst = reinterpret_cast<uint32_t*>(hq + (size_t)row * cols + c0);
-  const int n4 = min(4096, cols - c0) >> 2;                      // cols % 128 == 0
-  for (int i = threadIdx.x; i < n4; i += blockDim.x) {
-    const float4 v = __ldcg(src + i);
-    uint16_t lo, hi;
-    asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(lo) : "f"(__fdiv_rn(v.y, s)), "f"(__fdiv_rn(v.x, s)));
-    asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(hi) : "f"(__fdiv_rn(v.w, s)), "f"(__fdiv_rn(v.z, s)));
-    dst[i] = (uint32_t)lo | ((uint32_t)hi << 16);
+  const int n4 = min(chunk_cols, cols - c0) >> 2;                // cols, chunk_cols % 128 == 0
+  // four loads in flight per thread: a couple of CTAs per SM have few warps to hide the L2 latency with
+  const float r = __frcp_rn(s);
+  auto quant2 = [&](float a, float b) {
+    // a / s, b / s correctly rounded (Markstein, as in the GEMM epilogue; a zero quotient keeps its sign)
+    const float qa0 = a * r, qb0 = b * r;
+    float qa = fmaf(fmaf(-qa0, s, a), r, qa0), qb = fmaf(fmaf(-qb0, s, b), r, qb0);
+    qa = qa == 0.0f ? qa0 : qa;
+    qb = qb == 0.0f ? qb0 : qb;
+    uint16_t o;
+    asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(o) : "f"(qb), "f"(qa));
+    return (uint32_t)o;
+  };
+#pragma unroll 1
+  for (int i0 = threadIdx.x; i0 < n4; i0 += 4 * blockDim.x) {
+    float4 v[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      if (i0 + k * blockDim.x < n4) v[k] = __ldcg(src + i0 + k * blockDim.x);
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      if (i0 + k * blockDim.x < n4) dst[i0 + k * blockDim.x] = quant2(v[k].x, v[k].y) | (quant2(v[k].z, v[k].w) << 16);
   }
 }
 
 }  // namespace
 
 int launch_requant_rows(const float* d_h, int rows, int cols, const float* d_amax_part, int n_part, int part_stride,
-                        int block_rows, uint8_t* d_hq, float* d_sh, cudaStream_t stream) {
+                        int block_rows, uint8_t* d_hq, float* d_sh, int sms, cudaStream_t stream) {
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)((cols + 4095) / 4096), (unsigned)rows);
+  int per_row = (2 * sms + rows - 1) / rows;                     // chunks per row: about two CTAs per SM in all
+  per_row = per_row < 2 ? 2 : per_row;
+  int chunk_cols = ((cols + per_row - 1) / per_row + 127) / 128 * 128;
+  chunk_cols = chunk_cols < 1024 ? 1024 : chunk_cols;
+  cfg.gridDim = dim3((unsigned)((cols + chunk_cols - 1) / chunk_cols), (unsigned)rows);
   cfg.blockDim = dim3(256);
   cfg.stream = stream;
   cudaLaunchAttribute attr[1];
@@ -340,7 +361,7 @@ int launch_requant_rows(const float* d_h, int rows, int cols, const float* d_ama
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  const cudaError_t e = cudaLaunchKernelEx(&cfg, requant_rows_kernel, d_h, cols, d_amax_part, n_part, part_stride, block_rows, d_hq, d_sh);
+  const cudaError_t e = cudaLaunchKernelEx(&cfg, requant_rows_kernel, d_h, cols, chunk_cols, d_amax_part, n_part, part_stride, block_rows, d_hq, d_sh);
   return e == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;
 }
 

@@ -183,6 +183,51 @@ def prune_2to4_magnitude(wgate, wup, wdown, perm, I_dense: int):
     return wgate, wup, wdown
 
 
+def sparsegpt_2to4(w, hinv, k_sparse: int):
+    """NEXT-4: SparseGPT's 2:4 column sweep with the dense columns on the right as compensation buffer (PAPER.md:98-111,
+    Eqs. 2-3; PAPER.md:149-153 "placing dense columns on the right keeps them available as a compensation buffer";
+    PAPER.md:202 "apply SparseGPT ... to the sparse regions while protecting the selected dense indices").
+
+    w: float [N, K], columns in PERMUTED order (sparse columns [0, k_sparse) first, k_sparse % 4 == 0, dense columns
+    last); hinv: H^-1 [K, K] of the layer input Hessian H = X^T X (symmetric positive definite; damping is the caller's
+    business).  Follows the paper's description step by step, in float64:
+      * columns are processed from left to right; "once a column is processed, its values are frozen" and "the induced
+        error is then compensated by updating only the columns that have not yet been processed" (PAPER.md:109);
+      * Hi is the inverse Hessian of the NOT YET PROCESSED columns ("reuse shared inverse-Hessian information across
+        rows"): after column j it loses row / column j by Gaussian elimination, which is the textbook inverse of the
+        remaining principal sub-matrix of H (pinned against numpy.linalg.inv in the tests);
+      * "for 2:4 sparsity, within each group, SparseGPT selects the weights to prune using the OBS-based error criterion"
+        (PAPER.md:111): when the sweep reaches a group of 4 columns it computes, per row, eps_c = w_c^2 / [Hi_c]_cc
+        (Eq. 3) for its 4 columns c, with the current w and with [Hi_c]_cc the diagonal entry column c will have when it
+        is reached (reading Q24: SparseGPT's own choice), and marks the 2 columns of smallest eps for pruning (ties:
+        the lower column is pruned first);
+      * a marked weight w_m is removed with Eq. 3: w += delta_m = -w_m / [Hi]_mm * Hi[m, :] over the unprocessed
+        columns (which makes w_m itself exactly 0); an unmarked weight is kept as it is.
+    Columns >= k_sparse are never pruned: they only receive compensation.  Returns (w_new, pruned_mask)."""
+    W = np.array(w, dtype=np.float64, copy=True)
+    N, K = W.shape
+    assert 0 <= k_sparse <= K and k_sparse % 4 == 0
+    Hi = np.array(hinv, dtype=np.float64, copy=True)          # rows / columns < j are dead once column j is reached
+    pruned = np.zeros((N, K), dtype=bool)
+    for j in range(k_sparse):
+        if j % 4 == 0:
+            blk = Hi[j:j + 4, j:j + 4].copy()                 # the 4 x 4 corner decides the 4 diagonals the group will see
+            d = np.empty(4)
+            for c in range(4):
+                d[c] = blk[c, c]
+                blk[c + 1:, c + 1:] -= np.outer(blk[c + 1:, c], blk[c, c + 1:]) / blk[c, c]
+            eps = W[:, j:j + 4] ** 2 / d[None, :]
+            order = np.argsort(eps, axis=1, kind="stable")    # stable: ties -> the lower column first
+            for r in range(N):
+                pruned[r, j + order[r, 0]] = True
+                pruned[r, j + order[r, 1]] = True
+        err = np.where(pruned[:, j], W[:, j] / Hi[j, j], 0.0)
+        W[:, j:] -= err[:, None] * Hi[j, j:][None, :]
+        W[pruned[:, j], j] = 0.0
+        Hi[j + 1:, j + 1:] -= np.outer(Hi[j + 1:, j], Hi[j, j + 1:]) / Hi[j, j]
+    return W, pruned
+
+
 def check_perm(perm: np.ndarray, I: int):
     perm = np.asarray(perm)
     if perm.shape != (I,) or perm.min(initial=0) < 0 or perm.max(initial=0) >= I \

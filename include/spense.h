@@ -227,6 +227,24 @@ int spense_select_dense(const spense_shape_t* shape, const float* d_wgate, const
 int spense_prune_2to4_magnitude(const spense_shape_t* shape, float* d_wgate, float* d_wup, float* d_wdown,
                                 const int32_t* d_perm, spense_stream_t stream);
 
+/* spense_prune_obs_2to4 -- pruning front-end: SparseGPT's 2:4 column sweep on ONE matrix with the
+ * dense columns on the right as compensation buffer (Eqs. 2-3; "placing dense columns on the right
+ * keeps them available as a compensation buffer"; "apply SparseGPT ... to the sparse regions while
+ * protecting the selected dense indices").
+ *   d_w [N, K] fp32 row-major, columns in PERMUTED order: the sparse columns [0, K_sparse) first (K_sparse % 4 == 0),
+ *   the dense columns last; pruned and compensated IN PLACE.  d_u [K, K] fp32 row-major: the upper triangular factor U of
+ *   the inverse of the (damped) input Hessian, H^-1 = U^T U, which the caller computes with a library routine.
+ * Columns are processed left to right and frozen once processed; when the sweep reaches a group of 4 it marks, per row,
+ * the 2 weights of smallest eps_m = w_m^2 / [H^-1]_mm (Eq. 3, with the inverse Hessian of the not yet processed columns;
+ * ties to the lower column); a marked weight is removed with delta_m = -w_m / [H^-1]_mm * H^-1[m, :] over the columns
+ * not yet processed.  Columns >= K_sparse are never pruned.  For a layer: W_down P with K_sparse = I_s; the rows
+ * [0, I_s) of P^T W_gate / P^T W_up with K_sparse = K = H (their dense rows are left alone, Q9b).
+ * fp32 arithmetic; floating point decides the masks, so results are compared with the oracle on loss and on the rows
+ * whose masks agree.  Workspace: spense_prune_obs_workspace_size bytes.  No synchronisation.              */
+int spense_prune_obs_workspace_size(int32_t N, int32_t K, size_t* bytes);
+int spense_prune_obs_2to4(int32_t N, int32_t K, int32_t K_sparse, float* d_w, const float* d_u, void* d_ws, size_t ws_bytes,
+                          spense_stream_t stream);
+
 /* spense_quantize_e4m3 -- helper (reading Q5): scale = amax / 448 (1 if amax == 0), per tensor or
  * per row; out = E4M3_rne_sat(in / scale) with an IEEE fp32 division.  d_scales: 1 or rows floats.
  * d_ws needs 4 bytes * (rows + 1). Bit-exact against the oracle.                                  */

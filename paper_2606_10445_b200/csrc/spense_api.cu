@@ -786,6 +786,26 @@ int spense_prune_2to4_magnitude(const spense_shape_t* shape, float* d_wgate, flo
   return launch_prune(shape, d_wgate, d_wup, d_wdown, d_perm, reinterpret_cast<cudaStream_t>(stream));
 }
 
+int spense_prune_obs_workspace_size(int32_t N, int32_t K, size_t* bytes) {
+  if (N < 1 || K < 4 || K % 4 || N > (1 << 24) || K > (1 << 20) || !bytes) return SPENSE_ERR_ARG;
+  *bytes = (size_t)N * 128 * sizeof(float);                       // the per-block errors e of every row
+  return SPENSE_OK;
+}
+
+int spense_prune_obs_2to4(int32_t N, int32_t K, int32_t K_sparse, float* d_w, const float* d_u, void* d_ws, size_t ws_bytes,
+                          spense_stream_t stream) {
+  size_t need = 0;
+  int st = spense_prune_obs_workspace_size(N, K, &need);
+  if (st) return st;
+  if (K_sparse < 0 || K_sparse > K || K_sparse % 4 || !d_w || !d_u || !d_ws) return SPENSE_ERR_ARG;
+  if (!aligned(d_w, 16) || !aligned(d_u, 16) || !aligned(d_ws, 16)) return SPENSE_ERR_ALIGN;
+  if (ws_bytes < need) return SPENSE_ERR_BUFFER_TOO_SMALL;
+  st = check_device(nullptr, nullptr);
+  if (st) return st;
+  if (K_sparse == 0) return SPENSE_OK;
+  return launch_prune_obs(N, K, K_sparse, d_w, d_u, d_ws, reinterpret_cast<cudaStream_t>(stream));
+}
+
 int spense_quantize_e4m3(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out, float* d_scales,
                          void* d_ws, size_t ws_bytes, spense_stream_t stream) {
   if (!d_in || !d_out || !d_scales || !d_ws || rows < 1 || cols < 1 || (mode != SPENSE_PER_TENSOR && mode != SPENSE_PER_ROW))

@@ -400,6 +400,7 @@ int launch_select(const spense_shape_t* shape, const float* d_wgate, const float
                   const float* d_hdiag_x, const float* d_hdiag_h, float eps, float* d_score, int32_t* d_dense_idx,
                   int32_t* d_perm, void* d_ws, cudaStream_t stream);
 int launch_prune(const spense_shape_t* shape, float* d_wgate, float* d_wup, float* d_wdown, const int32_t* d_perm, cudaStream_t stream);
+int launch_prune_obs(int N, int K, int K_sparse, float* d_w, const float* d_u, void* d_ws, cudaStream_t stream);
 int launch_quantize(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out, float* d_scales,
                     void* d_ws, cudaStream_t stream);
 

@@ -26,7 +26,7 @@ EXPORTS = ["spense_version", "spense_strerror", "spense_device_status", "spense_
            "spense_workspace_size", "spense_workspace_init", "spense_gate_up", "spense_down", "spense_mlp",
            "spense_mlp_dyn", "spense_mlp_host", "spense_mlp_stack_host", "spense_quantize_e4m3", "spense_prune_2to4_magnitude", "spense_dense_idx_last", "spense_select_workspace_size",
            "spense_select_dense", "spense_linear_pack_sizes", "spense_pack_linear", "spense_linear_workspace_size",
-           "spense_linear_out_split", "spense_linear_in_split"]
+           "spense_linear_out_split", "spense_linear_in_split", "spense_prune_obs_workspace_size", "spense_prune_obs_2to4"]
 
 SPENSE_SPLIT_OUT, SPENSE_SPLIT_IN = 0, 1
 
@@ -106,6 +106,8 @@ def lib() -> ctypes.CDLL:
         for f in (L.spense_linear_out_split, L.spense_linear_in_split):
             f.argtypes = [POINTER(LinearShape), c_void_p, c_void_p, c_void_p, c_int32, c_int32, c_void_p, c_int32, c_void_p,
                           c_size_t, c_void_p]
+        L.spense_prune_obs_workspace_size.argtypes = [c_int32, c_int32, POINTER(c_size_t)]
+        L.spense_prune_obs_2to4.argtypes = [c_int32, c_int32, c_int32, c_void_p, c_void_p, c_void_p, c_size_t, c_void_p]
         for name in EXPORTS:
             if name not in ("spense_strerror",):
                 getattr(L, name).restype = c_int
@@ -404,3 +406,15 @@ def spense_linear(lin: PackedLinear, x, s_x, ws, y=None, dtype=torch.float32):
     _check(f(ctypes.byref(lin.shape), _ptr(lin.blob), _ptr(x), _ptr(s_x), 0 if s_x.numel() == 1 else 1, M, _ptr(y),
              SPENSE_F32 if y.dtype == torch.float32 else SPENSE_BF16, _ptr(ws), ws.numel(), _stream()))
     return y
+
+
+def spense_prune_obs_2to4(w, u, k_sparse: int):
+    """SparseGPT 2:4 column sweep in place on w fp32 [N, K] (CUDA, permuted column order, sparse columns first) with
+    u fp32 [K, K] = the upper Cholesky factor of the inverse input Hessian (H^-1 = u^T u).  Returns w."""
+    _dev(w, torch.float32), _dev(u, torch.float32)
+    N, K = w.shape
+    b = c_size_t()
+    _check(lib().spense_prune_obs_workspace_size(N, K, ctypes.byref(b)))
+    ws = torch.empty(b.value, dtype=torch.uint8, device=w.device)
+    _check(lib().spense_prune_obs_2to4(N, K, k_sparse, _ptr(w), _ptr(u), _ptr(ws), b.value, _stream()))
+    return w

@@ -96,3 +96,17 @@ def test_linear_size_queries_and_argument_errors(sp):
     st = L.spense_linear_in_split(ctypes.byref(shp), ctypes.c_void_p(128), ctypes.c_void_p(128), ctypes.c_void_p(4), 0, 8,
                                   ctypes.c_void_p(16), 0, ctypes.c_void_p(128), 1 << 30, None)
     assert sp.STATUS[st] == "SPENSE_ERR_ARG"                      # an out-split shape handed to the in-split call
+
+
+def test_prune_obs_size_query_and_argument_errors(sp):
+    L = sp.lib()
+    b = ctypes.c_size_t()
+    assert L.spense_prune_obs_workspace_size(5120, 25600, ctypes.byref(b)) == 0 and b.value == 5120 * 128 * 4
+    assert sp.STATUS[L.spense_prune_obs_workspace_size(0, 128, ctypes.byref(b))] == "SPENSE_ERR_ARG"
+    assert sp.STATUS[L.spense_prune_obs_workspace_size(8, 130, ctypes.byref(b))] == "SPENSE_ERR_ARG"      # K % 4 != 0
+    one = ctypes.c_void_p(1 << 20)
+    for ks in (-4, 6, 132):                                       # negative, not a multiple of 4, beyond K
+        assert sp.STATUS[L.spense_prune_obs_2to4(8, 128, ks, one, one, one, 1 << 30, None)] == "SPENSE_ERR_ARG"
+    assert sp.STATUS[L.spense_prune_obs_2to4(8, 128, 64, None, one, one, 1 << 30, None)] == "SPENSE_ERR_ARG"
+    assert sp.STATUS[L.spense_prune_obs_2to4(8, 128, 64, ctypes.c_void_p(4), one, one, 1 << 30, None)] == "SPENSE_ERR_ALIGN"
+    assert sp.STATUS[L.spense_prune_obs_2to4(8, 128, 64, one, one, one, 16, None)] == "SPENSE_ERR_BUFFER_TOO_SMALL"

@@ -40,20 +40,20 @@ GEMM_CASES = [
     (256, 1024, 0.25, None, 64),
     (256, 1024, 0.25, None, 100),
     (256, 1024, 0.25, None, 128),
-    (256, 1024, 0.25, None, 200),   # two token blocks
+    (256, 1024, 0.25, None, 200),   # one block of 208 token columns
     (384, 640, None, 128, 16),      # H % 256 == 128
     (128, 384, None, 0, 5),         # I_s % 256 == 128, single half down tile
     (640, 896, None, 384, 48),
     (1024, 4096, 0.25, None, 64),   # enough stages for many spans / split-K partials
-    (256, 1024, 0.25, None, 80),    # 64 < M <= 96: two accumulator buffers at a 96-column stride
+    (256, 1024, 0.25, None, 80),    # token columns not a multiple of 32
     (1024, 4096, 0.25, None, 96),
-    (1024, 4096, 0.25, None, 112),  # 96 < M <= 112: two buffers at a 112-column stride (448 of the 480 columns below the metadata)
+    (1024, 4096, 0.25, None, 112),  # 7 x 16 token columns
     (256, 1024, 0.25, None, 240),   # the widest double-buffered token tile
     (1024, 4096, 0.25, None, 241),  # 241..256 tokens: one 256-column tile, single accumulator buffer, ragged
     (256, 1024, 0.25, None, 256),   # the same, full
-    (1024, 4096, 0.25, None, 257),  # two blocks of 144 columns again
-    (1024, 4096, 0.25, None, 300),  # three token blocks, ragged last one, spans crossing block boundaries
-    (640, 896, None, 384, 513),     # five blocks, last one holds a single token
+    (1024, 4096, 0.25, None, 257),  # gate_up: two blocks of 144 columns; down: three of 96
+    (1024, 4096, 0.25, None, 300),  # gate_up two blocks of 160, down three of 112 (ragged last one)
+    (640, 896, None, 384, 513),     # three blocks of 176, the last one ragged
 ]
 
 

@@ -38,7 +38,7 @@ LINEAR_CASES = [
     (384, 1024, 1.0, "in", 100),
     (4096, 1024, 0.25, "out", 16),    # enough stages for many spans and split-K partials
     (1024, 4096, 0.25, "in", 16),
-    (4096, 1024, 0.25, "out", 128),   # wide kernel, one token block
+    (4096, 1024, 0.25, "out", 128),   # one full-width token block
     (1024, 4096, 0.25, "in", 200),
     (2048, 512, 0.5, "out", 300),     # two token blocks
     (512, 2048, 0.5, "in", 513),      # three token blocks, ragged last one

@@ -787,7 +787,7 @@ int spense_prune_2to4_magnitude(const spense_shape_t* shape, float* d_wgate, flo
 }
 
 int spense_prune_obs_workspace_size(int32_t N, int32_t K, size_t* bytes) {
-  if (N < 1 || K < 4 || K % 4 || N > (1 << 24) || K > (1 << 20) || !bytes) return SPENSE_ERR_ARG;
+  if (N < 1 || K < 4 || K % 4 || N > (1 << 22) || K > (1 << 20) || !bytes) return SPENSE_ERR_ARG;   // N / 64 row tiles fit gridDim.y
   *bytes = (size_t)N * 128 * sizeof(float);                       // the per-block errors e of every row
   return SPENSE_OK;
 }

@@ -56,7 +56,8 @@ enum {
   SPENSE_ERR_ARCH = -8,             /* current device is not sm_100 */
   SPENSE_ERR_CUDA = -9,             /* a CUDA call failed; cudaGetLastError is preserved */
   SPENSE_ERR_BAD_BLOB = -10,        /* blob header does not match the shape / version (detected on the device) */
-  SPENSE_ERR_TIMEOUT = -11          /* a CTA gave up waiting for the other CTAs of its launch (detected on the device) */
+  SPENSE_ERR_TIMEOUT = -11,         /* a CTA gave up waiting for the other CTAs of its launch (detected on the device) */
+  SPENSE_ERR_STATIC_SCRATCH = -12   /* the request does not fit the built-in scratch of an allocation-free entry point */
 };
 
 enum { SPENSE_F32 = 0, SPENSE_BF16 = 1 };          /* y_dtype */
@@ -250,6 +251,27 @@ int spense_prune_obs_2to4(int32_t N, int32_t K, int32_t K_sparse, float* d_w, co
  * d_ws needs 4 bytes * (rows + 1). Bit-exact against the oracle.                                  */
 int spense_quantize_e4m3(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out,
                          float* d_scales, void* d_ws, size_t ws_bytes, spense_stream_t stream);
+
+/* spense_quantize_e4m3_static -- spense_quantize_e4m3 for callers that cannot provide the d_ws scratch because they cannot
+ * allocate device memory at the point of the call: code running inside a serving engine after it has handed the whole
+ * HBM budget to its KV-cache pool, a plug-in invoked from a host callback or from inside a framework's own allocator
+ * hook (where cudaMalloc would re-enter or deadlock), a real-time loop that must not hit the implicit device
+ * synchronisation of cudaMalloc / cudaFree.  Same arithmetic, same kernels and bit-identical results as
+ * spense_quantize_e4m3; only the home of the (rows + 1) floats of scratch differs: a fixed array inside the library image
+ * (256.25 KB, held by every GPU that loads libspense.so until the process exits) instead of a caller buffer.
+ *   d_in [rows, cols] fp32, d_out [rows, cols] E4M3 bytes, d_scales [1] or [rows] fp32: DEVICE, caller-owned, as in
+ *   spense_quantize_e4m3.  rows <= SPENSE_QUANTIZE_STATIC_MAX_ROWS, else SPENSE_ERR_STATIC_SCRATCH and nothing is launched
+ *   (cols is not limited by the scratch).
+ * The call itself allocates nothing, on the host or on the device: no cudaMalloc / cudaFree / cudaHostAlloc and no
+ * library routine that allocates.  The first call on each device looks up the device address of the array (the device
+ * must be current, as for every call here); make that first call outside any stream capture.  Later calls only
+ * enqueue the three kernels on `stream`; no synchronisation.
+ * ALL calls on one device share the one array: two calls whose kernels can overlap on the GPU (different streams without
+ * an ordering between them, or different host threads doing so) race on it and give wrong scales -- order them on one
+ * stream or with events.  Nothing in the array needs to start at zero, it simply holds the last call's maxima.          */
+#define SPENSE_QUANTIZE_STATIC_MAX_ROWS 65536
+int spense_quantize_e4m3_static(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out,
+                                float* d_scales, spense_stream_t stream);
 
 /* ---- Stand-alone Spense linears: the format is defined per weight matrix -- "Spense splits the
  * weight matrix into two parts: the semi-structured sparse part and the dense part" (Sec. 3.2) -- and comes

@@ -1,6 +1,8 @@
 // spense_pack kernels: P1 permute, P2 validate + 2:4 compress, P3 re-tile into stage images.
 // Integer / byte work only: results are bit-exact by construction (Eq. 1 PAPER.md:69, PAPER.md:74,
 // Fig. 4).  Also the E4M3 quantise helper (reading Q5).
+#include <mutex>
+
 #include "spense_internal.cuh"
 
 namespace spense {
@@ -469,3 +471,51 @@ int launch_pack_linear(const spense_linear_shape_t* shape, const uint8_t* d_w, f
 }
 
 }  // namespace spense
+
+// ---------------------------------------------------------------- spense_quantize_e4m3_static (include/spense.h)
+// The quantise helper for callers that have no device allocator to ask for the (rows + 1)-float scratch: the row maxima
+// and the tensor maximum live in an array that is part of the library image.  Same three kernels as launch_quantize.
+namespace spense {
+namespace {
+
+// Resident on every GPU that loads libspense.so, from load to process exit: 4 * (65536 + 64) bytes = 256.25 KB.
+// Layout as in launch_quantize: [0, rows) row maxima, [rows] the tensor maximum.  Nothing in it has to start at zero
+// (row_amax_kernel writes every slot the later kernels read), so calls do not clear it; it keeps the last call's values.
+static __device__ __align__(256) float g_quant_scratch[SPENSE_QUANTIZE_STATIC_MAX_ROWS + 64];
+
+std::mutex g_quant_mu;
+float* g_quant_ptr[64];   // per device ordinal: the DEVICE address of g_quant_scratch on that device (null = not set up yet)
+
+// In host code `g_quant_scratch` names a host-side shadow of the symbol, not memory a kernel can use: the address the
+// kernels get is looked up once per device, with that device current.  Allocates nothing.
+int quant_scratch_of_current_device(float** out) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return SPENSE_ERR_CUDA;
+  std::lock_guard<std::mutex> lk(g_quant_mu);
+  if (!g_quant_ptr[dev]) {
+    int major = 0, minor = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev) != cudaSuccess)
+      return SPENSE_ERR_CUDA;
+    if (major != 10 || minor != 0) return SPENSE_ERR_ARCH;
+    float* p = nullptr;
+    if (cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_quant_scratch) != cudaSuccess || !p) return SPENSE_ERR_CUDA;
+    g_quant_ptr[dev] = p;
+  }
+  *out = g_quant_ptr[dev];
+  return SPENSE_OK;
+}
+
+}  // namespace
+}  // namespace spense
+
+extern "C" int spense_quantize_e4m3_static(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out,
+                                           float* d_scales, spense_stream_t stream) {
+  if (!d_in || !d_out || !d_scales || rows < 1 || cols < 1 || (mode != SPENSE_PER_TENSOR && mode != SPENSE_PER_ROW))
+    return SPENSE_ERR_ARG;
+  if (rows > SPENSE_QUANTIZE_STATIC_MAX_ROWS) return SPENSE_ERR_STATIC_SCRATCH;
+  float* scratch = nullptr;
+  const int st = spense::quant_scratch_of_current_device(&scratch);
+  if (st) return st;
+  return spense::launch_quantize(d_in, rows, cols, mode, d_out, d_scales, scratch, reinterpret_cast<cudaStream_t>(stream));
+}

@@ -20,15 +20,17 @@ SPENSE_PER_TENSOR, SPENSE_PER_ROW = 0, 1
 STATUS = {0: "SPENSE_OK", -1: "SPENSE_ERR_ARG", -2: "SPENSE_ERR_ALIGN", -3: "SPENSE_ERR_SHAPE",
           -4: "SPENSE_ERR_BUFFER_TOO_SMALL", -5: "SPENSE_ERR_NOT_2_4", -6: "SPENSE_ERR_NAN_WEIGHT",
           -7: "SPENSE_ERR_BAD_PERM", -8: "SPENSE_ERR_ARCH", -9: "SPENSE_ERR_CUDA", -10: "SPENSE_ERR_BAD_BLOB",
-          -11: "SPENSE_ERR_TIMEOUT"}
+          -11: "SPENSE_ERR_TIMEOUT", -12: "SPENSE_ERR_STATIC_SCRATCH"}
 
 EXPORTS = ["spense_version", "spense_strerror", "spense_device_status", "spense_schedule", "spense_perm_from_dense_idx", "spense_pack_sizes", "spense_pack",
            "spense_workspace_size", "spense_workspace_init", "spense_gate_up", "spense_down", "spense_mlp",
            "spense_mlp_dyn", "spense_mlp_host", "spense_mlp_stack_host", "spense_quantize_e4m3", "spense_prune_2to4_magnitude", "spense_dense_idx_last", "spense_select_workspace_size",
            "spense_select_dense", "spense_linear_pack_sizes", "spense_pack_linear", "spense_linear_workspace_size",
-           "spense_linear_out_split", "spense_linear_in_split", "spense_prune_obs_workspace_size", "spense_prune_obs_2to4"]
+           "spense_linear_out_split", "spense_linear_in_split", "spense_prune_obs_workspace_size", "spense_prune_obs_2to4",
+           "spense_quantize_e4m3_static"]
 
 SPENSE_SPLIT_OUT, SPENSE_SPLIT_IN = 0, 1
+SPENSE_QUANTIZE_STATIC_MAX_ROWS = 65536
 
 
 class SpenseError(RuntimeError):
@@ -99,6 +101,7 @@ def lib() -> ctypes.CDLL:
         L.spense_dense_idx_last.argtypes = [c_int32, c_int32, POINTER(c_int32)]
         L.spense_quantize_e4m3.argtypes = [c_void_p, c_int64, c_int64, c_int32, c_void_p, c_void_p, c_void_p,
                                            c_size_t, c_void_p]
+        L.spense_quantize_e4m3_static.argtypes = [c_void_p, c_int64, c_int64, c_int32, c_void_p, c_void_p, c_void_p]
         L.spense_linear_pack_sizes.argtypes = [POINTER(LinearShape), POINTER(c_size_t), POINTER(c_size_t)]
         L.spense_pack_linear.argtypes = [POINTER(LinearShape), c_void_p, c_float, c_void_p, c_void_p, c_size_t, POINTER(LinearCanon),
                                          c_void_p, c_size_t, POINTER(c_int64), c_void_p]
@@ -329,6 +332,24 @@ def spense_quantize_e4m3(x: torch.Tensor, mode: int):
     scales = torch.empty(rows if mode == SPENSE_PER_ROW else 1, dtype=torch.float32, device=x.device)
     ws = torch.empty((rows + 1) * 4, dtype=torch.uint8, device=x.device)
     _check(lib().spense_quantize_e4m3(_ptr(x), rows, cols, mode, _ptr(out), _ptr(scales), _ptr(ws), ws.numel(), _stream()))
+    return out, scales
+
+
+def spense_quantize_e4m3_static(x: torch.Tensor, mode: int, out: torch.Tensor, scales: torch.Tensor):
+    """spense_quantize_e4m3 without a scratch buffer, for callers that must not allocate device memory when they call
+    (an engine that already gave all of HBM to its cache pool, a host callback, a latency-critical loop): the scratch is a
+    fixed 256 KB array inside libspense.so, so at most SPENSE_QUANTIZE_STATIC_MAX_ROWS rows.  Unlike the other wrappers
+    this one creates no tensor either: `out` [rows, cols] uint8 and `scales` [rows] or [1] fp32 are the caller's.
+    All calls on a device share that array: keep them ordered on one stream.  Make the first call on a device outside
+    stream capture (it looks up the array's address).  Returns (out, scales)."""
+    _dev(x, torch.float32)
+    rows, cols = x.shape
+    n_scales = rows if mode == SPENSE_PER_ROW else 1
+    if out.dtype != torch.uint8 or tuple(out.shape) != (rows, cols) or not out.is_contiguous() or out.device != x.device:
+        raise ValueError("out must be a contiguous [rows, cols] uint8 tensor on x's device")
+    if scales.dtype != torch.float32 or scales.numel() != n_scales or not scales.is_contiguous() or scales.device != x.device:
+        raise ValueError("scales must be a contiguous fp32 tensor of rows (per row) or 1 (per tensor) elements on x's device")
+    _check(lib().spense_quantize_e4m3_static(_ptr(x), rows, cols, mode, _ptr(out), _ptr(scales), _stream()))
     return out, scales
 
 

@@ -29,7 +29,11 @@
  *     the blob header (magic, version, shape) is checked by the kernels that read the weight scales from it
  *     (SPENSE_ERR_BAD_BLOB), and a CTA that waits more than 2 s for the other CTAs of its launch records
  *     SPENSE_ERR_TIMEOUT and traps instead of hanging.  A recorded error is returned by every later GEMM call
- *     until it is cleared.
+ *     until it is cleared.  The two differ in what survives them: after SPENSE_ERR_BAD_BLOB the launch has ended
+ *     normally (nothing stored) and clearing the word is all it takes to go on.  SPENSE_ERR_TIMEOUT is FATAL to the
+ *     process's CUDA context: the trap is a sticky launch failure, every later CUDA call of the process (the
+ *     caller's own included) fails, device memory of the context is lost, and clearing the word recovers nothing --
+ *     the word, which lives in host memory, is there so that the process can still say WHY before it exits.
  *   - There is NO CPU fallback: on a device that is not sm_100 the calls return SPENSE_ERR_ARCH.
  */
 #ifndef SPENSE_H_
@@ -56,7 +60,8 @@ enum {
   SPENSE_ERR_ARCH = -8,             /* current device is not sm_100 */
   SPENSE_ERR_CUDA = -9,             /* a CUDA call failed; cudaGetLastError is preserved */
   SPENSE_ERR_BAD_BLOB = -10,        /* blob header does not match the shape / version (detected on the device) */
-  SPENSE_ERR_TIMEOUT = -11,         /* a CTA gave up waiting for the other CTAs of its launch (detected on the device) */
+  SPENSE_ERR_TIMEOUT = -11,         /* a CTA gave up waiting for the other CTAs of its launch (detected on the device);
+                                       the kernel trapped: the CUDA context is lost, restart the process */
   SPENSE_ERR_STATIC_SCRATCH = -12   /* the request does not fit the built-in scratch of an allocation-free entry point */
 };
 
@@ -91,7 +96,8 @@ const char* spense_strerror(int status);
 
 /* The first error a kernel of an earlier launch recorded (SPENSE_OK if none): SPENSE_ERR_BAD_BLOB or
  * SPENSE_ERR_TIMEOUT.  Host only; meaningful once the launches in question have completed (synchronise the
- * stream first).  clear != 0 resets the word.                                                            */
+ * stream first -- after a time-out that synchronise itself returns a CUDA error, the word is still readable).
+ * clear != 0 resets the word (enough to continue after BAD_BLOB; after TIMEOUT the context is gone, see above).                                                            */
 int spense_device_status(int clear);
 
 /* Host helper (Sec. 3.3.1; reading Q9): the permutation that moves the chosen dense
@@ -126,7 +132,8 @@ int spense_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8
  * launch advances the epoch word, so nothing needs resetting between calls or CUDA-graph replays.
  * One workspace must not be used by two streams concurrently.  The CTAs of one GEMM launch wait
  * for each other (split-K fix-up): the calls refuse (SPENSE_ERR_CUDA) a grid the device cannot hold resident at
- * once, and a launch starved of SMs by other work ends with SPENSE_ERR_TIMEOUT instead of hanging.          */
+ * once, and a launch starved of SMs by other work ends with SPENSE_ERR_TIMEOUT (a trap: fatal to the CUDA context,
+ * but reported) instead of hanging.                                                                         */
 int spense_workspace_size(const spense_shape_t* shape, int32_t M, size_t* bytes);
 int spense_workspace_init(void* d_ws, size_t ws_bytes, spense_stream_t stream);
 

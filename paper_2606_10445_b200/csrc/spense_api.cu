@@ -492,7 +492,7 @@ const char* spense_strerror(int status) {
     case SPENSE_ERR_ARCH: return "device is not sm_100 (no fallback path exists)";
     case SPENSE_ERR_CUDA: return "CUDA error";
     case SPENSE_ERR_BAD_BLOB: return "blob header does not match";
-    case SPENSE_ERR_TIMEOUT: return "a CTA gave up waiting for the other CTAs of its launch (device shared with other work?)";
+    case SPENSE_ERR_TIMEOUT: return "a CTA gave up waiting for the other CTAs of its launch and trapped (device shared with other work?); the CUDA context is lost";
     case SPENSE_ERR_STATIC_SCRATCH: return "request exceeds the built-in scratch of the allocation-free entry point (see its MAX in spense.h)";
     default: return "unknown status";
   }

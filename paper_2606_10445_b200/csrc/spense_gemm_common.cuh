@@ -79,7 +79,9 @@ __device__ __forceinline__ float silu_mul(float g, float u) {
 // a / b from the correctly rounded reciprocal r = RN(1/b) and two FMAs (Markstein): branch-free and
 // correctly rounded wherever the quotient is a normal number -- all the E4M3 cast after it can see
 // (a zero quotient keeps the sign IEEE division gives it: h = -0 must encode as 0x80 like the oracle's).
+// A divisor below 2^-128 (a caller's tiny s_h) has no finite fp32 reciprocal: those take the IEEE division.
 __device__ __forceinline__ float div_by(float a, float b, float r) {
+  if (__builtin_expect(!(fabsf(r) <= 3.402823466e+38f), 0)) return __fdiv_rn(a, b);
   const float q0 = a * r;
   const float rem = fmaf(-q0, b, a);
   const float q = fmaf(rem, r, q0);
@@ -116,7 +118,10 @@ __device__ __forceinline__ void st_release(int* p, int v) {
 // the same time; the host checks that against the occupancy the device offers before launching, and every wait here
 // gives up after kWaitBudgetNs: the CTA records SPENSE_ERR_TIMEOUT in the mapped host status word and traps, so a launch
 // whose peers never show up (device shared with work that pins SMs) fails with a CUDA error instead of hanging for ever;
-// spense_device_status() then says why.  A launch that works never reads the timer: the first try succeeds.
+// spense_device_status() then says why.  The trap is deliberate and documented as fatal to the context (spense.h): a
+// cooperative exit would have to unwind four warp roles, the pair's cluster barrier and the TMEM allocation of CTAs whose
+// peers are not coming, and a launch in that state has no result worth keeping.
+// A launch that works never reads the timer: the first try succeeds.
 static __device__ __noinline__ void give_up(int* status, int code) {
   atomicCAS_system(status, 0, code);
   __threadfence_system();

@@ -324,12 +324,14 @@ __global__ void __launch_bounds__(256) requant_rows_kernel(const float* __restri
   const int n4 = min(chunk_cols, cols - c0) >> 2;                // cols, chunk_cols % 128 == 0
   // four loads in flight per thread: a couple of CTAs per SM have few warps to hide the L2 latency with
   const float r = __frcp_rn(s);
+  const bool r_finite = r <= 3.402823466e+38f;   // a row maximum below 448 * 2^-128 gives s without a finite fp32 reciprocal
   auto quant2 = [&](float a, float b) {
     // a / s, b / s correctly rounded (Markstein, as in the GEMM epilogue; a zero quotient keeps its sign)
     const float qa0 = a * r, qb0 = b * r;
     float qa = fmaf(fmaf(-qa0, s, a), r, qa0), qb = fmaf(fmaf(-qb0, s, b), r, qb0);
     qa = qa == 0.0f ? qa0 : qa;
     qb = qb == 0.0f ? qb0 : qb;
+    if (!r_finite) { qa = __fdiv_rn(a, s); qb = __fdiv_rn(b, s); }   // uniform over the CTA (one row): IEEE division
     uint16_t o;
     asm("cvt.rn.satfinite.e4m3x2.f32 %0, %1, %2;" : "=h"(o) : "f"(qb), "f"(qa));
     return (uint32_t)o;

@@ -32,6 +32,9 @@ def test_mlp_dyn_parity(sp, H, I, p, M):
     if M > 2:                                            # an all-zero token: scale 1, zero bytes, zero y
         c.x = c.x.clone()
         c.x[1] = 0
+    if M > 4:                                            # a token whose h is ~1e-37: s_h = amax / 448 is below 2^-128 and has
+        c.s_x = c.s_x.clone()                            # no finite fp32 reciprocal (the quotients must still be IEEE's)
+        c.s_x[3] = 3e-19
     pk = c.pack_gpu(sp)
     ws = sp.spense_workspace(pk, M)
     ref = o.mlp_dynamic(c.x.numpy(), c.s_x.numpy(), c.wg, c.wu, c.wd, c.L.w_scale)
@@ -50,6 +53,13 @@ def test_mlp_dyn_parity(sp, H, I, p, M):
     assert np.array_equal(hq_gpu, own)
     live = np.abs(h_gpu).max(axis=1) > 0
     assert ((hq_gpu[live] & 0x7F).max(axis=1) == 0x7E).all()       # the row maximum lands on +-448
+    if M > 4:
+        assert 0 < sh_gpu[3] < 2.0 ** -128, sh_gpu[3]
+        assert (hq_gpu[3] & 0x7F).max() == 0x7E and not ((hq_gpu[3] & 0x7F) == 0x7F).any()
+        # the static path given that tiny scale divides by it in its epilogue: same bytes
+        hq_s = sp.spense_gate_up(pk, cuda(c.x), cuda(c.s_x), s_h, ws)
+        torch.cuda.synchronize()
+        assert torch.equal(hq_s, hq)
     if M > 2:
         assert sh_gpu[1] == 1.0 and not hq_gpu[1].any() and not y_gpu[1].any()
     diff = (hq_gpu != ref["hq"]).mean()

@@ -23,8 +23,11 @@ def _stale() -> bool:
 def build(force: bool = False, verbose: bool = False, debug_hooks: bool = False, out: str | None = None) -> str:
     """debug_hooks: also compile the per-CTA timeline hook (spense_debug_set_trace, not declared in spense.h) into a
     library written to `out`; the default build exports exactly what include/spense.h declares."""
-    lib = out or LIB
-    if not debug_hooks and not force and not _stale():
+    if debug_hooks and (out is None or os.path.abspath(out) == LIB):
+        raise ValueError("a debug_hooks build must be written to an explicit `out` other than libspense.so: it reads "
+                         "SPENSE_* environment knobs and exports a symbol spense.h does not declare")
+    lib = os.path.abspath(out) if out else LIB
+    if lib == LIB and not force and not _stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",

@@ -788,7 +788,7 @@ int spense_prune_2to4_magnitude(const spense_shape_t* shape, float* d_wgate, flo
 }
 
 int spense_prune_obs_workspace_size(int32_t N, int32_t K, size_t* bytes) {
-  if (N < 1 || K < 4 || K % 4 || N > (1 << 22) || K > (1 << 20) || !bytes) return SPENSE_ERR_ARG;   // N / 64 row tiles fit gridDim.y
+  if (N < 1 || K < 4 || K % 4 || N > 65535 * 64 || K > (1 << 20) || !bytes) return SPENSE_ERR_ARG;   // ceil(N / 64) row tiles must fit gridDim.y (65535)
   *bytes = (size_t)N * 128 * sizeof(float);                       // the per-block errors e of every row
   return SPENSE_OK;
 }

@@ -124,12 +124,17 @@ int launch_prune_obs(int N, int K, int K_sparse, float* d_w, const float* d_u, v
   if (cudaFuncSetAttribute(obs_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return SPENSE_ERR_CUDA;
   for (int j0 = 0; j0 < K_sparse; j0 += kObsBlock) {
     const int cols = K_sparse - j0 < kObsBlock ? K_sparse - j0 : kObsBlock;
+    // W is swept in place: a launch that is refused is reported at once, before the next block builds on a matrix
+    // that is only partly processed (the caller must then treat d_w as undefined)
     obs_block_kernel<<<(N + kObsRows - 1) / kObsRows, kObsRows, smem, stream>>>(d_w, d_u, N, K, j0, cols, err);
+    if (cudaGetLastError() != cudaSuccess) return SPENSE_ERR_CUDA;
     const int j1 = j0 + cols;
-    if (j1 < K)
+    if (j1 < K) {
       obs_trailing_kernel<<<dim3((K - j1 + kTile - 1) / kTile, (N + kTile - 1) / kTile), 256, 0, stream>>>(d_w, d_u, err, N, K, j0, cols, j1);
+      if (cudaGetLastError() != cudaSuccess) return SPENSE_ERR_CUDA;
+    }
   }
-  return cudaGetLastError() == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;
+  return SPENSE_OK;
 }
 
 }  // namespace spense

@@ -104,9 +104,23 @@ def test_prune_obs_size_query_and_argument_errors(sp):
     assert L.spense_prune_obs_workspace_size(5120, 25600, ctypes.byref(b)) == 0 and b.value == 5120 * 128 * 4
     assert sp.STATUS[L.spense_prune_obs_workspace_size(0, 128, ctypes.byref(b))] == "SPENSE_ERR_ARG"
     assert sp.STATUS[L.spense_prune_obs_workspace_size(8, 130, ctypes.byref(b))] == "SPENSE_ERR_ARG"      # K % 4 != 0
+    # the trailing update indexes 64-row tiles on gridDim.y: 65535 tiles is the last row count that fits
+    assert L.spense_prune_obs_workspace_size(65535 * 64, 128, ctypes.byref(b)) == 0
+    assert sp.STATUS[L.spense_prune_obs_workspace_size(65535 * 64 + 1, 128, ctypes.byref(b))] == "SPENSE_ERR_ARG"
     one = ctypes.c_void_p(1 << 20)
     for ks in (-4, 6, 132):                                       # negative, not a multiple of 4, beyond K
         assert sp.STATUS[L.spense_prune_obs_2to4(8, 128, ks, one, one, one, 1 << 30, None)] == "SPENSE_ERR_ARG"
     assert sp.STATUS[L.spense_prune_obs_2to4(8, 128, 64, None, one, one, 1 << 30, None)] == "SPENSE_ERR_ARG"
     assert sp.STATUS[L.spense_prune_obs_2to4(8, 128, 64, ctypes.c_void_p(4), one, one, 1 << 30, None)] == "SPENSE_ERR_ALIGN"
     assert sp.STATUS[L.spense_prune_obs_2to4(8, 128, 64, one, one, one, 16, None)] == "SPENSE_ERR_BUFFER_TOO_SMALL"
+
+
+def test_build_never_replaces_the_production_library_with_a_debug_build(sp, tmp_path):
+    from paper_2606_10445_b200 import build
+    with pytest.raises(ValueError):
+        build.build(debug_hooks=True)                              # no out: would overwrite libspense.so
+    with pytest.raises(ValueError):
+        build.build(debug_hooks=True, out=build.LIB)
+    # out= is honoured without debug hooks too (used to return libspense.so untouched when the tree was not stale)
+    out = str(tmp_path / "libspense_copy.so")
+    assert build.build(out=out) == out and os.path.getsize(out) > 0

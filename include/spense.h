@@ -23,7 +23,9 @@
  *   - Every call returns a status (0 = SPENSE_OK, negative = error).  Nothing throws, aborts or
  *     prints.  Argument errors are detected on the host before any launch.
  *   - All GPU work is enqueued on the caller's stream.  GEMM calls never synchronise and never read device
- *     memory on the host: the first call on a fresh blob may be issued inside a CUDA stream capture.
+ *     memory on the host: the first call on a fresh blob may be issued inside a CUDA stream capture.  The library's
+ *     one-time set-up per process and device (a pinned host status word, a driver entry point, per-kernel attributes)
+ *     is done by spense_workspace_init, which every GEMM caller has to call anyway and which must NOT be captured.
  *     spense_pack synchronises the stream once to read back its validation word.
  *   - What only the device can see is reported through a pinned host status word (spense_device_status):
  *     the blob header (magic, version, shape) is checked by the kernels that read the weight scales from it
@@ -128,7 +130,8 @@ int spense_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8
                 int64_t* h_err_where, spense_stream_t stream);
 
 /* Workspace for the GEMM calls at up to M tokens (split-K partial tiles, flags, a launch-epoch word).
- * The workspace must be initialised ONCE with spense_workspace_init before its first use; every
+ * The workspace must be initialised ONCE with spense_workspace_init before its first use (outside stream capture: the
+ * call also performs the library's one-time set-up for the current device, which allocates a few pinned host bytes); every
  * launch advances the epoch word, so nothing needs resetting between calls or CUDA-graph replays.
  * One workspace must not be used by two streams concurrently.  The CTAs of one GEMM launch wait
  * for each other (split-K fix-up): the calls refuse (SPENSE_ERR_CUDA) a grid the device cannot hold resident at
@@ -258,6 +261,15 @@ int spense_prune_obs_2to4(int32_t N, int32_t K, int32_t K_sparse, float* d_w, co
  * d_ws needs 4 bytes * (rows + 1). Bit-exact against the oracle.                                  */
 int spense_quantize_e4m3(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out,
                          float* d_scales, void* d_ws, size_t ws_bytes, spense_stream_t stream);
+
+/* spense_probe_read -- measurement helper ("time floors"): stream `bytes` of device memory through the SMs
+ * exactly as the GEMM kernels stream their weights (one cp.async.bulk of 32 KB after the other into a 192 KB shared-memory
+ * ring per SM, chunks dealt round robin over one CTA per SM) and discard them.  The rate of this call, timed by the caller
+ * with events around it, is the read-only HBM ceiling of the box for this access pattern: bench.py reports the GEMM's
+ * achieved GB/s against it next to the copy rate of MEASURED_PEAKS.json.  Not part of the Spense path.
+ *   d_buf: DEVICE, 128-byte aligned, bytes a multiple of 32768 (use more than the 126 MB L2, e.g. >= 2 GB).
+ *   d_sink: DEVICE, 256 uint32 (one XOR word per CTA, proof that the bytes arrived).  No synchronisation.             */
+int spense_probe_read(const void* d_buf, size_t bytes, uint32_t* d_sink, spense_stream_t stream);
 
 /* spense_quantize_e4m3_static -- spense_quantize_e4m3 for callers that cannot provide the d_ws scratch because they cannot
  * allocate device memory at the point of the call: code running inside a serving engine after it has handed the whole

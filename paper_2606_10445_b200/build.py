@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libspense.so")
-SOURCES = ["spense_api.cu", "spense_gemm.cu", "spense_pack.cu", "spense_select.cu", "spense_prune.cu"]
+SOURCES = ["spense_api.cu", "spense_gemm.cu", "spense_pack.cu", "spense_select.cu", "spense_prune.cu", "spense_probe.cu"]
 
 
 def _stale() -> bool:

@@ -581,6 +581,13 @@ int spense_workspace_size(const spense_shape_t* shape, int32_t M, size_t* bytes)
 int spense_workspace_init(void* d_ws, size_t ws_bytes, spense_stream_t stream) {
   if (!d_ws) return SPENSE_ERR_ARG;
   if (ws_bytes < (size_t)kWsFixedBytes) return SPENSE_ERR_BUFFER_TOO_SMALL;
+  // everything the library sets up once per process / device happens here, outside any capture: the pinned status word,
+  // the tensor-map encoder entry point, each GEMM kernel's shared-memory opt-in and residency query
+  int dev = 0;
+  int st = check_device(&dev, nullptr);
+  if (st) return st;
+  st = prepare_gemm_kernels(dev);
+  if (st) return st;
   return cudaMemsetAsync(d_ws, 0, kWsFixedBytes, reinterpret_cast<cudaStream_t>(stream)) == cudaSuccess ? SPENSE_OK : SPENSE_ERR_CUDA;
 }
 
@@ -805,6 +812,15 @@ int spense_prune_obs_2to4(int32_t N, int32_t K, int32_t K_sparse, float* d_w, co
   if (st) return st;
   if (K_sparse == 0) return SPENSE_OK;
   return launch_prune_obs(N, K, K_sparse, d_w, d_u, d_ws, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int spense_probe_read(const void* d_buf, size_t bytes, uint32_t* d_sink, spense_stream_t stream) {
+  if (!d_buf || !d_sink || bytes < 32768 || bytes % 32768) return SPENSE_ERR_ARG;
+  if (!aligned(d_buf, 128) || !aligned(d_sink, 4)) return SPENSE_ERR_ALIGN;
+  int sms = 0;
+  int st = check_device(nullptr, &sms);
+  if (st) return st;
+  return launch_read_probe(d_buf, bytes, d_sink, sms, reinterpret_cast<cudaStream_t>(stream));
 }
 
 int spense_quantize_e4m3(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out, float* d_scales,

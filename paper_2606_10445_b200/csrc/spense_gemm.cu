@@ -227,23 +227,27 @@ __device__ __forceinline__ void mma_issuer(const GemmParams& p, const Ctx& cx, i
     const int seg_end = min(se, tile_end);
     const int buf = p.num_acc_bufs == 2 ? seg & 1 : 0;
     const uint32_t use = (uint32_t)(p.num_acc_bufs == 2 ? seg >> 1 : seg);
-    long long tw0 = p.trace ? globaltimer() : 0;
+    long long tw0 = tracing(p) ? globaltimer() : 0;
     wait_bar(p, cx.acce_bar(buf), (use & 1u) ^ 1u);        // both CTAs' epilogues have drained this accumulator
     const bool pre = preloaded_segment(p, span, sb, se, c.first, tile_end, seg_end);
     if (pre) wait_bar(p, cx.pre_bar(), 0);                 // both CTAs have stored the partner's partial into this accumulator
-    if (p.trace) t_acce += globaltimer() - tw0;
+    if (tracing(p)) t_acce += globaltimer() - tw0;
     tc_fence_after();
     const uint32_t d = cx.tmem_base + (uint32_t)(buf * p.acc_stride);
     uint32_t acc = pre ? 1u : 0u;
 #pragma unroll 1
     for (; s < seg_end; ++s, ++it, ++c.j) {
-      if (p.trace) tw0 = globaltimer();
+      if (tracing(p)) tw0 = globaltimer();
       wait_bar(p, fb, ph);
-      if (p.trace) t_full += globaltimer() - tw0;
+      if (tracing(p)) t_full += globaltimer() - tw0;
       tc_fence_after();
       if (s == sb) trace(p, span, 3);
       const uint32_t b_lo = a_lo + (kSparseOperandBytes >> 4);
-      if (issuer && !(p.dbg & 2)) {
+#ifdef SPENSE_DEBUG_HOOKS
+      if (issuer && !(p.dbg & 2)) {              // experiment: stream the stages without issuing the MMAs
+#else
+      if (issuer) {
+#endif
         if (c.j < c.ns) {
           const uint32_t e_base = cx.tmem_base + kMetaCol + (it & 1u) * 8u;
           const uint32_t m_lo = (a_lo & 0x3FFFu) + (kOperandBytes >> 4);     // metadata atoms: LBO 0
@@ -269,7 +273,7 @@ __device__ __forceinline__ void mma_issuer(const GemmParams& p, const Ctx& cx, i
     if (s == tile_end) next_tile<MODE>(p, c);
   }
   trace(p, span, 4);
-  if (p.trace && cx.blk == p.blk0 && issuer) { p.trace[(size_t)span * 16 + 11] = t_full; p.trace[(size_t)span * 16 + 12] = t_acce; }
+  if (tracing(p) && cx.blk == p.blk0 && issuer) { p.trace[(size_t)span * 16 + 11] = t_full; p.trace[(size_t)span * 16 + 12] = t_acce; }
 }
 
 // scale tables of the pair's token block (weight scales come from the blob header, on the device)
@@ -517,7 +521,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
   tc_fence_after();
   cx.tmem_base = *cx.tmem_slot_ptr();
   pdl_launch_dependents();
-  if (p.trace && threadIdx.x == 0 && bp == 0 && cx.rank == 0) {
+  if (tracing(p) && threadIdx.x == 0 && bp == 0 && cx.rank == 0) {
     uint32_t smid;
     asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
     p.trace[(size_t)span * 16 + 0] = globaltimer(); p.trace[(size_t)span * 16 + 14] = smid;
@@ -548,7 +552,7 @@ spense_gemm_kernel(const __grid_constant__ GemmParams p, const __grid_constant__
       if (et < p.n_pad) p.amax_part[(size_t)(cx.slot0 + 2 * span) * p.n_pad + et] = et < Mb ? cx.sc0()[et].z : 0.0f;
     }
     if (et == 0) *cx.epi_done_ptr() = 1;
-    if (p.trace && et == 0 && bp == 0 && cx.rank == 0) p.trace[(size_t)span * 16 + 10] = globaltimer();
+    if (tracing(p) && et == 0 && bp == 0 && cx.rank == 0) p.trace[(size_t)span * 16 + 10] = globaltimer();
   }
 
   tc_fence_before();
@@ -581,6 +585,16 @@ int prepare(K kernel, int which, int dev, int grid) {
   return grid <= resident[which][dev] ? SPENSE_OK : SPENSE_ERR_CUDA;
 }
 }  // namespace
+
+// the once-per-device work of every kernel instance, done ahead of the first launch (spense_workspace_init): the first GEMM
+// call then only launches, which is what lets it sit inside a stream capture in a process that never packed a blob
+int prepare_gemm_kernels(int dev) {
+  int st = prepare(spense_gemm_kernel<0, false>, 0, dev, 0);
+  if (!st) st = prepare(spense_gemm_kernel<0, true>, 1, dev, 0);
+  if (!st) st = prepare(spense_gemm_kernel<1, false>, 2, dev, 0);
+  if (!st) st = prepare(spense_gemm_kernel<2, false>, 3, dev, 0);
+  return st;
+}
 
 int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, const CUtensorMap& tmap_ws, const CUtensorMap& tmap_wd, bool pdl, int dev,
                 cudaStream_t stream) {

@@ -101,9 +101,16 @@ __device__ __forceinline__ long long globaltimer() {
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
   return t;
 }
-// optional per-CTA timeline (SPENSE_DEBUG_HOOKS builds set GemmParams::trace; nullptr in production)
+// optional per-CTA timeline: SPENSE_DEBUG_HOOKS builds set GemmParams::trace; the shipped library compiles none of it
+__device__ __forceinline__ bool tracing(const GemmParams& p) {
+#ifdef SPENSE_DEBUG_HOOKS
+  return p.trace != nullptr;
+#else
+  return false;
+#endif
+}
 __device__ __forceinline__ void trace(const GemmParams& p, int span, int slot) {
-  if (p.trace) p.trace[(size_t)span * 16 + slot] = globaltimer();
+  if (tracing(p)) p.trace[(size_t)span * 16 + slot] = globaltimer();
 }
 __device__ __forceinline__ int ld_acquire(const int* p) {
   int v;
@@ -135,7 +142,9 @@ __device__ __forceinline__ void wait_bar(const GemmParams& p, uint32_t bar, uint
 #pragma unroll 1
     for (int i = 0; i < 32; ++i) {
       if (mbar_try(bar, parity)) return;
+#ifdef SPENSE_DEBUG_HOOKS
       if ((p.dbg & 4) && threadIdx.x >= 128) __nanosleep(200);
+#endif
     }
     if (globaltimer() - t0 > kWaitBudgetNs) give_up(p.status, SPENSE_ERR_TIMEOUT);
   }

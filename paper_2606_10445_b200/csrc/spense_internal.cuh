@@ -181,18 +181,6 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "WAIT_LOOP:\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-      "@p bra WAIT_DONE;\n\t"
-      "bra WAIT_LOOP;\n\t"
-      "WAIT_DONE:\n\t}" ::"r"(bar), "r"(parity) : "memory");
-}
 // one try (the hardware suspends the thread up to an implementation-defined time): true once the phase is complete
 __device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity) {
   uint32_t ok;
@@ -243,14 +231,7 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
       "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
       ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
 }
-// 2-D tiled TMA load (SASS: UTMALDG)
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar, uint64_t pol) {
-  asm volatile(
-      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint "
-      "[%0], [%1, {%2, %3}], [%4], %5;"
-      ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar), "l"(pol) : "memory");
-}
-// the same issued by either CTA of a pair: the bytes land in the issuing CTA, the transaction count goes to `cluster_bar`
+// 2-D tiled TMA load (SASS: UTMALDG) issued by either CTA of a pair: the bytes land in the issuing CTA, the transaction count goes to `cluster_bar`
 // (the LEADER CTA's barrier, a shared::cluster address), so the leader's MMA thread sees both halves of a stage
 __device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t cluster_bar, uint64_t pol) {
   asm volatile(
@@ -263,37 +244,8 @@ __device__ __forceinline__ void prefetch_tmap(const CUtensorMap* map) {
 }
 
 // TMEM
-__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {
-  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
-  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
-  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
-}
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-// tcgen05.commit: arrive on an mbarrier when all prior tcgen05 ops of this thread are done
-__device__ __forceinline__ void tc_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
-// dense FP8 MMA: D[tmem] (+)= A[smem] * B[smem]^T   (SASS: UTCQMMA)
-__device__ __forceinline__ void mma_f8_dense(uint32_t d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f8f6f4 [%0], %1, %2, %3, p;\n\t}"
-      ::"r"(d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
-}
-// 2:4 sparse FP8 MMA: A is compressed (K = 64 logical per instruction), metadata in TMEM at `e`
-__device__ __forceinline__ void mma_f8_sparse(uint32_t d, uint64_t adesc, uint64_t bdesc, uint32_t e, uint32_t idesc, uint32_t acc) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %5, 0;\n\t"
-      "tcgen05.mma.sp.cta_group::1.kind::f8f6f4 [%0], %1, %2, [%3], %4, p;\n\t}"
-      ::"r"(d), "l"(adesc), "l"(bdesc), "r"(e), "r"(idesc), "r"(acc) : "memory");
-}
-// shared -> TMEM copy of one metadata atom: 128 lanes x 128 bit (SASS: UTCCP)
-__device__ __forceinline__ void tc_cp_128x128b(uint32_t taddr, uint64_t sdesc) {
-  asm volatile("tcgen05.cp.cta_group::1.128x128b [%0], %1;" ::"r"(taddr), "l"(sdesc) : "memory");
-}
 // ---- CTA-pair (cta_group::2) forms: one thread of the leader CTA issues for both CTAs; A = 128 rows from each CTA
 // (same smem offset), B = N/2 rows from each, D = 128 lanes x N columns in each CTA's TMEM, metadata per CTA
 __device__ __forceinline__ void tmem_alloc_pair(uint32_t smem_dst, uint32_t ncols) {   // one warp of EACH CTA, same smem offset
@@ -392,6 +344,7 @@ int launch_pack(const spense_shape_t* shape, const uint8_t* d_wgate, const uint8
                 int64_t* h_err_where, cudaStream_t stream);
 int launch_pack_linear(const spense_linear_shape_t* shape, const uint8_t* d_w, float w_scale, const int32_t* d_perm, void* d_blob,
                        const spense_linear_canon_t* canon, void* d_ws, int64_t* h_err_where, cudaStream_t stream);
+int prepare_gemm_kernels(int dev);
 int launch_gemm(const GemmParams& p, const CUtensorMap& tmap_b, const CUtensorMap& tmap_ws, const CUtensorMap& tmap_wd, bool pdl, int dev,
                 cudaStream_t stream);
 int launch_requant_rows(const float* d_h, int rows, int cols, const float* d_amax_part, int n_part, int part_stride,
@@ -401,6 +354,7 @@ int launch_select(const spense_shape_t* shape, const float* d_wgate, const float
                   int32_t* d_perm, void* d_ws, cudaStream_t stream);
 int launch_prune(const spense_shape_t* shape, float* d_wgate, float* d_wup, float* d_wdown, const int32_t* d_perm, cudaStream_t stream);
 int launch_prune_obs(int N, int K, int K_sparse, float* d_w, const float* d_u, void* d_ws, cudaStream_t stream);
+int launch_read_probe(const void* d_buf, size_t bytes, uint32_t* d_sink, int sms, cudaStream_t stream);
 int launch_quantize(const float* d_in, int64_t rows, int64_t cols, int32_t mode, uint8_t* d_out, float* d_scales,
                     void* d_ws, cudaStream_t stream);
 

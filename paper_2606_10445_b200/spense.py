@@ -27,7 +27,7 @@ EXPORTS = ["spense_version", "spense_strerror", "spense_device_status", "spense_
            "spense_mlp_dyn", "spense_mlp_host", "spense_mlp_stack_host", "spense_quantize_e4m3", "spense_prune_2to4_magnitude", "spense_dense_idx_last", "spense_select_workspace_size",
            "spense_select_dense", "spense_linear_pack_sizes", "spense_pack_linear", "spense_linear_workspace_size",
            "spense_linear_out_split", "spense_linear_in_split", "spense_prune_obs_workspace_size", "spense_prune_obs_2to4",
-           "spense_quantize_e4m3_static"]
+           "spense_quantize_e4m3_static", "spense_probe_read"]
 
 SPENSE_SPLIT_OUT, SPENSE_SPLIT_IN = 0, 1
 SPENSE_QUANTIZE_STATIC_MAX_ROWS = 65536
@@ -102,6 +102,7 @@ def lib() -> ctypes.CDLL:
         L.spense_quantize_e4m3.argtypes = [c_void_p, c_int64, c_int64, c_int32, c_void_p, c_void_p, c_void_p,
                                            c_size_t, c_void_p]
         L.spense_quantize_e4m3_static.argtypes = [c_void_p, c_int64, c_int64, c_int32, c_void_p, c_void_p, c_void_p]
+        L.spense_probe_read.argtypes = [c_void_p, c_size_t, c_void_p, c_void_p]
         L.spense_linear_pack_sizes.argtypes = [POINTER(LinearShape), POINTER(c_size_t), POINTER(c_size_t)]
         L.spense_pack_linear.argtypes = [POINTER(LinearShape), c_void_p, c_float, c_void_p, c_void_p, c_size_t, POINTER(LinearCanon),
                                          c_void_p, c_size_t, POINTER(c_int64), c_void_p]
@@ -351,6 +352,16 @@ def spense_quantize_e4m3_static(x: torch.Tensor, mode: int, out: torch.Tensor, s
         raise ValueError("scales must be a contiguous fp32 tensor of rows (per row) or 1 (per tensor) elements on x's device")
     _check(lib().spense_quantize_e4m3_static(_ptr(x), rows, cols, mode, _ptr(out), _ptr(scales), _stream()))
     return out, scales
+
+
+def spense_probe_read(buf: torch.Tensor, sink: torch.Tensor = None):
+    """Stream `buf` (uint8, CUDA, a multiple of 32768 bytes) through the SMs the way the GEMM streams weights and discard
+    it; time it with events for the read-only HBM ceiling.  Returns the 256-word sink (XOR of one word per chunk, per CTA)."""
+    _dev(buf, torch.uint8)
+    if sink is None:
+        sink = torch.zeros(256, dtype=torch.int32, device=buf.device)
+    _check(lib().spense_probe_read(_ptr(buf), buf.numel(), _ptr(sink), _stream()))
+    return sink
 
 
 def spense_select_dense(wgate, wup, wdown, hdiag_x, hdiag_h, I_dense: int, eps: float = 1e-8):

@@ -34,10 +34,17 @@ def test_mlp_dyn_parity(sp, H, I, p, M):
         c.x[1] = 0
     if M > 4:                                            # a token whose h is ~1e-37: s_h = amax / 448 is below 2^-128 and has
         c.s_x = c.s_x.clone()                            # no finite fp32 reciprocal (the quotients must still be IEEE's)
-        c.s_x[3] = 3e-19
+        c.s_x[3] = 1e-20
     pk = c.pack_gpu(sp)
     ws = sp.spense_workspace(pk, M)
     ref = o.mlp_dynamic(c.x.numpy(), c.s_x.numpy(), c.wg, c.wu, c.wd, c.L.w_scale)
+    if M > 4:                                            # h ~ s_x^2: steer the row's scale into (2^-138, 2^-129)
+        for _ in range(4):
+            if 2.0 ** -138 < ref["s_h"][3] < 2.0 ** -129:
+                break
+            c.s_x[3] *= float(np.sqrt(2.0 ** -133 / max(float(ref["s_h"][3]), 1e-45)))
+            ref = o.mlp_dynamic(c.x.numpy(), c.s_x.numpy(), c.wg, c.wu, c.wd, c.L.w_scale)
+        assert 2.0 ** -138 < ref["s_h"][3] < 2.0 ** -129, ref["s_h"][3]
     y, s_h, hq, h = sp.spense_mlp_dyn(pk, cuda(c.x), cuda(c.s_x), ws)
     torch.cuda.synchronize()
     h_gpu, hq_gpu, sh_gpu, y_gpu = h.cpu().numpy(), hq.cpu().numpy(), s_h.cpu().numpy(), y.cpu().numpy()

@@ -278,6 +278,33 @@ def test_first_call_on_a_fresh_blob_inside_stream_capture(sp, M):
     assert_down_parity(y.cpu().numpy(), hq.cpu().numpy(), s_h, c2.wd, c2.L.w_scale[2], "replay after the blob was replaced in place")
 
 
+def test_first_call_in_a_fresh_process_is_capturable(sp, tmp_path):
+    """A process that loads a pre-packed blob and never calls spense_pack: its first spense_mlp, captured under torch's
+    default global capture mode, must not need any set-up that is illegal during capture (spense_workspace_init did it).
+    The child's replayed hq and y equal this process's eager result bit for bit."""
+    import os
+    import subprocess
+    import sys
+    M = 40
+    c = Case(256, 1024, 0.25, M, seed=4300)
+    pk = c.pack_gpu(sp)
+    s_h = torch.from_numpy(c.default_s_h())
+    ws = sp.spense_workspace(pk, M)
+    hq = torch.zeros(M, c.I, dtype=torch.uint8, device="cuda")
+    y = sp.spense_mlp(pk, cuda(c.x), cuda(c.s_x), cuda(s_h), ws, hq_scratch=hq)
+    torch.cuda.synchronize()
+    d = str(tmp_path)
+    torch.save(torch.tensor([c.H, c.I, c.I_d, M]), f"{d}/meta.pt")
+    torch.save(pk.blob.cpu(), f"{d}/blob.pt")
+    for n, t in (("x", c.x), ("sx", c.s_x), ("sh", s_h)):
+        torch.save(t, f"{d}/{n}.pt")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-m", "tests.capture_child", d], cwd=root, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-4000:]
+    out = torch.load(f"{d}/out.pt")
+    assert torch.equal(out["hq"], hq.cpu()) and torch.equal(out["y"], y.cpu())
+
+
 def test_mlp_host_buffers_equal_device_call(sp):
     """spense_mlp_host (HOST pinned x, scales and y; copies inside the call) == spense_mlp on device buffers."""
     H, I, p, M = 640, 896, 0.43, 48

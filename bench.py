@@ -41,6 +41,21 @@ def algorithmic_bytes(M: int, h: int, i: int, i_d: int) -> int:
     return int(w + act)
 
 
+NOMINAL_HBM_GBS = 8000.0     # north_star: "against the ~8 TB/s peak"
+
+
+def blob_bytes_of(h: int, i: int, i_d: int) -> int:
+    return 1024 + int(3 * h * (i_d + (i - i_d) * 0.625))
+
+
+def config_of(M: int, i_d: int, world: int) -> dict:
+    """The workload both arms report (the reference arm times a bounded sample of it, named in its cpu_baseline.sample)."""
+    return {"workload": f"qwen3_32b_mlp_layer H={H} I={I} p=25% (I_dense={i_d}) M={M}",
+            "layers_per_step": LAYERS, "launch": "CUDA graph of LAYERS x spense_mlp (2 PDL-chained kernels each)",
+            "l2": f"inputs larger than L2: {LAYERS} distinct packed layers = {LAYERS * blob_bytes_of(H, I, i_d) / 1e9:.2f} GB rotate",
+            "parallelism": "replicas only" if world > 1 else "single GPU"}
+
+
 def read_peaks():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
@@ -138,11 +153,11 @@ def oracle_layer(M: int):
     x, sx = si.make_activations(M, H, seed=1000 + M)
     c = o.pack_canonical(L.wgate.cpu().numpy(), L.wup.cpu().numpy(), L.wdown.cpu().numpy(), L.perm.cpu().numpy(), L.I_dense)
     wg, wu, wd = o.unpack_canonical(c)
-    w_scale = L.w_scale
+    w_scale, i_d = L.w_scale, int(L.I_dense)
     del L, c
     if dev == "cuda":
         torch.cuda.empty_cache()
-    return dict(o=o, x=x.numpy(), sx=sx.numpy(), wg=wg, wu=wu, wd=wd, w_scale=w_scale, s_h=np.full(M, 0.05, np.float32))
+    return dict(o=o, x=x.numpy(), sx=sx.numpy(), wg=wg, wu=wu, wd=wd, w_scale=w_scale, s_h=np.full(M, 0.05, np.float32), I_dense=i_d)
 
 
 def oracle_time_layer(ol, reps: int):
@@ -172,20 +187,24 @@ def run_reference(args):
     import torch
     ol = oracle_layer(args.M)
     t_start = time.perf_counter()
-    for _ in range(min(args.warmup, 2)):
+    n_warm = 0
+    for _ in range(args.warmup):                          # the requested warm-up (each step is ~2 s of host work)
         oracle_time_layer(ol, 1)
+        n_warm += 1
+        if time.perf_counter() - t_start > 60:
+            break
     steps = []
     for _ in range(args.steps):
         steps.append(oracle_time_layer(ol, 1))
-        if time.perf_counter() - t_start > 150:
+        if time.perf_counter() - t_start > 200:
             break
     v = sum(steps) / len(steps) * 1e6
     sample = (f"oracle.mlp on ONE full-size layer per step (H={H}, I={I}, p=25 %, M={args.M}), {len(steps)} timed steps; "
               f"ms_per_step is that one layer, not {LAYERS}")
     line = {"impl": "reference", "metric": "spense_fp8_mlp_us_per_layer", "value": v, "unit": "us/layer",
-            "n_gpus": args.gpus, "steps": len(steps), "warmup": min(args.warmup, 2), "ms_per_step": v / 1e3,
+            "n_gpus": args.gpus, "steps": len(steps), "warmup": n_warm, "ms_per_step": v / 1e3,
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"qwen3_32b_mlp_layer H={H} I={I} p=25% M={args.M}", "layers_per_step": 1},
+            "config": config_of(args.M, ol["I_dense"], 1 if args.gpus <= 1 else args.gpus),
             "cpu_baseline": {"value": v, "unit": "us/layer", "cores": int(torch.get_num_threads() or os.cpu_count()), "kind": "oracle",
                              "sample": sample},
             "e2e": {"value": v, "unit": "us/layer", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -241,6 +260,32 @@ def event_time_ms(replay, steps, warmup, dist=None, replicas=None, dev=None, hos
         ms = replicas.max_over_ranks(ms, dist, dev)
         dist.barrier()
     return ms / steps
+
+
+def hbm_probes(sp, dev, timed, sustained_s: float):
+    """SURVEY.md 8d "time floors", measured in THIS run on THIS box: (a) the read-only stream ceiling (spense_probe_read: the
+    GEMM's own bulk-copy producer with nothing behind it, 4 GiB per call >> L2), best of 10 single calls (burst, like
+    MEASURED_PEAKS.json's copy figure) and back to back for sustained_s seconds; (b) torch's b.copy_(a) over 2 x 2 GiB
+    (read + write bytes) back to back for sustained_s seconds, the sustained twin of MEASURED_PEAKS.json's hbm_gbs."""
+    import torch
+    n = 4 << 30
+    buf = torch.empty(n, dtype=torch.uint8, device=dev)
+    buf.view(torch.int64).random_()
+    sink = torch.zeros(256, dtype=torch.int32, device=dev)
+    call = lambda: sp.spense_probe_read(buf, sink)
+    best = min(timed(call, 1, 2 if k == 0 else 0) for k in range(10))
+    out = {"read_probe_gbs": round(n / best / 1e6, 1), "read_probe_bytes": n}
+    if sustained_s > 0:
+        reps = max(10, int(sustained_s / (best * 1e-3)))
+        out["read_probe_sustained_gbs"] = round(n / timed(call, reps, 2) / 1e6, 1)
+        a, b = buf[: n // 2], buf[n // 2:]
+        t_copy = min(timed(lambda: b.copy_(a), 1, 2 if k == 0 else 0) for k in range(10))
+        out["copy_gbs"] = round(n / t_copy / 1e6, 1)                     # n/2 read + n/2 written
+        reps = max(10, int(sustained_s / (t_copy * 1e-3)))
+        out["copy_sustained_gbs"] = round(n / timed(lambda: b.copy_(a), reps, 2) / 1e6, 1)
+    del buf
+    torch.cuda.empty_cache()
+    return out
 
 
 def fp8_dense_peak(sp, si, dev, dense_blobs, ws):
@@ -419,6 +464,7 @@ def main():
             sp.spense_mlp(b, xx, ssx, ssh, wsp, hq_scratch=hqq, y=yy, next_layer=layers[(i + 1) % len(layers)])
 
     timed = lambda replay, steps, wu, hw=None: event_time_ms(replay, steps, wu, dist, replicas, dev, hw)
+    timed_local = lambda replay, steps, wu: event_time_ms(replay, steps, wu)     # rank-0-only extras: no barrier, no all-reduce
 
     g_main = graph_of(lambda: step_eager(blobs, x, sx, sh, hq, y))
     sampler = ClockSampler(local)
@@ -457,9 +503,10 @@ def main():
     if sustained is not None:
         sustained["hbm_gbs"] = algo / (sustained["value"] * world * 1e-6) / 1e9
         sustained["frac"] = sustained["hbm_gbs"] / peak
+    probes = None
     if rank == 0:
         def t_us(fn, n=LAYERS):
-            return timed(graph_of(fn).replay, 20, 5) * 1e3 / n
+            return timed_local(graph_of(fn).replay, 20, 5) * 1e3 / n
         extras["gate_up_us"] = t_us(lambda: [sp.spense_gate_up(b, x, sx, sh, ws, hq=hq) for b in blobs])
         extras["down_us"] = t_us(lambda: [sp.spense_down(b, hq, sh, ws, y=y) for b in blobs])
         # NEXT-1: the same layers with dynamic per-token requant (gate_up -> row requant kernel -> down)
@@ -472,7 +519,7 @@ def main():
             # configs[1]: M sweep, Spense vs the all-dense kernel
             sweep = []
             dense = make_blobs(sp, si, dev, H, I, 1.0, 6, 3000)
-            for Ms in (1, 8, 32, 64, 128, 256):
+            for Ms in (1, 8, 32, 64, 128, 160, 192, 240, 256):
                 xs, sxs = si.make_activations(Ms, H, 1000 + Ms, device=dev)
                 shs = torch.full((Ms,), 0.05, device=dev)
                 hqs = torch.empty(Ms, I, dtype=torch.uint8, device=dev)
@@ -509,6 +556,13 @@ def main():
                                               "gbs": round(a50 / row[0.5][0] / 1e3, 1),
                                               "frac_of_hbm_peak": round(a50 / row[0.5][0] / 1e3 / peak, 3)}
 
+        # the HBM ceilings of this box in this run (after the decode rows, which seconds of full-rate streaming would heat;
+        # before the tensor-bound prefill rows)
+        probes = hbm_probes(sp, dev, timed_local, args.sustained_s)
+        if sustained is not None and probes.get("copy_sustained_gbs"):
+            sustained["frac_of_sustained_copy"] = sustained["hbm_gbs"] / probes["copy_sustained_gbs"]
+            sustained["frac_of_sustained_read_probe"] = sustained["hbm_gbs"] / probes["read_probe_sustained_gbs"]
+        if not args.no_sweep:
             # configs[4]: prefill-shaped GEMMs against the FP8 dense peak MEASURED on this box
             dense = make_blobs(sp, si, dev, H, I, 1.0, 1, 3000)
             extras["fp8_peak"] = fp8_dense_peak(sp, si, dev, dense, ws)
@@ -526,14 +580,14 @@ def main():
             "metric": "spense_fp8_mlp_us_per_layer", "value": replicas.whole_job_us_per_layer(ms_step, LAYERS, world), "unit": "us/layer",
             "n_gpus": world, "steps": args.steps, "warmup": warmup, "ms_per_step": ms_step,
             "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f8e4m3", "data": "synthetic",
-            "config": {"workload": f"qwen3_32b_mlp_layer H={H} I={I} p=25% (I_dense={I_d}) M={M}",
-                       "layers_per_step": LAYERS, "launch": "CUDA graph of LAYERS x spense_mlp (2 PDL-chained kernels each)",
-                       "l2": f"inputs larger than L2: {LAYERS} distinct packed layers = {LAYERS * (blobs[0].blob.numel()) / 1e9:.2f} GB rotate",
-                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "config": config_of(M, I_d, world),
             "hbm_gbs": achieved,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": traffic_from_profile(M), "traffic_source": os.path.relpath(TRAFFIC_CSV, ROOT) if M == TRAFFIC_M else None,
                          "peak_source": peak_src,
+                         "peak_read_gbs": probes["read_probe_gbs"], "frac_of_read_probe": achieved / probes["read_probe_gbs"],
+                         "nominal_gbs": NOMINAL_HBM_GBS, "frac_of_nominal": achieved / NOMINAL_HBM_GBS,
+                         "probes": probes,
                          "kernel": "spense_gemm_kernel (gate_up + down launches of one layer)",
                          "algorithmic_bytes_per_layer": algo},
             "sustained": sustained,

@@ -106,3 +106,23 @@ def test_quantize_helper_bit_exact(sp):
         rq, rs = ref(x.numpy())
         assert np.array_equal(s.cpu().numpy().reshape(-1), np.asarray(rs, np.float32).reshape(-1))
         assert np.array_equal(q.cpu().numpy(), rq)
+
+
+def test_read_probe_reads_every_chunk(sp):
+    """spense_probe_read (measurement helper): each CTA's sink word is the XOR of one word of every 32 KB chunk it was dealt
+    (chunk c -> CTA c % grid, word at byte (4 c) % 32768 of the chunk) -- recomputed here from the buffer."""
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    for n_chunks in (5, sms, 6 * sms + 17, 2048 + 5):           # fewer chunks than CTAs, one each, a ragged last ring pass, many
+        buf = torch.empty(n_chunks * 32768, dtype=torch.uint8, device="cuda")
+        buf.view(torch.int64).random_()
+        sink = sp.spense_probe_read(buf)
+        torch.cuda.synchronize()
+        words = buf.cpu().numpy().view(np.uint32).reshape(n_chunks, 8192)
+        grid = min(sms, n_chunks)
+        want = np.zeros(256, np.uint32)
+        for c in range(n_chunks):
+            want[c % grid] ^= words[c, c % 8192]
+        assert np.array_equal(sink.cpu().numpy().view(np.uint32), want), n_chunks
+    with pytest.raises(sp.SpenseError) as e:
+        sp.spense_probe_read(torch.empty(32768 + 128, dtype=torch.uint8, device="cuda"))
+    assert e.value.code == "SPENSE_ERR_ARG"

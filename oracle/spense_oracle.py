@@ -183,7 +183,7 @@ def prune_2to4_magnitude(wgate, wup, wdown, perm, I_dense: int):
     return wgate, wup, wdown
 
 
-def sparsegpt_2to4(w, hinv, k_sparse: int):
+def sparsegpt_2to4(w, hinv, k_sparse: int, on_group=None):
     """NEXT-4: SparseGPT's 2:4 column sweep with the dense columns on the right as compensation buffer (PAPER.md:98-111,
     Eqs. 2-3; PAPER.md:149-153 "placing dense columns on the right keeps them available as a compensation buffer";
     PAPER.md:202 "apply SparseGPT ... to the sparse regions while protecting the selected dense indices").
@@ -203,7 +203,9 @@ def sparsegpt_2to4(w, hinv, k_sparse: int):
         the lower column is pruned first);
       * a marked weight w_m is removed with Eq. 3: w += delta_m = -w_m / [Hi]_mm * Hi[m, :] over the unprocessed
         columns (which makes w_m itself exactly 0); an unmarked weight is kept as it is.
-    Columns >= k_sparse are never pruned: they only receive compensation.  Returns (w_new, pruned_mask)."""
+    Columns >= k_sparse are never pruned: they only receive compensation.  Returns (w_new, pruned_mask).
+    on_group (test hook, no arithmetic of its own): called as on_group(j, eps, d) with the [N, 4] criterion values the
+    group starting at column j was decided on and the 4 diagonal entries [Hi_c]_cc they were divided by."""
     W = np.array(w, dtype=np.float64, copy=True)
     N, K = W.shape
     assert 0 <= k_sparse <= K and k_sparse % 4 == 0
@@ -217,6 +219,8 @@ def sparsegpt_2to4(w, hinv, k_sparse: int):
                 d[c] = blk[c, c]
                 blk[c + 1:, c + 1:] -= np.outer(blk[c + 1:, c], blk[c, c + 1:]) / blk[c, c]
             eps = W[:, j:j + 4] ** 2 / d[None, :]
+            if on_group is not None:
+                on_group(j, eps, d)
             order = np.argsort(eps, axis=1, kind="stable")    # stable: ties -> the lower column first
             for r in range(N):
                 pruned[r, j + order[r, 0]] = True

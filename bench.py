@@ -346,30 +346,20 @@ def prefill_rows(sp, si, dev, blobs, ws, fp8_peak_tflops):
     return rows
 
 
-def run_report(args):
-    """--report: the other BASELINE.json configs in full (context rows, not the bench line): Seed-OSS-36B shape
-    dense-fraction sweep, the 64-layer Qwen3-32B-shaped stack, prefill-shaped GEMMs.  Writes one JSON object to stdout
-    and to gpurun_out/report.json.  Same timing rules as the bench line."""
+def w_bytes(h, i, i_d):
+    return 3 * h * (i_d + (i - i_d) * 0.625)
+
+
+def seed_sweep_rows(sp, si, dev, peak, ps=(1.0, 0.0, 0.10, 0.25, 0.50), ms=(1, 16, 64, 256), nl=5):
+    """BASELINE.json configs[2]: Seed-OSS-36B-shaped layer, dense fraction x token count, speedup vs the all-dense kernel
+    (p = 1.0 must come first: its times are the denominators)."""
     import torch
-    import spense_inputs as si
-    from paper_2606_10445_b200 import build, spense as sp
-    build.build()
-    dev = torch.device("cuda", 0)
-    torch.cuda.set_device(dev)
-    peak, bf16_peak, _ = read_peaks()
-    out = {"hbm_peak_gbs": peak}
-
-    def w_bytes(h, i, i_d):
-        return 3 * h * (i_d + (i - i_d) * 0.625)
-
-    # ---- config 3: Seed-OSS-36B-shaped layer, p sweep x M sweep, speedup vs the all-dense kernel
     rows, dense_t = [], {}
-    for p in (1.0, 0.0, 0.10, 0.25, 0.50):
-        nl = 5
+    for p in ps:
         bl = make_blobs(sp, si, dev, SEED_H, SEED_I, p, nl, 4000 + int(p * 100) * 10)
         i_d = bl[0].I_dense
         ws = sp.spense_workspace(bl[0], 256)
-        for m in (1, 16, 64, 256):
+        for m in ms:
             x, sx = si.make_activations(m, SEED_H, 1000 + m, device=dev)
             sh = torch.full((m,), 0.05, device=dev)
             hq = torch.empty(m, SEED_I, dtype=torch.uint8, device=dev)
@@ -384,14 +374,17 @@ def run_report(args):
                          "byte_ratio_bound": round(w_bytes(SEED_H, SEED_I, SEED_I) / w_bytes(SEED_H, SEED_I, i_d), 3)})
         del bl, ws
         torch.cuda.empty_cache()
-    out["seed_oss_36b_sweep"] = rows
+    return rows
 
-    # ---- config 4: 64 consecutive Qwen3-32B-shaped layers (18 GB of blobs), one CUDA graph, tokens/s
-    nl = 64
-    bl = make_blobs(sp, si, dev, H, I, P_DENSE, nl, 6000)
-    ws = sp.spense_workspace(bl[0], 8192)
+
+def stack_rows(sp, si, dev, peak, bl, ws, ms=(32, 128)):
+    """BASELINE.json configs[3]: 64 consecutive Qwen3-32B-shaped layers (18 GB of blobs) in one CUDA graph, tokens/s.
+    Every layer reads the same x (the layers are chained through the stream, not through data: the paper's method has
+    nothing between two MLPs; the data-chained variant with a normalise-and-quantise kernel is not built)."""
+    import torch
+    nl = len(bl)
     stack = []
-    for m in (32, 128):
+    for m in ms:
         x, sx = si.make_activations(m, H, 1000 + m, device=dev)
         sh = torch.full((m,), 0.05, device=dev)
         hq = torch.empty(m, I, dtype=torch.uint8, device=dev)
@@ -402,7 +395,63 @@ def run_report(args):
         stack.append({"M": m, "layers": nl, "ms_per_stack": round(t / 1e3, 4), "us_per_layer": round(t / nl, 2),
                       "tokens_per_s": round(m / (t * 1e-6), 1), "gbs": round(algo / t / 1e3, 1),
                       "frac_of_hbm_peak": round(algo / t / 1e3 / peak, 3)})
-    out["qwen3_32b_stack"] = stack
+    return stack
+
+
+def obs_rows(sp, dev):
+    """NEXT-4, spense_prune_obs_2to4 on the two Qwen3-32B shapes (the sparse rows of gate / up along H; down along the
+    permuted intermediate dimension with the 6400 dense columns as buffer): ms per sweep (best of 3, events) and the
+    trailing update's flops (2 N 128 (K - j1) per 128-column block) over that time.  Synthetic weights N(0, 0.02^2);
+    U = upper Cholesky factor of the inverse of a damped Gram matrix of K / 2 random samples (float64 library routines)."""
+    import torch
+    rows = []
+    for name, n, k, ks in (("gate_or_up_sparse_rows", I - int(I * P_DENSE), H, H), ("down", H, I, I - int(I * P_DENSE))):
+        g = torch.Generator(device=dev).manual_seed(k)
+        xs = torch.randn(k // 2, k, device=dev, generator=g)
+        hm = (xs.t() @ xs).double()
+        del xs
+        hm += 0.01 * hm.diagonal().mean() * torch.eye(k, device=dev, dtype=torch.float64)
+        hinv = torch.cholesky_inverse(torch.linalg.cholesky(hm))
+        del hm
+        u = torch.linalg.cholesky(hinv, upper=True).float().contiguous()
+        del hinv
+        w0 = torch.randn(n, k, device=dev, generator=g) * 0.02
+        w = torch.empty_like(w0)
+        best = None
+        for _ in range(3):
+            w.copy_(w0)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            sp.spense_prune_obs_2to4(w, u, ks)                       # in place on w
+            e1.record()
+            torch.cuda.synchronize()
+            best = e0.elapsed_time(e1) if best is None else min(best, e0.elapsed_time(e1))
+        ok = bool(((w[:, :ks].view(n, ks // 4, 4) == 0).sum(dim=2) == 2).all())
+        flops = sum(2.0 * n * min(128, ks - j0) * (k - min(j0 + 128, ks)) for j0 in range(0, ks, 128))
+        rows.append({"matrix": name, "N": n, "K": k, "K_sparse": ks, "ms": round(best, 2), "two_of_four_holds": ok,
+                     "trailing_update_tflops": round(flops / best / 1e9, 2), "arithmetic": "fp32 CUDA cores"})
+        del u, w, w0
+        torch.cuda.empty_cache()
+    return rows
+
+
+def run_report(args):
+    """--report: the other BASELINE.json configs in full (context rows, not the bench line): Seed-OSS-36B shape
+    dense-fraction sweep, the 64-layer Qwen3-32B-shaped stack, prefill-shaped GEMMs, the SparseGPT sweep's timing.
+    Writes one JSON object to stdout and to gpurun_out/report.json.  Same timing rules as the bench line."""
+    import torch
+    import spense_inputs as si
+    from paper_2606_10445_b200 import build, spense as sp
+    build.build()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peak, bf16_peak, _ = read_peaks()
+    out = {"hbm_peak_gbs": peak}
+    out["seed_oss_36b_sweep"] = seed_sweep_rows(sp, si, dev, peak)
+    bl = make_blobs(sp, si, dev, H, I, P_DENSE, 64, 6000)
+    ws = sp.spense_workspace(bl[0], 8192)
+    out["qwen3_32b_stack"] = stack_rows(sp, si, dev, peak, bl, ws)
 
     # ---- config 5: prefill-shaped GEMMs against the measured FP8 dense peak
     dense = make_blobs(sp, si, dev, H, I, 1.0, 1, 3000)
@@ -410,6 +459,9 @@ def run_report(args):
     del dense
     fp8 = out["fp8_peak"].get("scaled_mm_8192_tflops") or 2 * bf16_peak
     out["prefill_shaped"] = prefill_rows(sp, si, dev, bl, ws, fp8)
+    del bl, ws
+    torch.cuda.empty_cache()
+    out["obs_sweep"] = obs_rows(sp, dev)
     os.makedirs(os.path.join(ROOT, "gpurun_out"), exist_ok=True)
     with open(os.path.join(ROOT, "gpurun_out", "report.json"), "w") as f:
         json.dump(out, f, indent=1)
@@ -555,6 +607,14 @@ def main():
                                               "speedup_vs_dense": round(row[1.0][0] / row[0.5][0], 3), "byte_ratio_bound": 1.231,
                                               "gbs": round(a50 / row[0.5][0] / 1e3, 1),
                                               "frac_of_hbm_peak": round(a50 / row[0.5][0] / 1e3 / peak, 3)}
+
+        if not args.no_sweep:
+            # configs[2] in full (dense fraction x token count) and configs[3] (the 64-layer stack), as in --report
+            extras["seed_oss_36b_sweep"] = seed_sweep_rows(sp, si, dev, peak, nl=4)
+            bl64 = blobs + make_blobs(sp, si, dev, H, I, P_DENSE, 64 - LAYERS, 6000)
+            extras["qwen3_32b_stack"] = stack_rows(sp, si, dev, peak, bl64, ws)
+            del bl64
+            torch.cuda.empty_cache()
 
         # the HBM ceilings of this box in this run (after the decode rows, which seconds of full-rate streaming would heat;
         # before the tensor-bound prefill rows)

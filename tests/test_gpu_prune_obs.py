@@ -41,7 +41,14 @@ def check_against_oracle(sp, N, K, ks, seed):
     got = sp.spense_prune_obs_2to4(torch.from_numpy(w).cuda(), torch.from_numpy(U).cuda(), ks).cpu().numpy()
     torch.cuda.synchronize()
     U64 = U.astype(np.float64)
-    ref, pruned = o.sparsegpt_2to4(w, U64.T @ U64, ks)          # the oracle sees exactly the fp32 factor the GPU got
+    eps_all = np.empty((N, ks // 4, 4))                         # the criterion values every group was decided on
+
+    d_all = np.empty((ks // 4, 4))                              # and the diagonals [Hi_c]_cc of Eq. 3 behind them
+
+    def keep_eps(j, eps, d):
+        eps_all[:, j // 4] = eps
+        d_all[j // 4] = d
+    ref, pruned = o.sparsegpt_2to4(w, U64.T @ U64, ks, on_group=keep_eps)   # the oracle sees exactly the fp32 factor the GPU got
     # unique: Eq. 1 holds on the sparse region, exactly 2 pruned per group; the dense columns hold no forced zeros
     gz = (got[:, :ks] == 0).reshape(N, ks // 4, 4)
     assert (gz.sum(axis=2) == 2).all()
@@ -50,10 +57,29 @@ def check_against_oracle(sp, N, K, ks, seed):
     same_group = (gz == pruned[:, :ks].reshape(N, ks // 4, 4)).all(axis=2)
     assert same_group.mean() > 0.999, same_group.mean()
     rows = same_group.all(axis=1)
-    assert rows.mean() > 0.9
+    assert rows.mean() > (0.9 if ks <= 1024 else 0.5)          # a long row has many groups to meet a near-tie in
     err = np.abs(got[rows].astype(np.float64) - ref[rows])
     scale = np.abs(ref[rows]).max(axis=1, keepdims=True)
     assert (err <= 2e-3 * scale + 1e-7).all(), (err / scale).max()
+    # rows whose masks differ somewhere, checked group by group: up to the first differing group the row followed the
+    # oracle (frozen columns equal within tolerance), and AT that group the GPU's choice is a valid one -- the eps (Eq. 3)
+    # of what it pruned exceed the eps of what it kept by no more than a weight error of 1e-4 of the row's scale moves them
+    worst = 0.0
+    for r in np.where(~rows)[0]:
+        g0 = int(np.argmin(same_group[r]))
+        c0 = 4 * g0
+        sc = np.abs(ref[r]).max()
+        assert (np.abs(got[r, :c0].astype(np.float64) - ref[r, :c0]) <= 2e-3 * sc + 1e-7).all(), (r, g0)
+        e, gp, d = eps_all[r, g0], gz[r, g0], d_all[g0]
+        a = np.where(gp)[0][np.argmax(e[gp])]                   # the GPU pruned a although it kept b with a smaller eps
+        b = np.where(~gp)[0][np.argmin(e[~gp])]
+        gap = e[a] - e[b]
+        # eps = w^2 / d, so a weight error dw moves it by 2 sqrt(eps / d) dw + dw^2 / d; dw = 1e-4 of the row's scale
+        dw = 1e-4 * sc
+        allow = sum(2 * np.sqrt(e[c] / d[c]) * dw + dw * dw / d[c] for c in (a, b))
+        worst = max(worst, gap / allow)
+        assert gap <= allow, (r, g0, e, gp)
+    print(f"[obs] N={N} K={K} ks={ks}: {int((~rows).sum())} rows differ somewhere, worst eps gap / allowance {worst:.3e}")
     # validity of everything (Eq. 2): the reconstruction loss is the oracle's
     loss = lambda a: np.linalg.norm(X @ (a.astype(np.float64) - w).T) ** 2
     assert abs(loss(got) - loss(ref)) <= 0.01 * loss(ref)
@@ -88,6 +114,19 @@ def test_identity_hessian_is_magnitude_pruning_bit_for_bit(sp):
 def test_obs_mid_size_down_shaped(sp):
     # a down-projection-shaped case: more columns than rows, a quarter of them dense on the right
     check_against_oracle(sp, 256, 1024, 768, seed=9)
+
+
+def test_obs_many_column_blocks(sp):
+    """fp32 error growth over many 128-column blocks, on a sample of rows (rows are independent): a gate/up-shaped sweep
+    (K_sparse = K, 20 blocks) and a down-shaped one whose sweep crosses 24 blocks with 1024 dense columns on the right."""
+    check_against_oracle(sp, 64, 2560, 2560, seed=31)
+    check_against_oracle(sp, 64, 4096, 3072, seed=32)
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("SPENSE_SLOW_TESTS"), reason="5 min of oracle on the host: set SPENSE_SLOW_TESTS=1")
+def test_obs_gate_up_real_reduction_length(sp):
+    """the Qwen3-32B gate/up reduction length, K = K_sparse = 5120 (40 column blocks), 64 rows"""
+    check_against_oracle(sp, 64, 5120, 5120, seed=33)
 
 
 def test_obs_pruned_layer_packs_and_runs(sp):

@@ -30,7 +30,7 @@ SEED_H, SEED_I = 5120, 27648
 LAYERS = 8
 # dram__bytes_read.sum + dram__bytes_write.sum of the GEMM launches of a real step, from the committed ncu
 # application-replay capture of THIS kernel version (profiles/, with the command that made it); keyed by M
-TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_traffic_app_replay_M64.csv")
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r03_traffic_app_replay_M64.csv")
 TRAFFIC_M = 64
 
 
